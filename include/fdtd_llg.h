@@ -1,0 +1,163 @@
+/*
+ * fdtd_llg.h -- C ABI of the B200-native coupled FDTD-LLG time stepper.
+ *
+ * The library advances the second-order coupled Maxwell / Landau-Lifshitz-Gilbert scheme of
+ * Yao, Jambunathan, Zeng, Nonaka, arXiv 2103.12819 (citations: /root/reference/PAPER.md lines)
+ * on ONE GPU (sm_100a), fp64:
+ *
+ *   per time step:   (H,M)^n -> (H,M)^{n+1/2}  with curl E^n       [S3.2.2 Step 1]
+ *                                       E^n -> E^{n+1}            eq. 11              [S3.2.1 Step 2]
+ *                                       (H,M)^{n+1/2} -> (H,M)^{n+1} with curl E^{n+1} [Step 3]
+ *   each (H,M) half-step is the iterated trapezoidal LLG solve of eqs. 18-21
+ *   with |M| = Ms renormalisation and the global stopping test of PAPER.md:154.
+ *
+ * Plain C types only: pointers (each argument says HOST or DEVICE), sizes, PODs.  No torch types.
+ * Every step of the path runs in the library's own CUDA kernels; there is no CPU fallback.
+ *
+ * DATA LAYOUT (all arrays, user side and device side).  nx*ny*nz cells, x fastest, no ghost cells:
+ *   idx = i + nx*(j + ny*k).  Entry (i,j,k) is the edge / face on the LOW side of cell (i,j,k):
+ *     Ex (i+1/2,j,k)  Ey (i,j+1/2,k)  Ez (i,j,k+1/2)             tangential E on edges
+ *     Hx (i,j+1/2,k+1/2)  Hy (i+1/2,j,k+1/2)  Hz (i+1/2,j+1/2,k)  normal H on faces
+ *     M on the x-, y-, z-faces: all three components at every face (9 arrays)
+ *     materials eps_r, sigma, mu_r, Ms, alpha, gamma at cell centres
+ *   Boundaries per axis: FDTD_LLG_PEC or FDTD_LLG_PERIODIC.  On a PEC axis index 0
+ *   is the lower wall, index n (not stored) the upper wall; wall-tangential E, wall-normal H and M on
+ *   wall faces are identically 0.
+ *
+ * ERRORS.  Every call returns FDTD_LLG_OK (0) or a negative code; fdtd_llg_last_error() gives the
+ * text (for a failed create: pass NULL).  Nothing is thrown, nothing aborts.
+ *
+ * THREADING.  A handle may be used by one host thread at a time.
+ */
+#ifndef FDTD_LLG_H
+#define FDTD_LLG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdtd_llg fdtd_llg; /* opaque */
+
+enum {
+  FDTD_LLG_OK = 0,
+  FDTD_LLG_EINVAL = -1, /* bad argument (message says which)                       */
+  FDTD_LLG_ENOMEM = -2, /* workspace too small / host allocation failed            */
+  FDTD_LLG_ECUDA = -3,  /* a CUDA runtime call failed (message has the CUDA text)   */
+  FDTD_LLG_ESTATE = -4  /* call not valid in this state                             */
+};
+
+enum { FDTD_LLG_PEC = 0, FDTD_LLG_PERIODIC = 1 };
+
+/* where a user array lives */
+enum { FDTD_LLG_HOST = 0, FDTD_LLG_DEVICE = 1 };
+
+/* bits of `material_mask`: which material arrays are non-NULL */
+enum {
+  FDTD_LLG_MAT_EPS_R = 1, FDTD_LLG_MAT_SIGMA = 2, FDTD_LLG_MAT_MU_R = 4,
+  FDTD_LLG_MAT_MS = 8, FDTD_LLG_MAT_ALPHA = 16, FDTD_LLG_MAT_GAMMA = 32
+};
+
+typedef struct {
+  int bc[3];          /* per axis x,y,z: FDTD_LLG_PEC / FDTD_LLG_PERIODIC                        */
+  int enable_llg;     /* 0: M = 0 everywhere, plain Maxwell                   */
+  double h_bias[3];   /* uniform static bias H_0, A/m; enters H_eff only           */
+  double ani_hk;      /* uniaxial anisotropy field H_k, A/m; 0 = off.  H_ani = H_k (M.u/Ms) u.
+                         Not in the paper (future work); BASELINE config 4     */
+  double ani_axis[3]; /* unit vector u                                                            */
+  double llg_tol;     /* stop when max |M^r - M^{r-1}|/Ms < tol (paper uses 1e-6)   */
+  int llg_max_iter;   /* iteration cap (the paper has none); at the cap the iterate is accepted   */
+  int use_graph;      /* 1 (default): the step is captured once in a CUDA Graph and replayed      */
+  unsigned scalar_material_mask; /* FDTD_LLG_MAT_* bits: that material pointer addresses ONE double
+                         in HOST memory, the uniform value (no nx*ny*nz array needed)            */
+} fdtd_llg_options;
+
+typedef struct {
+  long long steps;                  /* time steps taken                                        */
+  double time;                      /* steps * dt, s                                           */
+  int iters_last;                   /* LLG iterations of the last (H,M) half-step              */
+  int iters_max;                    /* largest iteration count of any half-step so far         */
+  long long iters_total;            /* sum over all half-steps                                 */
+  long long nonconverged_halfsteps; /* half-steps that hit llg_max_iter with residual >= tol   */
+  double resid_last;                /* max |M^r - M^{r-1}|/Ms of the last executed iteration   */
+  long long halfsteps;              /* (H,M) half-steps taken                                  */
+  double courant;                   /* dt / vacuum Courant limit (>1 is allowed, not an error) */
+  long long kernel_launches;        /* kernels this handle has launched in fdtd_llg_step       */
+  long long magnetic_cells;         /* cells with Ms > 0 (0 when LLG is disabled)              */
+  int launches_per_step;            /* kernel nodes in one captured step                       */
+} fdtd_llg_stats;
+
+/* Fill *opt with the defaults: PEC x3, LLG on, no bias, no anisotropy (axis z), tol 1e-6
+ * (PAPER.md:154), max 20 iterations, graph on. */
+void fdtd_llg_default_options(fdtd_llg_options *opt);
+
+/* Bytes of DEVICE workspace fdtd_llg_create needs for this grid.  `material_mask` = OR of the
+ * FDTD_LLG_MAT_* bits of the material arrays that will be passed non-NULL (a uniform array costs
+ * nothing once detected, so this is an upper bound).  Returns 0 on invalid arguments.
+ * Budget: 6 doubles/cell for E,H; +24/cell when enable_llg (two more H sets for the Jacobi
+ * iterates, M and its time-n copy); +1/cell per material array. */
+size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
+                                unsigned material_mask);
+
+/* Create a simulation (the user supplies CELL-CENTRED material maps).
+ *   nx,ny,nz >= 1; dx,dy,dz,dt > 0 (SI).  dt above the Courant limit is allowed (stats.courant).
+ *   eps_r, sigma, mu_r, Ms, alpha, gamma: nx*ny*nz doubles each, x fastest, in `mem_space`
+ *     (HOST or DEVICE); NULL = uniform default 1, 0, 1, 0, 0, 0; with the material's bit set in
+ *     opt->scalar_material_mask the pointer addresses one HOST double, the uniform value.  Read
+ *     during the call, not retained.  Requirements: eps_r > 0, mu_r > 0, sigma >= 0, Ms >= 0 (else EINVAL).  gamma
+ *     enters only as |gamma| (eqs. 19-20 use |gamma|).  Edge eps, sigma = mean of
+ *     the 4 cells sharing the edge; face Ms, alpha, |gamma|, mu = mean of the 2 cells sharing the
+ *     face, evaluated inside the kernels.  A face is magnetic iff enable_llg,
+ *     Ms_face > 0 and it is not a PEC wall face.
+ *   dev_workspace: DEVICE memory, >= fdtd_llg_workspace_bytes(), 256-byte aligned, owned by the
+ *     caller and kept alive until fdtd_llg_destroy; the library allocates no device memory.
+ *   cuda_stream: a cudaStream_t (NULL = default stream); all work is enqueued on it.
+ * On success *out is the handle and all fields are zero. */
+int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                    double dt, const double *eps_r, const double *sigma, const double *mu_r,
+                    const double *Ms, const double *alpha, const double *gamma, int mem_space,
+                    const fdtd_llg_options *opt, void *dev_workspace, size_t workspace_bytes,
+                    void *cuda_stream);
+
+/* Initial condition.  E[3], H[3]: values directly on their Yee locations; M_cell[3]:
+ * magnetisation at CELL CENTRES, averaged to the faces (two-cell mean) and renormalised to the
+ * face's Ms so that |M| = Ms holds discretely.  The array-of-pointers arguments are HOST arrays of
+ * 3 pointers; the pointed-to data (nx*ny*nz doubles) lives in `mem_space`.  A NULL array or NULL
+ * entry means zero.  Wall-tangential E and wall-normal H are forced to 0.
+ * EINVAL if a magnetic face receives a zero averaged M.  Resets the step counter and statistics.
+ * Synchronises the stream before returning. */
+int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const *H,
+                        const double *const *M_cell, int mem_space);
+
+/* Add a soft current source to eq. 11, envelope of eq. 31:
+ *   J_comp(t) = amplitude * exp(-(t-t0)^2 / (2 tp^2)) * cos(2 pi f0 t) * profile,  t = (n+1/2) dt,
+ * on the comp-edges (comp 0,1,2 = Jx,Jy,Jz) with lo[d] <= index_d < hi[d].  profile: box-sized
+ * ((hi-lo) doubles, x fastest) in `mem_space`, copied; NULL = 1.  Up to 8 sources. */
+int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
+                        const double *profile, int mem_space, double amplitude, double f0,
+                        double t0, double tp);
+
+/* Advance n >= 0 time steps.  Asynchronous: only enqueues work on the stream (n graph launches). */
+int fdtd_llg_step(fdtd_llg *s, int n);
+
+/* Copy the present fields out.  E[3], H[3], M[9] are HOST arrays of pointers (or NULL); each
+ * non-NULL entry receives nx*ny*nz doubles in `mem_space`.  M order: x-face (Mx,My,Mz), y-face
+ * (Mx,My,Mz), z-face (Mx,My,Mz).  Synchronises the stream before returning. */
+int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double *const *M,
+                         int mem_space);
+
+/* Statistics so far (synchronises the stream). */
+int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out);
+
+/* Text of the last error on this handle; with s == NULL, of the last failed fdtd_llg_create on
+ * this thread.  Never NULL. */
+const char *fdtd_llg_last_error(const fdtd_llg *s);
+
+/* Release the handle (host memory, graph).  The workspace stays the caller's.  NULL is a no-op. */
+void fdtd_llg_destroy(fdtd_llg *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDTD_LLG_H */

@@ -1,0 +1,657 @@
+// fdtd_llg.cu -- host side of the C ABI declared in include/fdtd_llg.h.
+//
+// Owns: workspace carve-up, material analysis (uniformity, magnetic bounding box), the static
+// buffer rotation of the Jacobi iterates, and the CUDA Graph of one time step.  All arithmetic of
+// the path is in kernels.cuh.  No device memory is allocated here: everything lives in the
+// caller's workspace.
+#include <climits>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/fdtd_llg.h"
+#include "kernels.cuh"
+
+using namespace fl;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+
+constexpr size_t ALIGN_D = 32;  // arrays start on 256-byte boundaries
+
+size_t padded(size_t n) { return (n + ALIGN_D - 1) / ALIGN_D * ALIGN_D; }
+
+struct MatInfo {
+  bool is_array = false;  // non-uniform: kept on the device
+  double uniform = 0.0;   // value when uniform
+  double *dev = nullptr;
+};
+
+}  // namespace
+
+struct fdtd_llg {
+  GridP g{};
+  double d[3]{}, dt = 0;
+  size_t ncell = 0, stride = 0;  // stride = padded(ncell)
+  fdtd_llg_options opt{};
+  cudaStream_t stream = nullptr;
+  char *ws = nullptr;
+  size_t ws_bytes = 0;
+
+  double *E[3]{};
+  double *Hset[3][3]{};  // three H sets (time-n, ping, pong), statically rotated per half-step
+  double *Mset[2][9]{};  // two M sets
+  MatInfo eps_r, sigma, mu_r, Ms, alpha, gamma;
+  bool llg = false;  // LLG enabled AND at least one magnetic cell
+  long long magnetic_cells = 0;
+  int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
+
+  DevState *dstate = nullptr;
+  unsigned long long *resid = nullptr;
+  double *scratch = nullptr;  // 2*1024 doubles for reductions + 8 ints
+  SourcesP src{};
+  double *profile_pool = nullptr;
+  size_t profile_cap = 0, profile_used = 0;
+
+  cudaGraphExec_t graph = nullptr;
+  bool graph_valid = false;
+  int launches_per_step = 0;
+  long long kernel_launches = 0;
+  long long host_steps = 0;
+  std::string err = "";
+};
+
+namespace {
+
+int fail(fdtd_llg *s, int code, const char *fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (s) s->err = buf; else g_create_error = buf;
+  return code;
+}
+
+#define CU(s, call)                                                                      \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess)                                                               \
+      return fail((s), FDTD_LLG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));         \
+  } while (0)
+
+dim3 grid_for(int ex, int ey, int ez) {
+  return dim3((ex + BX - 1) / BX, (ey + BY - 1) / BY, (ez + BZ - 1) / BZ);
+}
+
+bool valid_opts(const fdtd_llg_options *o, const char **why) {
+  for (int d = 0; d < 3; ++d)
+    if (o->bc[d] != FDTD_LLG_PEC && o->bc[d] != FDTD_LLG_PERIODIC) { *why = "bc must be 0 (PEC) or 1 (periodic)"; return false; }
+  if (o->enable_llg) {
+    if (!(o->llg_tol > 0) || !std::isfinite(o->llg_tol)) { *why = "llg_tol must be > 0"; return false; }
+    if (o->llg_max_iter < 1 || o->llg_max_iter > 1000) { *why = "llg_max_iter must be in 1..1000"; return false; }
+    if (o->ani_hk != 0.0) {
+      double n2 = 0;
+      for (int d = 0; d < 3; ++d) n2 += o->ani_axis[d] * o->ani_axis[d];
+      if (!(std::fabs(n2 - 1.0) < 1e-9)) { *why = "ani_axis must be a unit vector"; return false; }
+    }
+    for (int d = 0; d < 3; ++d)
+      if (!std::isfinite(o->h_bias[d])) { *why = "h_bias must be finite"; return false; }
+  }
+  return true;
+}
+
+size_t small_bytes(const fdtd_llg_options *o) {
+  size_t b = 0;
+  b += 4096;                                                  // DevState
+  b += padded((size_t)(o->llg_max_iter + 2)) * 8 + 4096;      // residual words
+  b += (2 * 1024 + 64) * 8;                                   // reduction scratch
+  b += (size_t)1 << 20;                                       // source profiles pool (1 MiB)
+  return (b + 255) / 256 * 256;
+}
+
+// min/max of a user array (host or device)
+int array_minmax(fdtd_llg *s, const double *a, int mem_space, double *lo, double *hi) {
+  const size_t n = s->ncell;
+  if (mem_space == FDTD_LLG_HOST) {
+    double l = INFINITY, h = -INFINITY;
+    bool nan = false;
+    for (size_t i = 0; i < n; ++i) {
+      const double v = a[i];
+      if (v != v) nan = true;
+      if (v < l) l = v;
+      if (v > h) h = v;
+    }
+    *lo = nan ? NAN : l;
+    *hi = nan ? NAN : h;
+    return FDTD_LLG_OK;
+  }
+  const int blocks = 1024;
+  k_minmax<<<blocks, 256, 0, s->stream>>>(a, (long long)n, s->scratch);
+  CU(s, cudaGetLastError());
+  std::vector<double> part(2 * blocks);
+  CU(s, cudaMemcpyAsync(part.data(), s->scratch, sizeof(double) * 2 * blocks,
+                        cudaMemcpyDeviceToHost, s->stream));
+  CU(s, cudaStreamSynchronize(s->stream));
+  double l = INFINITY, h = -INFINITY;
+  bool nan = false;
+  for (int b = 0; b < blocks; ++b) {
+    if (part[2 * b] != part[2 * b] || part[2 * b + 1] != part[2 * b + 1]) nan = true;
+    l = std::fmin(l, part[2 * b]);
+    h = std::fmax(h, part[2 * b + 1]);
+  }
+  *lo = nan ? NAN : l;
+  *hi = nan ? NAN : h;
+  return FDTD_LLG_OK;
+}
+
+// analyse one material: uniform -> scalar, else copy into the workspace slot
+int take_material(fdtd_llg *s, MatInfo *m, const double *user, int mem_space, double dflt,
+                  double **slot, const char *name, double min_allowed, bool strict_min,
+                  unsigned bit) {
+  m->is_array = false;
+  m->uniform = dflt;
+  m->dev = nullptr;
+  if (!user) return FDTD_LLG_OK;
+  double lo, hi;
+  if (s->opt.scalar_material_mask & bit) {
+    lo = hi = *user;  // one HOST double: the uniform value
+  } else {
+    int rc = array_minmax(s, user, mem_space, &lo, &hi);
+    if (rc) return rc;
+  }
+  if (!(lo == lo) || !std::isfinite(lo) || !std::isfinite(hi))
+    return fail(s, FDTD_LLG_EINVAL, "%s contains a non-finite value", name);
+  if (strict_min ? !(lo > min_allowed) : !(lo >= min_allowed))
+    return fail(s, FDTD_LLG_EINVAL, "%s must be %s %g everywhere (min is %g)", name,
+                strict_min ? ">" : ">=", min_allowed, lo);
+  if (lo == hi) {
+    m->uniform = lo;
+    return FDTD_LLG_OK;
+  }
+  m->is_array = true;
+  m->dev = *slot;
+  *slot += s->stride;
+  CU(s, cudaMemcpyAsync(m->dev, user, s->ncell * sizeof(double),
+                        mem_space == FDTD_LLG_HOST ? cudaMemcpyHostToDevice
+                                                   : cudaMemcpyDeviceToDevice,
+                        s->stream));
+  return FDTD_LLG_OK;
+}
+
+int find_sweep_box(fdtd_llg *s) {
+  s->llg = false;
+  s->magnetic_cells = 0;
+  if (!s->opt.enable_llg) return FDTD_LLG_OK;
+  int clo[3], chi[3];  // cell box, inclusive
+  if (!s->Ms.is_array) {
+    if (!(s->Ms.uniform > 0.0)) return FDTD_LLG_OK;
+    for (int d = 0; d < 3; ++d) { clo[d] = 0; chi[d] = s->g.n[d] - 1; }
+    s->magnetic_cells = (long long)s->ncell;
+  } else {
+    int *box = reinterpret_cast<int *>(s->scratch + 2 * 1024);
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(s->scratch + 2 * 1024 + 8);
+    int init[6] = {INT_MAX, INT_MAX, INT_MAX, -1, -1, -1};
+    unsigned long long zero = 0;
+    CU(s, cudaMemcpyAsync(box, init, sizeof init, cudaMemcpyHostToDevice, s->stream));
+    CU(s, cudaMemcpyAsync(cnt, &zero, sizeof zero, cudaMemcpyHostToDevice, s->stream));
+    k_mag_box<<<1024, 256, 0, s->stream>>>(s->Ms.dev, s->g, box, cnt);
+    CU(s, cudaGetLastError());
+    int out[6];
+    unsigned long long c = 0;
+    CU(s, cudaMemcpyAsync(out, box, sizeof out, cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaMemcpyAsync(&c, cnt, sizeof c, cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    if (c == 0) return FDTD_LLG_OK;
+    for (int d = 0; d < 3; ++d) { clo[d] = out[d]; chi[d] = out[3 + d]; }
+    s->magnetic_cells = (long long)c;
+  }
+  // index triples owning a magnetic face: cells clo..chi+1; plus one triple of halo each side,
+  // because the four-point averages of a magnetic face read its neighbours' H from the Jacobi
+  // buffers.  A box touching a periodic end wraps: take the full axis there.
+  for (int d = 0; d < 3; ++d) {
+    int l = clo[d] - 1, h = chi[d] + 3;  // exclusive upper bound
+    const int n = s->g.n[d];
+    if (s->g.per[d] && (l < 0 || h > n)) { l = 0; h = n; }
+    s->lo[d] = l < 0 ? 0 : l;
+    s->hi[d] = h > n ? n : h;
+  }
+  s->llg = true;
+  return FDTD_LLG_OK;
+}
+
+// ---- launching one step ----------------------------------------------------------------
+
+template <bool FIRST>
+int launch_sweep(fdtd_llg *s, const HMArgs &a, dim3 grid) {
+  const dim3 blk(BX, BY, BZ);
+  const bool ms = s->Ms.is_array, ag = s->alpha.is_array || s->gamma.is_array,
+             mu = s->mu_r.is_array, an = s->opt.ani_hk != 0.0;
+#define SW(MS, AG, MU, AN)                                                               \
+  if (ms == MS && ag == AG && mu == MU && an == AN) {                                    \
+    k_hm_sweep<FIRST, MS, AG, MU, AN><<<grid, blk, 0, s->stream>>>(a);                   \
+    return FDTD_LLG_OK;                                                                  \
+  }
+  SW(false, false, false, false) SW(false, false, false, true) SW(false, false, true, false)
+  SW(false, false, true, true) SW(false, true, false, false) SW(false, true, false, true)
+  SW(false, true, true, false) SW(false, true, true, true) SW(true, false, false, false)
+  SW(true, false, false, true) SW(true, false, true, false) SW(true, false, true, true)
+  SW(true, true, false, false) SW(true, true, false, true) SW(true, true, true, false)
+  SW(true, true, true, true)
+#undef SW
+  return FDTD_LLG_OK;
+}
+
+// (H,M) half-step: time-n set `in`, result in set `out`, `tmp` is the other Jacobi buffer.
+// M: time-n set `min`, result in set `mout`.
+int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool last,
+                 int *launches) {
+  const dim3 blk(BX, BY, BZ);
+  HArgs h{};
+  h.g = s->g;
+  for (int d = 0; d < 3; ++d) { h.E[d] = s->E[d]; h.Hn[d] = s->Hset[in][d]; h.Hc[d] = s->Hset[out][d]; }
+  h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
+  h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
+  h.has_box = s->llg;
+  for (int d = 0; d < 3; ++d) { h.lo[d] = s->lo[d]; h.hi[d] = s->hi[d]; }
+  bool box_is_all = s->llg;
+  for (int d = 0; d < 3; ++d) box_is_all = box_is_all && s->lo[d] == 0 && s->hi[d] == s->g.n[d];
+  if (!box_is_all) {
+    const dim3 grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+    if (s->mu_r.is_array) k_h_update<true><<<grid, blk, 0, s->stream>>>(h);
+    else k_h_update<false><<<grid, blk, 0, s->stream>>>(h);
+    ++*launches;
+  }
+  if (s->llg) {
+    HMArgs a{};
+    a.g = s->g;
+    for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.Hn[d] = s->Hset[in][d]; }
+    for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
+    a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
+    a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
+    a.ch_uniform = h.ch_uniform;
+    for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
+    a.hk = s->opt.ani_hk;
+    a.tol = s->opt.llg_tol;
+    for (int d = 0; d < 3; ++d) { a.lo[d] = s->lo[d]; a.hi[d] = s->hi[d]; }
+    a.resid = s->resid;
+    const dim3 grid = grid_for(s->hi[0] - s->lo[0], s->hi[1] - s->lo[1], s->hi[2] - s->lo[2]);
+    for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
+      // iterate r reads H^{r-1} and writes H^r: odd r -> `out`, even r -> `tmp`
+      const int from = (r == 1) ? in : ((r & 1) ? tmp : out);
+      const int to = (r & 1) ? out : tmp;
+      for (int d = 0; d < 3; ++d) { a.Hp[d] = s->Hset[from][d]; a.Hc[d] = s->Hset[to][d]; }
+      a.r = r;
+      int rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
+      if (rc) return rc;
+      ++*launches;
+    }
+  }
+  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->opt.llg_max_iter, s->opt.llg_tol,
+                                     s->llg ? 1 : 0, last ? 1 : 0);
+  ++*launches;
+  if (s->llg && s->opt.llg_max_iter >= 2) {
+    CanonArgs c{};
+    c.g = s->g;
+    for (int d = 0; d < 3; ++d) { c.src[d] = s->Hset[tmp][d]; c.dst[d] = s->Hset[out][d]; c.lo[d] = s->lo[d]; c.hi[d] = s->hi[d]; }
+    c.st = s->dstate;
+    const dim3 grid = grid_for(s->hi[0] - s->lo[0], s->hi[1] - s->lo[1], s->hi[2] - s->lo[2]);
+    k_canon<<<grid, blk, 0, s->stream>>>(c);
+    ++*launches;
+  }
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
+int enqueue_e(fdtd_llg *s, int hset, int *launches) {
+  const dim3 blk(BX, BY, BZ);
+  EArgs a{};
+  a.g = s->g;
+  for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.H[d] = s->Hset[hset][d]; }
+  a.eps_r = s->eps_r.dev; a.sigma = s->sigma.dev;
+  a.eps_u = kEps0 * s->eps_r.uniform; a.sigma_u = s->sigma.uniform;
+  a.src = s->src;
+  a.st = s->dstate;
+  const dim3 grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+  const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = s->src.count > 0;
+#define EK(EA, SA, HS)                                                        \
+  if (ea == EA && sa == SA && hs == HS) k_e_update<EA, SA, HS><<<grid, blk, 0, s->stream>>>(a);
+  EK(false, false, false) EK(false, false, true) EK(false, true, false) EK(false, true, true)
+  EK(true, false, false) EK(true, false, true) EK(true, true, false) EK(true, true, true)
+#undef EK
+  ++*launches;
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
+// one full time step: HM half (curl E^n), E update, HM half (curl E^{n+1}).
+// H sets: state in 0 -> half 1 result in 1 -> half 2 result back in 0.  M sets: 0 -> 1 -> 0.
+int enqueue_step(fdtd_llg *s, int *launches) {
+  *launches = 0;
+  if (s->src.count > 0) {
+    k_step_begin<<<1, 32, 0, s->stream>>>(s->dstate, s->src, s->dt);
+    ++*launches;
+  }
+  int rc = enqueue_half(s, 0, 1, 2, 0, 1, false, launches);
+  if (rc) return rc;
+  rc = enqueue_e(s, 1, launches);
+  if (rc) return rc;
+  return enqueue_half(s, 1, 0, 2, 1, 0, true, launches);
+}
+
+int build_graph(fdtd_llg *s) {
+  if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+  s->graph_valid = false;
+  cudaGraph_t g = nullptr;
+  CU(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+  int launches = 0;
+  int rc = enqueue_step(s, &launches);
+  cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+  if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+  if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+  e = cudaGraphInstantiate(&s->graph, g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+  s->launches_per_step = launches;
+  s->graph_valid = true;
+  return FDTD_LLG_OK;
+}
+
+cudaMemcpyKind to_dev(int mem_space) {
+  return mem_space == FDTD_LLG_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+}
+cudaMemcpyKind from_dev(int mem_space) {
+  return mem_space == FDTD_LLG_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+}
+
+}  // namespace
+
+// ===================================================================================== C ABI
+
+extern "C" {
+
+void fdtd_llg_default_options(fdtd_llg_options *o) {
+  if (!o) return;
+  std::memset(o, 0, sizeof *o);
+  o->bc[0] = o->bc[1] = o->bc[2] = FDTD_LLG_PEC;
+  o->enable_llg = 1;
+  o->ani_axis[2] = 1.0;
+  o->llg_tol = 1e-6;
+  o->llg_max_iter = 20;
+  o->use_graph = 1;
+}
+
+size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
+                                unsigned material_mask) {
+  if (nx < 1 || ny < 1 || nz < 1 || !opt) return 0;
+  const size_t stride = padded((size_t)nx * ny * nz);
+  size_t arrays = 6;                       // E, H
+  if (opt->enable_llg) arrays += 6 + 18;   // two more H sets, two M sets
+  for (unsigned b = 0; b < 6; ++b)
+    if (material_mask & (1u << b)) ++arrays;
+  return arrays * stride * sizeof(double) + small_bytes(opt);
+}
+
+int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy, double dz,
+                    double dt, const double *eps_r, const double *sigma, const double *mu_r,
+                    const double *Ms, const double *alpha, const double *gamma, int mem_space,
+                    const fdtd_llg_options *opt, void *dev_workspace, size_t workspace_bytes,
+                    void *cuda_stream) {
+  if (!out) return fail(nullptr, FDTD_LLG_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, FDTD_LLG_EINVAL, "nx, ny, nz must be >= 1");
+  if ((double)nx * ny * nz > 2.0e9) return fail(nullptr, FDTD_LLG_EINVAL, "grid too large (> 2e9 cells)");
+  if (!(dx > 0) || !(dy > 0) || !(dz > 0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
+    return fail(nullptr, FDTD_LLG_EINVAL, "dx, dy, dz must be finite and > 0");
+  if (!(dt > 0) || !std::isfinite(dt)) return fail(nullptr, FDTD_LLG_EINVAL, "dt must be finite and > 0");
+  if (!opt) return fail(nullptr, FDTD_LLG_EINVAL, "opt is NULL");
+  if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
+    return fail(nullptr, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
+  const char *why = "";
+  if (!valid_opts(opt, &why)) return fail(nullptr, FDTD_LLG_EINVAL, "%s", why);
+  if (!dev_workspace) return fail(nullptr, FDTD_LLG_EINVAL, "dev_workspace is NULL");
+  if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) return fail(nullptr, FDTD_LLG_EINVAL, "dev_workspace must be 256-byte aligned");
+  unsigned mask = (eps_r ? 1u : 0) | (sigma ? 2u : 0) | (mu_r ? 4u : 0) | (Ms ? 8u : 0) | (alpha ? 16u : 0) | (gamma ? 32u : 0);
+  mask &= ~opt->scalar_material_mask;
+  const size_t need = fdtd_llg_workspace_bytes(nx, ny, nz, opt, mask);
+  if (workspace_bytes < need)
+    return fail(nullptr, FDTD_LLG_ENOMEM, "workspace too small: %zu bytes given, %zu needed", workspace_bytes, need);
+
+  fdtd_llg *s = new (std::nothrow) fdtd_llg();
+  if (!s) return fail(nullptr, FDTD_LLG_ENOMEM, "host allocation failed");
+  s->g.n[0] = nx; s->g.n[1] = ny; s->g.n[2] = nz;
+  s->g.s[0] = 1; s->g.s[1] = nx; s->g.s[2] = (long long)nx * ny;
+  s->d[0] = dx; s->d[1] = dy; s->d[2] = dz;
+  for (int d = 0; d < 3; ++d) { s->g.per[d] = opt->bc[d] == FDTD_LLG_PERIODIC; s->g.rd[d] = 1.0 / s->d[d]; }
+  s->g.dt = dt;
+  s->dt = dt;
+  s->ncell = (size_t)nx * ny * nz;
+  s->stride = padded(s->ncell);
+  s->opt = *opt;
+  if (!opt->enable_llg) { s->opt.llg_max_iter = 1; s->opt.llg_tol = 1.0; }
+  s->stream = static_cast<cudaStream_t>(cuda_stream);
+  if (!cuda_stream) s->opt.use_graph = 0;  // the legacy default stream cannot be captured
+  s->ws = static_cast<char *>(dev_workspace);
+  s->ws_bytes = workspace_bytes;
+
+  auto bail = [&](int rc) { g_create_error = s->err; delete s; return rc; };
+#define CUB(call)                                                                        \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess) {                                                             \
+      fail(s, FDTD_LLG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));                  \
+      return bail(FDTD_LLG_ECUDA);                                                       \
+    }                                                                                    \
+  } while (0)
+
+  // carve the workspace: small state first, then the big arrays
+  char *p = s->ws;
+  s->dstate = reinterpret_cast<DevState *>(p); p += 4096;
+  s->resid = reinterpret_cast<unsigned long long *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 4096;
+  s->scratch = reinterpret_cast<double *>(p); p += (2 * 1024 + 64) * 8;
+  s->profile_pool = reinterpret_cast<double *>(p); s->profile_cap = ((size_t)1 << 20) / 8; p += (size_t)1 << 20;
+  p = s->ws + small_bytes(&s->opt);
+  double *q = reinterpret_cast<double *>(p);
+  for (int d = 0; d < 3; ++d) { s->E[d] = q; q += s->stride; }
+  const int nh = opt->enable_llg ? 3 : 1;
+  for (int h = 0; h < nh; ++h)
+    for (int d = 0; d < 3; ++d) { s->Hset[h][d] = q; q += s->stride; }
+  if (!opt->enable_llg)
+    for (int h = 1; h < 3; ++h)
+      for (int d = 0; d < 3; ++d) s->Hset[h][d] = s->Hset[0][d];  // Maxwell only: in place
+  if (opt->enable_llg)
+    for (int m = 0; m < 2; ++m)
+      for (int c = 0; c < 9; ++c) { s->Mset[m][c] = q; q += s->stride; }
+  const size_t state_arrays = 3 + 3 * nh + (opt->enable_llg ? 18 : 0);
+  CUB(cudaMemsetAsync(s->ws, 0, small_bytes(&s->opt) + state_arrays * s->stride * sizeof(double), s->stream));
+
+  int rc;
+  if ((rc = take_material(s, &s->eps_r, eps_r, mem_space, 1.0, &q, "eps_r", 0.0, true, 1u))) return bail(rc);
+  if ((rc = take_material(s, &s->sigma, sigma, mem_space, 0.0, &q, "sigma", 0.0, false, 2u))) return bail(rc);
+  if ((rc = take_material(s, &s->mu_r, mu_r, mem_space, 1.0, &q, "mu_r", 0.0, true, 4u))) return bail(rc);
+  if (opt->enable_llg) {
+    if ((rc = take_material(s, &s->Ms, Ms, mem_space, 0.0, &q, "Ms", 0.0, false, 8u))) return bail(rc);
+    if ((rc = take_material(s, &s->alpha, alpha, mem_space, 0.0, &q, "alpha", -INFINITY, false, 16u))) return bail(rc);
+    if ((rc = take_material(s, &s->gamma, gamma, mem_space, 0.0, &q, "gamma", -INFINITY, false, 32u))) return bail(rc);
+  }
+  if ((rc = find_sweep_box(s))) return bail(rc);
+  CUB(cudaStreamSynchronize(s->stream));
+#undef CUB
+  *out = s;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const *H,
+                        const double *const *M_cell, int mem_space) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
+    return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
+  const size_t bytes = s->ncell * sizeof(double);
+  const dim3 blk(BX, BY, BZ), grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+  for (int d = 0; d < 3; ++d) {
+    if (E && E[d]) CU(s, cudaMemcpyAsync(s->E[d], E[d], bytes, to_dev(mem_space), s->stream));
+    else CU(s, cudaMemsetAsync(s->E[d], 0, bytes, s->stream));
+    if (H && H[d]) CU(s, cudaMemcpyAsync(s->Hset[0][d], H[d], bytes, to_dev(mem_space), s->stream));
+    else CU(s, cudaMemsetAsync(s->Hset[0][d], 0, bytes, s->stream));
+  }
+  if (s->opt.enable_llg)
+    for (int h = 1; h < 3; ++h)
+      for (int d = 0; d < 3; ++d) CU(s, cudaMemsetAsync(s->Hset[h][d], 0, bytes, s->stream));
+  FieldsP f{};
+  f.g = s->g;
+  for (int d = 0; d < 3; ++d) { f.E[d] = s->E[d]; f.H[d] = s->Hset[0][d]; }
+  k_enforce_walls<<<grid, blk, 0, s->stream>>>(f);
+  CU(s, cudaGetLastError());
+  // reset run state
+  CU(s, cudaMemsetAsync(s->dstate, 0, sizeof(DevState), s->stream));
+  CU(s, cudaMemsetAsync(s->resid, 0, (size_t)(s->opt.llg_max_iter + 2) * 8, s->stream));
+  if (s->opt.enable_llg) {
+    InitMP a{};
+    a.g = s->g;
+    for (int c = 0; c < 3; ++c) {
+      a.Mc[c] = nullptr;
+      if (M_cell && M_cell[c]) {
+        if (mem_space == FDTD_LLG_DEVICE) {
+          a.Mc[c] = M_cell[c];
+        } else {  // stage the host array in the second M set
+          CU(s, cudaMemcpyAsync(s->Mset[1][c], M_cell[c], bytes, cudaMemcpyHostToDevice, s->stream));
+          a.Mc[c] = s->Mset[1][c];
+        }
+      }
+    }
+    for (int c = 0; c < 9; ++c) a.M[c] = s->Mset[0][c];
+    a.Ms = s->Ms.dev;
+    a.Ms_u = s->Ms.uniform;
+    a.enable_llg = s->llg ? 1 : 0;
+    a.st = s->dstate;
+    k_init_m<<<grid, blk, 0, s->stream>>>(a);
+    CU(s, cudaGetLastError());
+    for (int c = 0; c < 9; ++c) CU(s, cudaMemsetAsync(s->Mset[1][c], 0, bytes, s->stream));
+    int err = 0;
+    CU(s, cudaMemcpyAsync(&err, &s->dstate->init_error, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    if (err) return fail(s, FDTD_LLG_EINVAL, "a magnetic face received a zero averaged M (PAPER.md:90 needs a direction to normalise)");
+  }
+  CU(s, cudaStreamSynchronize(s->stream));
+  s->host_steps = 0;
+  s->kernel_launches = 0;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
+                        const double *profile, int mem_space, double amplitude, double f0,
+                        double t0, double tp) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (s->src.count >= MAX_SOURCES) return fail(s, FDTD_LLG_ESTATE, "at most %d sources", MAX_SOURCES);
+  if (comp < 0 || comp > 2) return fail(s, FDTD_LLG_EINVAL, "comp must be 0, 1 or 2");
+  if (!lo || !hi) return fail(s, FDTD_LLG_EINVAL, "lo / hi is NULL");
+  if (!(tp > 0) || !std::isfinite(tp) || !std::isfinite(amplitude) || !std::isfinite(f0) || !std::isfinite(t0))
+    return fail(s, FDTD_LLG_EINVAL, "tp must be > 0 and amplitude, f0, t0 finite");
+  size_t nb = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (lo[d] < 0 || hi[d] > s->g.n[d] || lo[d] >= hi[d])
+      return fail(s, FDTD_LLG_EINVAL, "source box outside the grid or empty on axis %d", d);
+    nb *= (size_t)(hi[d] - lo[d]);
+  }
+  SourceP &S = s->src.s[s->src.count];
+  S.comp = comp;
+  for (int d = 0; d < 3; ++d) { S.lo[d] = lo[d]; S.hi[d] = hi[d]; }
+  S.amplitude = amplitude; S.f0 = f0; S.t0 = t0; S.tp = tp;
+  S.profile = nullptr;
+  if (profile) {
+    if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
+      return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
+    if (s->profile_used + nb > s->profile_cap)
+      return fail(s, FDTD_LLG_ENOMEM, "source profiles exceed the 1 MiB pool");
+    double *dst = s->profile_pool + s->profile_used;
+    CU(s, cudaMemcpyAsync(dst, profile, nb * sizeof(double), to_dev(mem_space), s->stream));
+    CU(s, cudaStreamSynchronize(s->stream));
+    S.profile = dst;
+    s->profile_used += padded(nb);
+  }
+  s->src.count++;
+  s->graph_valid = false;  // the step's kernel arguments changed
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_step(fdtd_llg *s, int n) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (n < 0) return fail(s, FDTD_LLG_EINVAL, "n must be >= 0");
+  if (n == 0) return FDTD_LLG_OK;
+  if (s->opt.use_graph) {
+    if (!s->graph_valid) {
+      int rc = build_graph(s);
+      if (rc) return rc;
+    }
+    for (int t = 0; t < n; ++t) CU(s, cudaGraphLaunch(s->graph, s->stream));
+  } else {
+    for (int t = 0; t < n; ++t) {
+      int launches = 0;
+      int rc = enqueue_step(s, &launches);
+      if (rc) return rc;
+      s->launches_per_step = launches;
+    }
+  }
+  s->host_steps += n;
+  s->kernel_launches += (long long)n * s->launches_per_step;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double *const *M,
+                         int mem_space) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
+    return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
+  const size_t bytes = s->ncell * sizeof(double);
+  for (int d = 0; d < 3; ++d) {
+    if (E && E[d]) CU(s, cudaMemcpyAsync(E[d], s->E[d], bytes, from_dev(mem_space), s->stream));
+    if (H && H[d]) CU(s, cudaMemcpyAsync(H[d], s->Hset[0][d], bytes, from_dev(mem_space), s->stream));
+  }
+  if (M)
+    for (int c = 0; c < 9; ++c)
+      if (M[c]) {
+        if (s->opt.enable_llg) CU(s, cudaMemcpyAsync(M[c], s->Mset[0][c], bytes, from_dev(mem_space), s->stream));
+        else if (mem_space == FDTD_LLG_HOST) std::memset(M[c], 0, bytes);
+        else CU(s, cudaMemsetAsync(M[c], 0, bytes, s->stream));
+      }
+  CU(s, cudaStreamSynchronize(s->stream));
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
+  if (!s || !out) return FDTD_LLG_EINVAL;
+  DevState h{};
+  CU(s, cudaMemcpyAsync(&h, s->dstate, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+  CU(s, cudaStreamSynchronize(s->stream));
+  std::memset(out, 0, sizeof *out);
+  out->steps = h.steps;
+  out->time = (double)h.steps * s->dt;
+  out->iters_last = h.iters_last;
+  out->iters_max = h.iters_max;
+  out->iters_total = h.iters_total;
+  out->nonconverged_halfsteps = h.nonconverged;
+  out->resid_last = h.resid_last;
+  out->halfsteps = h.halfsteps;
+  const double lim = 1.0 / (kC0 * std::sqrt(1.0 / (s->d[0] * s->d[0]) + 1.0 / (s->d[1] * s->d[1]) + 1.0 / (s->d[2] * s->d[2])));
+  out->courant = s->dt / lim;
+  out->kernel_launches = s->kernel_launches;
+  out->magnetic_cells = s->magnetic_cells;
+  out->launches_per_step = s->launches_per_step;
+  return FDTD_LLG_OK;
+}
+
+const char *fdtd_llg_last_error(const fdtd_llg *s) {
+  return s ? s->err.c_str() : g_create_error.c_str();
+}
+
+void fdtd_llg_destroy(fdtd_llg *s) {
+  if (!s) return;
+  if (s->graph) cudaGraphExecDestroy(s->graph);
+  delete s;
+}
+
+}  // extern "C"

@@ -113,7 +113,8 @@ class Workload:
     ani_axis: tuple = (0.0, 0.0, 1.0)
     llg_tol: float = 1e-12
     llg_max_iter: int = 20
-    # cell-centred material maps, shape (nz, ny, nx) float64, or None for the default
+    # cell-centred material maps, shape (nz, ny, nx) float64; a python float = uniform value;
+    # missing/None = the default
     materials: dict = field(default_factory=dict)
     E: list = field(default_factory=lambda: [None, None, None])
     H: list = field(default_factory=lambda: [None, None, None])
@@ -128,8 +129,14 @@ class Workload:
 
     def numpy(self):
         """Host numpy views of every array (for the oracle)."""
+        import numpy as np
+
         def cv(t):
-            return None if t is None else t.detach().cpu().numpy()
+            if t is None:
+                return None
+            if isinstance(t, (int, float)):   # uniform material given as a scalar
+                return np.full((self.nz, self.ny, self.nx), float(t))
+            return t.detach().cpu().numpy()
         return {
             "materials": {k: cv(v) for k, v in self.materials.items()},
             "E": [cv(t) for t in self.E],
@@ -265,9 +272,7 @@ def config4(shape=(384, 384, 384), device="cpu", steps=2000) -> Workload:
     kslab = max(1, nz // 12)                     # 32 of 384
     Ms = _zeros(nx, ny, nz, device)
     Ms[:kslab] = 1.4e5
-    w.materials = {"Ms": Ms,
-                   "alpha": torch.full_like(Ms, 1e-3),
-                   "gamma": torch.full_like(Ms, 1.759e11)}
+    w.materials = {"Ms": Ms, "alpha": 1e-3, "gamma": 1.759e11}
     w.M_cell = tilted_m_cell(seed, nx, ny, nz, Ms, 0.5, device)
     f0 = 5e9
     tp = 1.0 / f0
@@ -286,9 +291,7 @@ def config5(shape=(768, 768, 768), device="cpu", steps=200, e_fields=True) -> Wo
                  llg_tol=1e-12, llg_max_iter=20, seed=seed)
     Ms = _zeros(nx, ny, nz, device)
     Ms[: nz // 2] = 8e5
-    w.materials = {"Ms": Ms,
-                   "alpha": torch.full_like(Ms, 0.01),
-                   "gamma": torch.full_like(Ms, 1.759e11)}
+    w.materials = {"Ms": Ms, "alpha": 0.01, "gamma": 1.759e11}
     w.M_cell = tilted_m_cell(seed, nx, ny, nz, Ms, 2.0, device)
     if e_fields:
         for c in range(3):

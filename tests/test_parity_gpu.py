@@ -1,0 +1,179 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle -- the first gate.
+
+Same seeded inputs on both sides; element-by-element comparison; the bar is BASELINE.json's:
+max relative L-infinity error <= 1e-9 on E, H and M after 100 steps (A21 defines the
+norm).  Shapes span several 32x4x2 thread blocks plus a ragged tail in every axis.
+"""
+import numpy as np
+import pytest
+import torch
+
+from tests._util import FIELD_GROUPS, oracle_from_workload, rel_linf
+from paper_2103_12819_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9  # north_star: max relative L-inf on E, H and M after 100 steps
+
+
+def _gpu_fields(sim):
+    return {k: v.numpy() for k, v in sim.read_fields().items()}
+
+
+def _run_both(w, steps, use_graph=True, chunks=(None,)):
+    from paper_2103_12819_b200.binding import from_workload
+    o = oracle_from_workload(w)
+    o.step(steps)
+    ref = o.read_fields()
+    sim = from_workload(w, use_graph=use_graph)
+    if chunks == (None,):
+        sim.step(steps)
+    else:
+        for c in chunks:
+            sim.step(c)
+    got = _gpu_fields(sim)
+    return got, ref, sim.stats(), o.stats()
+
+
+def _assert_parity(got, ref, llg, tol=TOL):
+    errs = {g: rel_linf(got, ref, g) for g in ("E", "H") + (("M",) if llg else ())}
+    for g, e in errs.items():
+        assert e <= tol, (g, errs)
+    return errs
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_parity_100_steps_all_configs(cfg):
+    w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
+    got, ref, gs, os_ = _run_both(w, 100)
+    _assert_parity(got, ref, w.enable_llg)
+    assert gs["steps"] == 100
+    if w.enable_llg:
+        # same number of LLG iterations, all converged
+        assert gs["iters_total"] == int(os_["iters_total"])
+        assert gs["nonconverged_halfsteps"] == 0
+        assert gs["halfsteps"] == 200
+        # wall faces / non-magnetic faces carry exactly M = 0 on both sides
+        for n in FIELD_GROUPS["M"]:
+            assert np.array_equal(got[n] == 0.0, ref[n] == 0.0)
+    # the fields are not trivially zero
+    assert max(np.abs(ref[n]).max() for n in FIELD_GROUPS["E"]) > 0
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 1, 1), (1, 0, 1), (0, 1, 1), (1, 1, 0)])
+def test_parity_every_boundary_mix_with_everything_on(bc):
+    """Spatially varying eps, sigma, mu, Ms, alpha, gamma, anisotropy, two sources with and
+    without profile, partially magnetic box: all template branches of the kernels."""
+    rng = np.random.default_rng(5)
+    shape = (37, 11, 9)
+    nx, ny, nz = shape
+    shp = (nz, ny, nx)
+    w = wl.Workload("everything", nx, ny, nz, 1e-6, 1.2e-6, 0.8e-6,
+                    wl.courant_dt(0.9, 1e-6, 1.2e-6, 0.8e-6), bc, 30, enable_llg=True,
+                    h_bias=(1e3, -2e3, 1e4), ani_hk=3e3, ani_axis=(0.6, 0.0, 0.8),
+                    llg_tol=1e-13, llg_max_iter=30)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a))
+    Ms = 1.4e5 * (1 + rng.random(shp)) * (rng.random(shp) < 0.6)
+    Ms[:, :, 30:] = 0.0          # the sweep box does not cover the whole grid
+    mu = np.where(Ms > 0, 1.0, 1 + rng.random(shp) * (rng.random(shp) < 0.3))
+    w.materials = {"eps_r": t(1 + 3 * rng.random(shp)),
+                   "sigma": t(100 * rng.random(shp) * (rng.random(shp) < 0.5)),
+                   "mu_r": t(mu), "Ms": t(Ms), "alpha": t(0.01 + 0.05 * rng.random(shp)),
+                   "gamma": t(-1.759e11 * (1 + 0.1 * rng.random(shp)))}
+    th, ph = np.pi * rng.random(shp), 2 * np.pi * rng.random(shp)
+    w.M_cell = [t(Ms * np.sin(th) * np.cos(ph)), t(Ms * np.sin(th) * np.sin(ph)), t(Ms * np.cos(th))]
+    w.E = [t(1e6 * rng.standard_normal(shp)) for _ in range(3)]
+    w.H = [t(1e3 * rng.standard_normal(shp)) for _ in range(3)]
+    lo, hi = (1, 2, 1), (nx - 1, 5, 4)
+    nb = int(np.prod([h - l for l, h in zip(lo, hi)]))
+    w.sources = [wl.Source(1, lo, hi, 1e12, 2e12, 3e-15, 2e-15, profile=t(rng.random(nb))),
+                 wl.Source(2, (0, 0, 0), shape, 5e11, 1e12, 1e-15, 4e-15)]
+    got, ref, gs, os_ = _run_both(w, 30)
+    _assert_parity(got, ref, True)
+    assert gs["iters_total"] == int(os_["iters_total"])
+
+
+def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
+    """step(100) == step(37)+step(63) == the same without a CUDA graph, bit for bit."""
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(4, shape=wl.SMALL_SHAPES[4])
+    outs = []
+    for use_graph, chunks in ((True, (100,)), (True, (37, 63)), (False, (100,))):
+        sim = from_workload(w, use_graph=use_graph)
+        for c in chunks:
+            sim.step(c)
+        outs.append(_gpu_fields(sim))
+        assert sim.stats()["steps"] == 100
+        assert sim.stats()["kernel_launches"] == 100 * sim.stats()["launches_per_step"]
+    for other in outs[1:]:
+        for n in outs[0]:
+            assert np.array_equal(outs[0][n], other[n]), n
+
+
+def test_device_resident_inputs_equal_host_inputs():
+    from paper_2103_12819_b200.binding import from_workload
+    wh = wl.make_config(5, shape=wl.SMALL_SHAPES[5])
+    wd = wl.make_config(5, shape=wl.SMALL_SHAPES[5], device="cuda:0")
+    # the generator is counter based: host and device give the same inputs (to libm rounding)
+    for a, b in zip(wh.E + wh.M_cell, wd.E + wd.M_cell):
+        assert torch.allclose(a, b.cpu(), rtol=1e-13, atol=1e-13 * float(a.abs().max()))
+    sh, sd = from_workload(wh), from_workload(wd)
+    sh.step(20)
+    sd.step(20)
+    fh, fd = _gpu_fields(sh), {k: v.cpu().numpy() for k, v in sd.read_fields(device="cuda:0").items()}
+    for g in ("E", "H", "M"):
+        assert rel_linf(fd, fh, g) < 1e-11
+
+
+@pytest.mark.parametrize("shape,bc", [((1, 1, 1), (1, 1, 1)), ((1, 5, 3), (1, 0, 1)),
+                                      ((2, 2, 2), (0, 0, 0)), ((33, 1, 2), (1, 1, 0)),
+                                      ((64, 8, 4), (1, 1, 1)), ((65, 9, 5), (0, 0, 0))])
+def test_degenerate_and_ragged_shapes(shape, bc):
+    """Single-cell axes (periodic neighbours are the cell itself), grids smaller than one thread
+    block, exact multiples of the block and one more."""
+    w = wl.config5(shape=shape)
+    w.bc = bc
+    got, ref, gs, os_ = _run_both(w, 12)
+    _assert_parity(got, ref, True)
+    assert gs["iters_total"] == int(os_["iters_total"])
+
+
+def test_iteration_cap_is_accepted_and_counted():
+    """A4: at llg_max_iter the iterate is accepted and the half-step counted as non-converged."""
+    w = wl.make_config(1, shape=(16, 12, 10))
+    w.llg_max_iter, w.llg_tol = 2, 1e-30
+    got, ref, gs, os_ = _run_both(w, 5)
+    _assert_parity(got, ref, True)
+    assert gs["nonconverged_halfsteps"] == 10 == int(os_["nonconverged"])
+    assert gs["iters_total"] == 20
+    w.llg_max_iter = 1            # odd and even caps exercise both Jacobi buffers
+    got, ref, gs, _ = _run_both(w, 5)
+    _assert_parity(got, ref, True)
+
+
+def test_llg_enabled_without_magnetic_cells_is_plain_maxwell():
+    w = wl.make_config(2, shape=(24, 10, 6), steps=20)
+    w.enable_llg = True
+    got, ref, gs, _ = _run_both(w, 20)
+    _assert_parity(got, ref, True)
+    assert gs["magnetic_cells"] == 0 and gs["iters_total"] == 0
+
+
+def test_errors_are_reported_not_thrown_from_c():
+    from paper_2103_12819_b200 import binding as B
+    with pytest.raises(B.FdtdLlgError) as e:
+        B.FdtdLlg(8, 8, 8, 1e-6, 1e-6, 1e-6, 1e-15, materials={"eps_r": torch.zeros(8, 8, 8, dtype=torch.float64)})
+    assert e.value.code == B.EINVAL and "eps_r" in str(e.value)
+    with pytest.raises(B.FdtdLlgError) as e:
+        B.FdtdLlg(8, 8, 8, 1e-6, 1e-6, 1e-6, 1e-15, materials={"Ms": -torch.ones(8, 8, 8, dtype=torch.float64)})
+    assert e.value.code == B.EINVAL and "Ms" in str(e.value)
+    sim = B.FdtdLlg(8, 8, 8, 1e-6, 1e-6, 1e-6, 1e-15, materials={"Ms": 1e5, "gamma": 1.759e11})
+    with pytest.raises(B.FdtdLlgError) as e:
+        sim.set_fields()          # magnetic faces with no M direction
+    assert e.value.code == B.EINVAL
+    with pytest.raises(B.FdtdLlgError):
+        sim.set_source(0, (0, 0, 0), (9, 8, 8))
+    with pytest.raises(B.FdtdLlgError):
+        sim.step(-1)
+    st = sim.stats()
+    assert st["courant"] == pytest.approx(1e-15 / wl.courant_dt(1.0, 1e-6, 1e-6, 1e-6))

@@ -1,0 +1,98 @@
+"""The seeded input generators: pinned to a pure-python splitmix64, to the paper's printed time
+step, and checked for the structure the configs promise."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2103_12819_b200 import workloads as wl
+
+
+def test_generator_matches_pure_python_splitmix64():
+    idx = torch.tensor([0, 1, 2, 12345, 2 ** 31 + 7, 452984831], dtype=torch.int64)
+    for seed, stream in ((wl.BASE_SEED + 5, 0), (wl.BASE_SEED + 1, 21), (2 ** 63 + 11, 81)):
+        got = wl.uniform(seed, stream, idx)
+        ref = [(wl.splitmix64_py(seed, stream, int(i)) >> 11) * 2.0 ** -53 for i in idx]
+        assert got.tolist() == ref
+    # first output of the textbook splitmix64 with state 0 (Vigna's reference): seed chosen so that
+    # seed + G*(0 + 0 + 1) == G, i.e. seed = 0, stream 0, idx 0
+    assert wl.splitmix64_py(0, 0, 0) == 0xE220A8397B1DCDAF
+
+
+def test_uniform_and_normal_statistics():
+    idx = torch.arange(200000, dtype=torch.int64)
+    u = wl.uniform(7, 3, idx)
+    assert 0.0 <= float(u.min()) and float(u.max()) < 1.0
+    assert abs(float(u.mean()) - 0.5) < 3e-3 and abs(float(u.var()) - 1 / 12) < 1e-3
+    n = wl.normal(7, 4, idx)
+    assert abs(float(n.mean())) < 8e-3 and abs(float(n.var()) - 1) < 1e-2
+    # streams are independent
+    assert abs(float(torch.corrcoef(torch.stack([u, wl.uniform(7, 4, idx)]))[0, 1])) < 8e-3
+
+
+def test_courant_dt_matches_the_papers_printed_time_step():
+    """512x4x512 cells over W = 14.95 mm, h = 10.16 mm, L = 500 mm, CFL 0.8
+    gives dt = 77.87961902 fs (tests/golden/paper_dt.txt)."""
+    gold = float(open(__file__.replace("test_workloads_cpu.py", "golden/paper_dt.txt")).read().split()[-1])
+    dt = wl.courant_dt(0.8, 14.95e-3 / 512, 10.16e-3 / 4, 500e-3 / 512)
+    assert dt == pytest.approx(gold, rel=2e-5)      # dimensions as printed
+    dt = wl.courant_dt(0.8, 14.95e-3 / 512, 10.16e-3 / 4, 508e-3 / 512)
+    assert dt == pytest.approx(gold, rel=2e-7)      # L = 20 in reproduces the printed digits
+    # and the value SURVEY.md quotes for the configs (dx = 1 um, 0.9 Courant)
+    assert wl.courant_dt(0.9, 1e-6, 1e-6, 1e-6) == pytest.approx(1.7332498813918e-15, rel=1e-12)
+
+
+def test_paper_pulse_width_is_one_period():
+    """T_p = one period of f0 = 10.5 GHz = 0.095238 ns."""
+    assert 1.0 / 10.5e9 == pytest.approx(0.095238e-9, rel=1e-5)
+    # config 3's 40 % bandwidth reading (A15): spectral FWHM of exp(-t^2/2Tp^2) is 2 sqrt(2 ln 2)/(2 pi Tp)
+    tp = wl.bandwidth_tp(10e9, 0.4)
+    assert 2 * math.sqrt(2 * math.log(2)) / (2 * math.pi * tp) == pytest.approx(4e9)
+    assert tp * 10e9 == pytest.approx(0.937, abs=1e-3)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_small_configs_have_the_structure_of_the_full_ones(cfg):
+    w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
+    a = w.numpy()
+    nx, ny, nz = wl.SMALL_SHAPES[cfg]
+    assert w.dt == pytest.approx(0.9 * wl.courant_dt(1.0, w.dx, w.dy, w.dz))
+    for arr in a["E"] + a["H"] + a["M_cell"] + list(a["materials"].values()):
+        assert arr is None or arr.shape == (nz, ny, nx)
+    if cfg == 1:
+        assert w.bc == (0, 0, 0) and np.all(a["materials"]["Ms"] == 1.4e5)
+        m = np.stack(a["M_cell"])
+        assert np.allclose(np.linalg.norm(m, axis=0), 1.4e5, rtol=1e-14)
+        tilt = np.degrees(np.arccos(m[2] / 1.4e5))
+        assert 0.3 < tilt.max() <= 1.0 and a["E"][0].max() > 5e5
+    if cfg == 2:
+        assert w.bc == (1, 1, 1) and not w.enable_llg
+        assert abs(a["E"][1]).max() == pytest.approx(1.0, abs=1e-5)
+        assert 0 < abs(a["E"][0]).max() <= 1e-6
+    if cfg == 3:
+        eps, sig = a["materials"]["eps_r"], a["materials"]["sigma"]
+        assert set(np.unique(eps)) == {1.0, 11.7} and set(np.unique(sig)) == {0.0, 5.8e7}
+        assert np.all(sig[eps == 11.7] == 0) and len(w.sources) == 1 and w.sources[0].comp == 1
+        # two separate strips running the full x length
+        cols = np.nonzero(sig[nz // 8, :, 0])[0]
+        assert np.any(np.diff(cols) > 1) and np.all(sig[nz // 8, cols[0], :] == 5.8e7)
+    if cfg == 4:
+        Ms = a["materials"]["Ms"]
+        frac = (Ms > 0).mean()
+        assert 0.05 < frac < 0.12 and w.ani_hk == 2e3 and w.sources[0].comp == 0
+        assert w.sources[0].lo[2] > np.nonzero(Ms[:, 0, 0])[0].max()     # source above the slab
+    if cfg == 5:
+        Ms = a["materials"]["Ms"]
+        assert w.bc == (1, 1, 0) and (Ms > 0).mean() == pytest.approx(0.5, abs=0.02)
+        e = np.stack(a["E"])
+        assert abs(e.mean()) < 0.05 and e.std() == pytest.approx(1.0, abs=0.05)
+
+
+def test_full_size_configs_are_the_baseline_json_ones():
+    import inspect
+    shapes = {n: inspect.signature(f).parameters["shape"].default for n, f in wl.CONFIGS.items()}
+    assert shapes == {1: (32, 32, 32), 2: (256, 256, 256), 3: (512, 128, 128),
+                      4: (384, 384, 384), 5: (768, 768, 768)}
+    steps = {n: inspect.signature(f).parameters["steps"].default for n, f in wl.CONFIGS.items()}
+    assert steps == {1: 100, 2: 1000, 3: 2000, 4: 2000, 5: 200}
