@@ -4,6 +4,7 @@
 // buffer rotation of the Jacobi iterates, and the CUDA Graph of one time step.  All arithmetic of
 // the path is in kernels.cuh.  No device memory is allocated here: everything lives in the
 // caller's workspace.
+#include <algorithm>
 #include <climits>
 #include <cmath>
 #include <cstdarg>
@@ -25,6 +26,12 @@ constexpr size_t ALIGN_D = 32;  // arrays start on 256-byte boundaries
 
 size_t padded(size_t n) { return (n + ALIGN_D - 1) / ALIGN_D * ALIGN_D; }
 
+// device layout of one array (kernels.cuh "DEVICE LAYOUT"): one ghost layer, 128-byte aligned rows
+size_t row_pitch(int nx) { return ((size_t)PADL + nx + 1 + 15) / 16 * 16; }
+size_t array_stride(int nx, int ny, int nz) {
+  return padded(row_pitch(nx) * (size_t)(ny + 2) * (size_t)(nz + 2));
+}
+
 struct MatInfo {
   bool is_array = false;  // non-uniform: kept on the device
   double uniform = 0.0;   // value when uniform
@@ -36,7 +43,9 @@ struct MatInfo {
 struct fdtd_llg {
   GridP g{};
   double d[3]{}, dt = 0;
-  size_t ncell = 0, stride = 0;  // stride = padded(ncell)
+  size_t ncell = 0, stride = 0;  // stride = array_stride(): doubles between consecutive arrays
+  int num_sms = 148;
+  int sweep_blocks_per_sm = 4;
   fdtd_llg_options opt{};
   cudaStream_t stream = nullptr;
   char *ws = nullptr;
@@ -49,6 +58,9 @@ struct fdtd_llg {
   bool llg = false;  // LLG enabled AND at least one magnetic cell
   long long magnetic_cells = 0;
   int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
+  BoxP box_llg{}, box_all{};
+  BoxP box_out[6]{};     // the complement of the sweep box, as slabs
+  int n_out = 0;
 
   DevState *dstate = nullptr;
   unsigned long long *resid = nullptr;
@@ -84,8 +96,61 @@ int fail(fdtd_llg *s, int code, const char *fmt, ...) {
       return fail((s), FDTD_LLG_ECUDA, "%s: %s", #call, cudaGetErrorString(e_));         \
   } while (0)
 
-dim3 grid_for(int ex, int ey, int ez) {
-  return dim3((ex + BX - 1) / BX, (ey + BY - 1) / BY, (ez + BZ - 1) / BZ);
+// Work items: TX x TY columns marched over kz planes.  kz is as long as possible (amortises the
+// cold first plane of the prefetch pipeline) while leaving >= 8 items per SM.
+BoxP make_box(const fdtd_llg *s, const int lo[3], const int hi[3]) {
+  BoxP b{};
+  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
+  b.ntx = (hi[0] - lo[0] + TX - 1) / TX;
+  b.nty = (hi[1] - lo[1] + TY - 1) / TY;
+  const int ez = std::max(0, hi[2] - lo[2]);
+  int kz = std::min(KZ_MAX, std::max(1, ez));
+  while (kz > 1 && (long long)b.ntx * b.nty * ((ez + kz - 1) / kz) < 8LL * s->num_sms) kz = (kz + 1) / 2;
+  b.kz = kz;
+  b.items = b.ntx * b.nty * ((ez + kz - 1) / kz);
+  return b;
+}
+
+// blocks_per_sm == 0: one block per work item (the hardware scheduler balances the load);
+// otherwise a persistent grid of num_sms * blocks_per_sm blocks looping over the items
+int grid_for(const fdtd_llg *s, const BoxP &b, int blocks_per_sm) {
+  if (blocks_per_sm == 0) return std::max(1, b.items);
+  const long long want = (long long)s->num_sms * blocks_per_sm;
+  return (int)std::max(1LL, std::min<long long>(want, b.items));
+}
+int grid_1d(const fdtd_llg *s, long long n) {
+  return (int)std::max(1LL, std::min<long long>((long long)s->num_sms * 8, (n + 255) / 256));
+}
+
+// strided copies between a user's compact array and the ghosted device layout
+int copy_in(fdtd_llg *s, double *dev, const double *user, int mem_space) {
+  cudaMemcpy3DParms p{};
+  p.srcPtr = make_cudaPitchedPtr(const_cast<double *>(user), (size_t)s->g.n[0] * 8, (size_t)s->g.n[0] * 8, (size_t)s->g.n[1]);
+  p.dstPtr = make_cudaPitchedPtr(dev, (size_t)s->g.sy * 8, (size_t)s->g.sy * 8, (size_t)s->g.n[1] + 2);
+  p.dstPos = make_cudaPos((size_t)PADL * 8, 1, 1);
+  p.extent = make_cudaExtent((size_t)s->g.n[0] * 8, (size_t)s->g.n[1], (size_t)s->g.n[2]);
+  p.kind = mem_space == FDTD_LLG_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  cudaError_t e = cudaMemcpy3DAsync(&p, s->stream);
+  if (e != cudaSuccess) { s->err = std::string("cudaMemcpy3DAsync (in): ") + cudaGetErrorString(e); return FDTD_LLG_ECUDA; }
+  return FDTD_LLG_OK;
+}
+int copy_out(fdtd_llg *s, double *user, const double *dev, int mem_space) {
+  cudaMemcpy3DParms p{};
+  p.srcPtr = make_cudaPitchedPtr(const_cast<double *>(dev), (size_t)s->g.sy * 8, (size_t)s->g.sy * 8, (size_t)s->g.n[1] + 2);
+  p.srcPos = make_cudaPos((size_t)PADL * 8, 1, 1);
+  p.dstPtr = make_cudaPitchedPtr(user, (size_t)s->g.n[0] * 8, (size_t)s->g.n[0] * 8, (size_t)s->g.n[1]);
+  p.extent = make_cudaExtent((size_t)s->g.n[0] * 8, (size_t)s->g.n[1], (size_t)s->g.n[2]);
+  p.kind = mem_space == FDTD_LLG_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+  cudaError_t e = cudaMemcpy3DAsync(&p, s->stream);
+  if (e != cudaSuccess) { s->err = std::string("cudaMemcpy3DAsync (out): ") + cudaGetErrorString(e); return FDTD_LLG_ECUDA; }
+  return FDTD_LLG_OK;
+}
+int fill_ghosts(fdtd_llg *s, double *dev) {
+  const long long total = (long long)(s->g.n[0] + 2) * (s->g.n[1] + 2) * (s->g.n[2] + 2);
+  k_fill_ghosts<<<grid_1d(s, total), 256, 0, s->stream>>>(dev, s->g);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { s->err = std::string("k_fill_ghosts: ") + cudaGetErrorString(e); return FDTD_LLG_ECUDA; }
+  return FDTD_LLG_OK;
 }
 
 bool valid_opts(const fdtd_llg_options *o, const char **why) {
@@ -176,11 +241,10 @@ int take_material(fdtd_llg *s, MatInfo *m, const double *user, int mem_space, do
   m->is_array = true;
   m->dev = *slot;
   *slot += s->stride;
-  CU(s, cudaMemcpyAsync(m->dev, user, s->ncell * sizeof(double),
-                        mem_space == FDTD_LLG_HOST ? cudaMemcpyHostToDevice
-                                                   : cudaMemcpyDeviceToDevice,
-                        s->stream));
-  return FDTD_LLG_OK;
+  CU(s, cudaMemsetAsync(m->dev, 0, s->stride * sizeof(double), s->stream));
+  int rc = copy_in(s, m->dev, user, mem_space);
+  if (rc) return rc;
+  return fill_ghosts(s, m->dev);
 }
 
 int find_sweep_box(fdtd_llg *s) {
@@ -199,7 +263,7 @@ int find_sweep_box(fdtd_llg *s) {
     unsigned long long zero = 0;
     CU(s, cudaMemcpyAsync(box, init, sizeof init, cudaMemcpyHostToDevice, s->stream));
     CU(s, cudaMemcpyAsync(cnt, &zero, sizeof zero, cudaMemcpyHostToDevice, s->stream));
-    k_mag_box<<<1024, 256, 0, s->stream>>>(s->Ms.dev, s->g, box, cnt);
+    k_mag_box<<<grid_1d(s, (long long)s->ncell), 256, 0, s->stream>>>(s->Ms.dev, s->g, box, cnt);
     CU(s, cudaGetLastError());
     int out[6];
     unsigned long long c = 0;
@@ -224,11 +288,38 @@ int find_sweep_box(fdtd_llg *s) {
   return FDTD_LLG_OK;
 }
 
+// work decomposition: the sweep box, the whole grid, and the complement of the box as <= 6 slabs
+void make_boxes(fdtd_llg *s) {
+  const int zero[3] = {0, 0, 0};
+  s->box_all = make_box(s, zero, s->g.n);
+  s->n_out = 0;
+  if (!s->llg) {
+    s->box_out[s->n_out++] = s->box_all;
+    return;
+  }
+  s->box_llg = make_box(s, s->lo, s->hi);
+  int lo[3] = {0, 0, 0}, hi[3] = {s->g.n[0], s->g.n[1], s->g.n[2]};
+  for (int d = 2; d >= 0; --d) {  // peel z slabs first (contiguous planes), then y, then x
+    if (s->lo[d] > lo[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      h[d] = s->lo[d];
+      s->box_out[s->n_out++] = make_box(s, l, h);
+    }
+    if (s->hi[d] < hi[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      l[d] = s->hi[d];
+      s->box_out[s->n_out++] = make_box(s, l, h);
+    }
+    lo[d] = s->lo[d];
+    hi[d] = s->hi[d];
+  }
+}
+
 // ---- launching one step ----------------------------------------------------------------
 
 template <bool FIRST>
-int launch_sweep(fdtd_llg *s, const HMArgs &a, dim3 grid) {
-  const dim3 blk(BX, BY, BZ);
+int launch_sweep(fdtd_llg *s, const HMArgs &a, int grid) {
+  const dim3 blk(TX, TY, 1);
   const bool ms = s->Ms.is_array, ag = s->alpha.is_array || s->gamma.is_array,
              mu = s->mu_r.is_array, an = s->opt.ani_hk != 0.0;
 #define SW(MS, AG, MU, AN)                                                               \
@@ -250,18 +341,19 @@ int launch_sweep(fdtd_llg *s, const HMArgs &a, dim3 grid) {
 // M: time-n set `min`, result in set `mout`.
 int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool last,
                  int *launches) {
-  const dim3 blk(BX, BY, BZ);
+  const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
   for (int d = 0; d < 3; ++d) { h.E[d] = s->E[d]; h.Hn[d] = s->Hset[in][d]; h.Hc[d] = s->Hset[out][d]; }
   h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
   h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
-  h.has_box = s->llg;
-  for (int d = 0; d < 3; ++d) { h.lo[d] = s->lo[d]; h.hi[d] = s->hi[d]; }
-  bool box_is_all = s->llg;
-  for (int d = 0; d < 3; ++d) box_is_all = box_is_all && s->lo[d] == 0 && s->hi[d] == s->g.n[d];
-  if (!box_is_all) {
-    const dim3 grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+  h.npf = 0;
+  for (int d = 0; d < 3; ++d) { h.pf[h.npf++] = s->E[d]; h.pf[h.npf++] = s->Hset[in][d]; }
+  if (h.mu_r) h.pf[h.npf++] = h.mu_r;
+  for (int b = 0; b < s->n_out; ++b) {
+    h.box = s->box_out[b];
+    if (h.box.items == 0) continue;
+    const int grid = grid_for(s, h.box, 0);
     if (s->mu_r.is_array) k_h_update<true><<<grid, blk, 0, s->stream>>>(h);
     else k_h_update<false><<<grid, blk, 0, s->stream>>>(h);
     ++*launches;
@@ -269,23 +361,34 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
   if (s->llg) {
     HMArgs a{};
     a.g = s->g;
+    a.box = s->box_llg;
     for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.Hn[d] = s->Hset[in][d]; }
     for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
+    a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
     a.ch_uniform = h.ch_uniform;
     for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
     a.hk = s->opt.ani_hk;
     a.tol = s->opt.llg_tol;
-    for (int d = 0; d < 3; ++d) { a.lo[d] = s->lo[d]; a.hi[d] = s->hi[d]; }
     a.resid = s->resid;
-    const dim3 grid = grid_for(s->hi[0] - s->lo[0], s->hi[1] - s->lo[1], s->hi[2] - s->lo[2]);
     for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
+      // r <= 3 normally run: one block per item.  Later iterates almost never run: a small
+      // persistent grid keeps their early exit at launch-latency cost.
+      const int grid = grid_for(s, a.box, r <= 3 ? 0 : s->sweep_blocks_per_sm);
       // iterate r reads H^{r-1} and writes H^r: odd r -> `out`, even r -> `tmp`
       const int from = (r == 1) ? in : ((r & 1) ? tmp : out);
       const int to = (r & 1) ? out : tmp;
       for (int d = 0; d < 3; ++d) { a.Hp[d] = s->Hset[from][d]; a.Hc[d] = s->Hset[to][d]; }
       a.r = r;
+      a.npf = 0;
+      for (int d = 0; d < 3; ++d) { a.pf[a.npf++] = a.E[d]; a.pf[a.npf++] = a.Hn[d]; }
+      for (int q = 0; q < 9; ++q) a.pf[a.npf++] = a.Mn[q];
+      if (r > 1) {
+        for (int d = 0; d < 3; ++d) a.pf[a.npf++] = a.Hp[d];
+        for (int q = 0; q < 9; ++q) a.pf[a.npf++] = a.Mr[q];
+      }
+      if (a.Ms) a.pf[a.npf++] = a.Ms;
       int rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
       if (rc) return rc;
       ++*launches;
@@ -297,10 +400,10 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
   if (s->llg && s->opt.llg_max_iter >= 2) {
     CanonArgs c{};
     c.g = s->g;
-    for (int d = 0; d < 3; ++d) { c.src[d] = s->Hset[tmp][d]; c.dst[d] = s->Hset[out][d]; c.lo[d] = s->lo[d]; c.hi[d] = s->hi[d]; }
+    c.box = s->box_llg;
+    for (int d = 0; d < 3; ++d) { c.src[d] = s->Hset[tmp][d]; c.dst[d] = s->Hset[out][d]; }
     c.st = s->dstate;
-    const dim3 grid = grid_for(s->hi[0] - s->lo[0], s->hi[1] - s->lo[1], s->hi[2] - s->lo[2]);
-    k_canon<<<grid, blk, 0, s->stream>>>(c);
+    k_canon<<<grid_for(s, c.box, 8), blk, 0, s->stream>>>(c);
     ++*launches;
   }
   CU(s, cudaGetLastError());
@@ -308,15 +411,20 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
 }
 
 int enqueue_e(fdtd_llg *s, int hset, int *launches) {
-  const dim3 blk(BX, BY, BZ);
+  const dim3 blk(TX, TY, 1);
   EArgs a{};
   a.g = s->g;
+  a.box = s->box_all;
   for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.H[d] = s->Hset[hset][d]; }
   a.eps_r = s->eps_r.dev; a.sigma = s->sigma.dev;
   a.eps_u = kEps0 * s->eps_r.uniform; a.sigma_u = s->sigma.uniform;
   a.src = s->src;
   a.st = s->dstate;
-  const dim3 grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+  const int grid = grid_for(s, a.box, 0);
+  a.npf = 0;
+  for (int d = 0; d < 3; ++d) { a.pf[a.npf++] = a.E[d]; a.pf[a.npf++] = a.H[d]; }
+  if (a.eps_r) a.pf[a.npf++] = a.eps_r;
+  if (a.sigma) a.pf[a.npf++] = a.sigma;
   const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = s->src.count > 0;
 #define EK(EA, SA, HS)                                                        \
   if (ea == EA && sa == SA && hs == HS) k_e_update<EA, SA, HS><<<grid, blk, 0, s->stream>>>(a);
@@ -388,7 +496,7 @@ void fdtd_llg_default_options(fdtd_llg_options *o) {
 size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
                                 unsigned material_mask) {
   if (nx < 1 || ny < 1 || nz < 1 || !opt) return 0;
-  const size_t stride = padded((size_t)nx * ny * nz);
+  const size_t stride = array_stride(nx, ny, nz);
   size_t arrays = 6;                       // E, H
   if (opt->enable_llg) arrays += 6 + 18;   // two more H sets, two M sets
   for (unsigned b = 0; b < 6; ++b)
@@ -404,7 +512,8 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   if (!out) return fail(nullptr, FDTD_LLG_EINVAL, "out is NULL");
   *out = nullptr;
   if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, FDTD_LLG_EINVAL, "nx, ny, nz must be >= 1");
-  if ((double)nx * ny * nz > 2.0e9) return fail(nullptr, FDTD_LLG_EINVAL, "grid too large (> 2e9 cells)");
+  if ((double)row_pitch(nx) * (ny + 2.0) * (nz + 2.0) > 2.0e9)
+    return fail(nullptr, FDTD_LLG_EINVAL, "grid too large (> 2e9 elements per array with ghosts)");
   if (!(dx > 0) || !(dy > 0) || !(dz > 0) || !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz))
     return fail(nullptr, FDTD_LLG_EINVAL, "dx, dy, dz must be finite and > 0");
   if (!(dt > 0) || !std::isfinite(dt)) return fail(nullptr, FDTD_LLG_EINVAL, "dt must be finite and > 0");
@@ -424,13 +533,21 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   fdtd_llg *s = new (std::nothrow) fdtd_llg();
   if (!s) return fail(nullptr, FDTD_LLG_ENOMEM, "host allocation failed");
   s->g.n[0] = nx; s->g.n[1] = ny; s->g.n[2] = nz;
-  s->g.s[0] = 1; s->g.s[1] = nx; s->g.s[2] = (long long)nx * ny;
+  s->g.sy = (int)row_pitch(nx);
+  s->g.sz = s->g.sy * (ny + 2);
+  s->g.org = PADL + s->g.sy + s->g.sz;
   s->d[0] = dx; s->d[1] = dy; s->d[2] = dz;
   for (int d = 0; d < 3; ++d) { s->g.per[d] = opt->bc[d] == FDTD_LLG_PERIODIC; s->g.rd[d] = 1.0 / s->d[d]; }
   s->g.dt = dt;
   s->dt = dt;
   s->ncell = (size_t)nx * ny * nz;
-  s->stride = padded(s->ncell);
+  s->stride = array_stride(nx, ny, nz);
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      s->num_sms = sms;
+  }
   s->opt = *opt;
   if (!opt->enable_llg) { s->opt.llg_max_iter = 1; s->opt.llg_tol = 1.0; }
   s->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -479,6 +596,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
     if ((rc = take_material(s, &s->gamma, gamma, mem_space, 0.0, &q, "gamma", -INFINITY, false, 32u))) return bail(rc);
   }
   if ((rc = find_sweep_box(s))) return bail(rc);
+  make_boxes(s);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
   *out = s;
@@ -490,22 +608,26 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
   if (!s) return FDTD_LLG_EINVAL;
   if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
     return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
-  const size_t bytes = s->ncell * sizeof(double);
-  const dim3 blk(BX, BY, BZ), grid = grid_for(s->g.n[0], s->g.n[1], s->g.n[2]);
+  const size_t abytes = s->stride * sizeof(double);
+  int rc;
   for (int d = 0; d < 3; ++d) {
-    if (E && E[d]) CU(s, cudaMemcpyAsync(s->E[d], E[d], bytes, to_dev(mem_space), s->stream));
-    else CU(s, cudaMemsetAsync(s->E[d], 0, bytes, s->stream));
-    if (H && H[d]) CU(s, cudaMemcpyAsync(s->Hset[0][d], H[d], bytes, to_dev(mem_space), s->stream));
-    else CU(s, cudaMemsetAsync(s->Hset[0][d], 0, bytes, s->stream));
+    CU(s, cudaMemsetAsync(s->E[d], 0, abytes, s->stream));
+    CU(s, cudaMemsetAsync(s->Hset[0][d], 0, abytes, s->stream));
+    if (E && E[d] && (rc = copy_in(s, s->E[d], E[d], mem_space))) return rc;
+    if (H && H[d] && (rc = copy_in(s, s->Hset[0][d], H[d], mem_space))) return rc;
   }
   if (s->opt.enable_llg)
     for (int h = 1; h < 3; ++h)
-      for (int d = 0; d < 3; ++d) CU(s, cudaMemsetAsync(s->Hset[h][d], 0, bytes, s->stream));
+      for (int d = 0; d < 3; ++d) CU(s, cudaMemsetAsync(s->Hset[h][d], 0, abytes, s->stream));
   FieldsP f{};
   f.g = s->g;
   for (int d = 0; d < 3; ++d) { f.E[d] = s->E[d]; f.H[d] = s->Hset[0][d]; }
-  k_enforce_walls<<<grid, blk, 0, s->stream>>>(f);
+  k_enforce_walls<<<grid_1d(s, (long long)s->ncell), 256, 0, s->stream>>>(f);
   CU(s, cudaGetLastError());
+  for (int d = 0; d < 3; ++d) {
+    if ((rc = fill_ghosts(s, s->E[d]))) return rc;
+    if ((rc = fill_ghosts(s, s->Hset[0][d]))) return rc;
+  }
   // reset run state
   CU(s, cudaMemsetAsync(s->dstate, 0, sizeof(DevState), s->stream));
   CU(s, cudaMemsetAsync(s->resid, 0, (size_t)(s->opt.llg_max_iter + 2) * 8, s->stream));
@@ -514,23 +636,27 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
     a.g = s->g;
     for (int c = 0; c < 3; ++c) {
       a.Mc[c] = nullptr;
-      if (M_cell && M_cell[c]) {
-        if (mem_space == FDTD_LLG_DEVICE) {
-          a.Mc[c] = M_cell[c];
-        } else {  // stage the host array in the second M set
-          CU(s, cudaMemcpyAsync(s->Mset[1][c], M_cell[c], bytes, cudaMemcpyHostToDevice, s->stream));
-          a.Mc[c] = s->Mset[1][c];
-        }
+      if (M_cell && M_cell[c]) {  // stage the cell-centred array, ghosted, in the second M set
+        CU(s, cudaMemsetAsync(s->Mset[1][c], 0, abytes, s->stream));
+        if ((rc = copy_in(s, s->Mset[1][c], M_cell[c], mem_space))) return rc;
+        if ((rc = fill_ghosts(s, s->Mset[1][c]))) return rc;
+        a.Mc[c] = s->Mset[1][c];
       }
     }
-    for (int c = 0; c < 9; ++c) a.M[c] = s->Mset[0][c];
+    for (int c = 0; c < 9; ++c) {
+      CU(s, cudaMemsetAsync(s->Mset[0][c], 0, abytes, s->stream));
+      a.M[c] = s->Mset[0][c];
+    }
     a.Ms = s->Ms.dev;
     a.Ms_u = s->Ms.uniform;
     a.enable_llg = s->llg ? 1 : 0;
     a.st = s->dstate;
-    k_init_m<<<grid, blk, 0, s->stream>>>(a);
+    k_init_m<<<grid_1d(s, (long long)s->ncell), 256, 0, s->stream>>>(a);
     CU(s, cudaGetLastError());
-    for (int c = 0; c < 9; ++c) CU(s, cudaMemsetAsync(s->Mset[1][c], 0, bytes, s->stream));
+    for (int c = 0; c < 9; ++c) {
+      if ((rc = fill_ghosts(s, s->Mset[0][c]))) return rc;
+      CU(s, cudaMemsetAsync(s->Mset[1][c], 0, abytes, s->stream));
+    }
     int err = 0;
     CU(s, cudaMemcpyAsync(&err, &s->dstate->init_error, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
     CU(s, cudaStreamSynchronize(s->stream));
@@ -607,14 +733,15 @@ int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double
   if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
     return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
   const size_t bytes = s->ncell * sizeof(double);
+  int rc;
   for (int d = 0; d < 3; ++d) {
-    if (E && E[d]) CU(s, cudaMemcpyAsync(E[d], s->E[d], bytes, from_dev(mem_space), s->stream));
-    if (H && H[d]) CU(s, cudaMemcpyAsync(H[d], s->Hset[0][d], bytes, from_dev(mem_space), s->stream));
+    if (E && E[d] && (rc = copy_out(s, E[d], s->E[d], mem_space))) return rc;
+    if (H && H[d] && (rc = copy_out(s, H[d], s->Hset[0][d], mem_space))) return rc;
   }
   if (M)
     for (int c = 0; c < 9; ++c)
       if (M[c]) {
-        if (s->opt.enable_llg) CU(s, cudaMemcpyAsync(M[c], s->Mset[0][c], bytes, from_dev(mem_space), s->stream));
+        if (s->opt.enable_llg) { if ((rc = copy_out(s, M[c], s->Mset[0][c], mem_space))) return rc; }
         else if (mem_space == FDTD_LLG_HOST) std::memset(M[c], 0, bytes);
         else CU(s, cudaMemsetAsync(M[c], 0, bytes, s->stream));
       }

@@ -1,17 +1,30 @@
-// kernels.cuh -- sm_100a device code of the coupled FDTD-LLG step (fp64, HBM-bound stencils).
+// kernels.cuh -- sm_100a device code of the coupled FDTD-LLG step (fp64 stencils).
 //
-// Citations are /root/reference/PAPER.md lines of arXiv 2103.12819.  Layout and staggering:
-// include/fdtd_llg.h.  No ghost cells: periodic wrap and PEC walls are resolved per thread as
-// neighbour OFFSETS with a validity bit (a read beyond a PEC wall is the constant 0).
+// Citations are /root/reference/PAPER.md lines of arXiv 2103.12819.  Staggering: include/fdtd_llg.h.
+//
+// DEVICE LAYOUT.  Every array (fields and cell-centred materials) is stored with one ghost layer:
+//   element (i,j,k), -1 <= i <= nx, -1 <= j <= ny, -1 <= k <= nz, lives at
+//       org + i + sy*j + sz*k,   sy = row pitch (multiple of 16 doubles), sz = sy*(ny+2),
+//   with org chosen so that the interior row start (i = 0) is 128-byte aligned.  Ghosts of a PEC
+//   axis are zero for ever (a read beyond a PEC wall is the constant 0: wall-normal H and
+//   wall-tangential E vanish there); ghosts of a periodic axis mirror the opposite
+//   interior plane and are refreshed IN-KERNEL by the thread that writes the
+//   boundary cell.  Hence every stencil neighbour is a constant offset from the centre: no index
+//   arithmetic, no predicates in the inner loops.
+//
+// THREADING.  A block is TX x TY columns (x fastest, coalesced 256-byte rows) and marches KZ planes
+// in z, so the k-1 / k+1 neighbours of consecutive planes are served by L1.  Grids are persistent
+// (a multiple of the SM count) and loop over work items; an LLG sweep that finds the previous
+// iterate converged exits after one flag read.
 //
 // Kernels
-//   k_h_update   Maxwell (H) half-step on every face OUTSIDE the LLG sweep box   eq. 21 with M = 0
+//   k_h_update   Maxwell (H) half-step on the faces OUTSIDE the LLG sweep box     eq. 21 with M = 0
 //   k_hm_sweep   one Jacobi iterate r of the trapezoidal LLG solve + eq. 21 inside the sweep box
 //   k_half_end   1 thread: iteration count / statistics from the residual words, re-arm them
 //   k_canon      copies H^R into the canonical buffer when R is even
 //   k_e_update   eq. 11 with in-kernel edge means of eps_r, sigma and the soft sources
 //   k_step_begin source amplitudes g_s((n+1/2) dt) for this step
-//   set-up: k_enforce_walls, k_init_m, k_minmax, k_mag_box
+//   set-up: k_fill_ghosts, k_enforce_walls, k_init_m, k_minmax, k_mag_box
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -19,8 +32,11 @@
 namespace fl {
 
 constexpr int MAX_SOURCES = 8;
-constexpr int BX = 32, BY = 4, BZ = 2;  // thread block = BX x BY x BZ cells, x fastest
-constexpr int NTHREADS = BX * BY * BZ;
+constexpr int PADL = 16;         // doubles left of i = 0 in a row (ghost i = -1 sits at PADL-1)
+constexpr int TX = 32, TY = 8;   // thread block = TX x TY columns
+constexpr int NTHREADS = TX * TY;
+constexpr int KZ_MAX = 16;       // planes marched per work item (fewer on small grids)
+constexpr int MAX_PF = 32;       // arrays a kernel can prefetch
 
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kMu0 = 4.0e-7 * kPi;
@@ -28,11 +44,19 @@ constexpr double kC0 = 299792458.0;
 constexpr double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
 
 struct GridP {
-  int n[3];        // nx, ny, nz
-  int per[3];      // 1 = periodic, 0 = PEC
-  long long s[3];  // element strides 1, nx, nx*ny
-  double rd[3];    // 1/dx, 1/dy, 1/dz
+  int n[3];    // nx, ny, nz
+  int per[3];  // 1 = periodic, 0 = PEC
+  int sy, sz;  // element strides of j and k (the stride of i is 1)
+  int org;     // offset of cell (0,0,0)
+  double rd[3];  // 1/dx, 1/dy, 1/dz
   double dt;
+};
+
+// a box of cells cut into work items of TX x TY x kz
+struct BoxP {
+  int lo[3], hi[3];  // hi exclusive
+  int ntx, nty, items;
+  int kz;  // planes marched per work item
 };
 
 // device-resident run state (one per handle)
@@ -61,105 +85,175 @@ struct SourcesP {
   SourceP s[MAX_SOURCES];
 };
 
-// per-thread neighbourhood: centre index, wrapped neighbour offsets and their validity
-struct Stencil {
-  int idx[3];
-  long long c;
-  long long m[3], p[3];  // offset (elements) to the -1 / +1 neighbour along each axis
-  bool vm[3], vp[3];     // false: beyond a PEC wall (value 0)
+template <int D> __device__ __forceinline__ int stride_of(const GridP &g) {
+  return D == 0 ? 1 : (D == 1 ? g.sy : g.sz);
+}
+
+// this thread's cell
+struct Cell {
+  int i, j, k;
+  int c;      // element offset of (i,j,k)
+  bool edge;  // on the first / last plane of a periodic axis: its stores have ghost images
 };
 
-__device__ __forceinline__ Stencil make_stencil(const GridP &g, int i, int j, int k) {
-  Stencil st;
-  st.idx[0] = i; st.idx[1] = j; st.idx[2] = k;
-  st.c = (long long)i + g.s[1] * j + g.s[2] * k;
+// per-column (i,j) part of the predicates, hoisted out of the z march
+struct Column {
+  int i, j;
+  bool edge_ij;   // periodic first/last plane in x or y
+  bool wall[2];   // PEC lower wall in x / y
+};
+__device__ __forceinline__ Column make_column(const GridP &g, int i, int j) {
+  Column q;
+  q.i = i; q.j = j;
+  q.edge_ij = (g.per[0] && (i == 0 || i == g.n[0] - 1)) || (g.per[1] && (j == 0 || j == g.n[1] - 1));
+  q.wall[0] = !g.per[0] && i == 0;
+  q.wall[1] = !g.per[1] && j == 0;
+  return q;
+}
+__device__ __forceinline__ bool edge_k(const GridP &g, int k) {
+  return g.per[2] && (k == 0 || k == g.n[2] - 1);
+}
+__device__ __forceinline__ bool wall_k(const GridP &g, int k) { return !g.per[2] && k == 0; }
+
+// slow path of a store: the periodic ghost images of an interior value
+__device__ __noinline__ void store_images(double *a, const GridP &g, int i, int j, int k, int c,
+                                          double v) {
+  const int idx[3] = {i, j, k};
+  const int st[3] = {1, g.sy, g.sz};
+  int sh[3][3], cnt[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    const int v = st.idx[d], n = g.n[d];
-    st.vm[d] = (v > 0) || g.per[d];
-    st.vp[d] = (v < n - 1) || g.per[d];
-    st.m[d] = (v > 0) ? -g.s[d] : g.s[d] * (long long)(n - 1);
-    st.p[d] = (v < n - 1) ? g.s[d] : -g.s[d] * (long long)(n - 1);
+    cnt[d] = 0;
+    sh[d][cnt[d]++] = 0;
+    if (g.per[d]) {
+      if (idx[d] == 0) sh[d][cnt[d]++] = g.n[d] * st[d];            // ghost at index n
+      if (idx[d] == g.n[d] - 1) sh[d][cnt[d]++] = -g.n[d] * st[d];  // ghost at index -1
+    }
   }
-  return st;
-}
-
-__device__ __forceinline__ double ldv(const double *__restrict__ a, long long at, bool ok) {
-  return ok ? __ldg(a + at) : 0.0;
-}
-
-__device__ __forceinline__ bool wall_face(const GridP &g, const Stencil &st, int d) {
-  return !g.per[d] && st.idx[d] == 0;
-}
-__device__ __forceinline__ bool wall_edge(const GridP &g, const Stencil &st, int d) {
-  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
-  return (!g.per[t1] && st.idx[t1] == 0) || (!g.per[t2] && st.idx[t2] == 0);
+  for (int x = 0; x < cnt[0]; ++x)
+    for (int y = 0; y < cnt[1]; ++y)
+      for (int z = 0; z < cnt[2]; ++z)
+        if (x | y | z) a[c + sh[0][x] + sh[1][y] + sh[2][z]] = v;
 }
 
 // (curl E)_D at the D-face: forward differences (standard Yee)
 template <int D>
-__device__ __forceinline__ double curl_e(const GridP &g, const Stencil &st,
-                                         const double *const *E) {
+__device__ __forceinline__ double curl_e(const GridP &g, int c, const double *const *E) {
   constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
-  const double a0 = __ldg(E[d2] + st.c), a1 = ldv(E[d2], st.c + st.p[d1], st.vp[d1]);
-  const double b0 = __ldg(E[d1] + st.c), b1 = ldv(E[d1], st.c + st.p[d2], st.vp[d2]);
+  const int s1 = stride_of<d1>(g), s2 = stride_of<d2>(g);
+  const double a0 = __ldg(E[d2] + c), a1 = __ldg(E[d2] + c + s1);
+  const double b0 = __ldg(E[d1] + c), b1 = __ldg(E[d1] + c + s2);
   return (a1 - a0) * g.rd[d1] - (b1 - b0) * g.rd[d2];
 }
 
 // transverse component T of H at the D-face: four-point average
 template <int D, int T>
-__device__ __forceinline__ double avg4(const Stencil &st, const double *__restrict__ Ht) {
-  const double v00 = __ldg(Ht + st.c);
-  const double v10 = ldv(Ht, st.c + st.m[D], st.vm[D]);
-  const double v01 = ldv(Ht, st.c + st.p[T], st.vp[T]);
-  const double v11 = ldv(Ht, st.c + st.m[D] + st.p[T], st.vm[D] && st.vp[T]);
+__device__ __forceinline__ double avg4(const GridP &g, int c, const double *__restrict__ Ht) {
+  const int sd = stride_of<D>(g), st = stride_of<T>(g);
+  const double v00 = __ldg(Ht + c), v10 = __ldg(Ht + c - sd);
+  const double v01 = __ldg(Ht + c + st), v11 = __ldg(Ht + c - sd + st);
   return 0.25 * ((v00 + v10) + (v01 + v11));
+}
+
+// work-item decode shared by the sweeping kernels
+struct Item {
+  int i, j, k0, k1;
+  int i0, j0, rows, width;  // tile origin and its valid extent (for the plane prefetch)
+  bool active;
+};
+__device__ __forceinline__ Item decode_item(const BoxP &b, int it) {
+  const int tx = it % b.ntx, r = it / b.ntx;
+  const int ty = r % b.nty, tz = r / b.nty;
+  Item w;
+  w.i0 = b.lo[0] + tx * TX;
+  w.j0 = b.lo[1] + ty * TY;
+  w.i = w.i0 + (int)threadIdx.x;
+  w.j = w.j0 + (int)threadIdx.y;
+  w.rows = min(TY, b.hi[1] - w.j0);
+  w.width = min(TX, b.hi[0] - w.i0);
+  w.k0 = b.lo[2] + tz * b.kz;
+  w.k1 = min(w.k0 + b.kz, b.hi[2]);
+  w.active = w.i < b.hi[0] && w.j < b.hi[1];
+  return w;
+}
+
+// L2 prefetch of the NEXT z-plane of this block's tile: one cp.async.bulk.prefetch per
+// (array, row), issued by one thread each, so that the z march finds its streamed operands in
+// L2 instead of paying the HBM latency.  A hint only: rows are widened to 16-byte alignment.
+// ptrs[n]: the arrays; c_row0: offset of (tile x0, tile y0, k+1); rows: valid rows of the tile.
+__device__ __forceinline__ void prefetch_plane(const double *const *ptrs, int n, int c_row0, int sy,
+                                               int rows, int width) {
+  const int t = threadIdx.x + TX * threadIdx.y;
+  for (int q = t; q < n * TY; q += NTHREADS) {
+    const int arr = q / TY, row = q % TY;
+    if (row < rows) {
+      const unsigned long long addr =
+          (unsigned long long)(ptrs[arr] + c_row0 + row * sy) & ~15ull;
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(addr), "r"((width * 8 + 23) & ~15)
+                   : "memory");
+    }
+  }
 }
 
 // ------------------------------------------------------------------ Maxwell H half-step
 
 struct HArgs {
   GridP g;
+  BoxP box;            // the cells this launch updates (a slab of the complement of the LLG box)
   const double *E[3];
   const double *Hn[3];
   double *Hc[3];
   const double *mu_r;  // cell-centred array or nullptr (uniform)
   double ch_uniform;   // dt / (2 mu0 mu_r) when uniform
-  int has_box;
-  int lo[3], hi[3];    // LLG sweep box (cells handled by k_hm_sweep), excluded here
+  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
+  int npf;
 };
 
+// eq. 21 with M = 0 and the local mu; a PEC wall face stays 0
 template <int D, bool MU_ARR>
-__device__ __forceinline__ void h_face(const HArgs &a, const Stencil &st) {
-  if (wall_face(a.g, st, D)) return;  // stays 0
+__device__ __forceinline__ double h_face(const HArgs &a, int c, bool wall) {
   double ch = a.ch_uniform;
   if (MU_ARR) {
-    const double mu = 0.5 * (__ldg(a.mu_r + st.c) + __ldg(a.mu_r + st.c + st.m[D]));
+    const double mu = 0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + c - stride_of<D>(a.g)));
     ch = a.g.dt / (2.0 * kMu0 * mu);
   }
-  const double C = curl_e<D>(a.g, st, a.E);
-  a.Hc[D][st.c] = __ldg(a.Hn[D] + st.c) - ch * C;  // eq. 21 with M = 0, local mu
+  const double C = curl_e<D>(a.g, c, a.E);
+  // plain load: Hn aliases Hc when the update is done in place (Maxwell-only runs)
+  const double h = a.Hn[D][c] - ch * C;
+  return wall ? 0.0 : h;
 }
 
 template <bool MU_ARR>
 __global__ void __launch_bounds__(NTHREADS) k_h_update(const __grid_constant__ HArgs a) {
-  const int i = blockIdx.x * BX + threadIdx.x;
-  const int j = blockIdx.y * BY + threadIdx.y;
-  const int k = blockIdx.z * BZ + threadIdx.z;
-  if (i >= a.g.n[0] || j >= a.g.n[1] || k >= a.g.n[2]) return;
-  if (a.has_box && i >= a.lo[0] && i < a.hi[0] && j >= a.lo[1] && j < a.hi[1] && k >= a.lo[2] &&
-      k < a.hi[2])
-    return;
-  const Stencil st = make_stencil(a.g, i, j, k);
-  h_face<0, MU_ARR>(a, st);
-  h_face<1, MU_ARR>(a, st);
-  h_face<2, MU_ARR>(a, st);
+  for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
+    const Item w = decode_item(a.box, it);
+    const Column col = make_column(a.g, w.i, w.j);
+    int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
+    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
+    for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
+      c_tile += a.g.sz;
+      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
+      if (!w.active) continue;
+      const double hx = h_face<0, MU_ARR>(a, c, col.wall[0]);
+      const double hy = h_face<1, MU_ARR>(a, c, col.wall[1]);
+      const double hz = h_face<2, MU_ARR>(a, c, wall_k(a.g, k));
+      a.Hc[0][c] = hx;
+      a.Hc[1][c] = hy;
+      a.Hc[2][c] = hz;
+      if (col.edge_ij || edge_k(a.g, k)) {
+        store_images(a.Hc[0], a.g, w.i, w.j, k, c, hx);
+        store_images(a.Hc[1], a.g, w.i, w.j, k, c, hy);
+        store_images(a.Hc[2], a.g, w.i, w.j, k, c, hz);
+      }
+    }
+  }
 }
 
 // ------------------------------------------------------------------ LLG sweep
 
 struct HMArgs {
   GridP g;
+  BoxP box;             // the LLG sweep box
   const double *E[3];
   const double *Hn[3];  // H^n
   const double *Hp[3];  // H^{r-1}  (== Hn when FIRST)
@@ -167,12 +261,13 @@ struct HMArgs {
   const double *Mn[9];  // M^n      [face*3 + comp]
   double *Mr[9];        // M^{r-1} in, M^r out (same thread); FIRST: out only
   const double *Ms, *alpha, *gamma, *mu_r;  // cell-centred arrays or nullptr (uniform)
-  double Ms_u, alpha_u, gamma_u, ch_uniform;
+  double Ms_u, rMs_u, alpha_u, gamma_u, ch_uniform;
   double hb[3], hk, u[3];
   double tol;
-  int lo[3], hi[3];
   unsigned long long *resid;  // [max_iter + 1] bit patterns of the residual of iterate r
   int r;
+  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
+  int npf;
 };
 
 struct Vec3 { double x, y, z; };
@@ -188,97 +283,157 @@ template <int D> __device__ __forceinline__ double comp(const Vec3 &v) {
 
 // H_EM at the D-face from one H set: own normal component + two four-point averages
 template <int D>
-__device__ __forceinline__ Vec3 h_em(const Stencil &st, const double *const *H) {
+__device__ __forceinline__ Vec3 h_em(const GridP &g, int c, const double *const *H) {
   Vec3 h;
   if (D == 0) {
-    h.x = __ldg(H[0] + st.c); h.y = avg4<0, 1>(st, H[1]); h.z = avg4<0, 2>(st, H[2]);
+    h.x = __ldg(H[0] + c); h.y = avg4<0, 1>(g, c, H[1]); h.z = avg4<0, 2>(g, c, H[2]);
   } else if (D == 1) {
-    h.x = avg4<1, 0>(st, H[0]); h.y = __ldg(H[1] + st.c); h.z = avg4<1, 2>(st, H[2]);
+    h.x = avg4<1, 0>(g, c, H[0]); h.y = __ldg(H[1] + c); h.z = avg4<1, 2>(g, c, H[2]);
   } else {
-    h.x = avg4<2, 0>(st, H[0]); h.y = avg4<2, 1>(st, H[1]); h.z = __ldg(H[2] + st.c);
+    h.x = avg4<2, 0>(g, c, H[0]); h.y = avg4<2, 1>(g, c, H[1]); h.z = __ldg(H[2] + c);
   }
   return h;
 }
 
-// One Jacobi iterate on the D-face of this thread's cell.  Returns the face's residual
-// max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces).
-template <int D, bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
-__device__ __forceinline__ double hm_face(const HMArgs &a, const Stencil &st) {
-  if (wall_face(a.g, st, D)) return 0.0;  // H = 0, M = 0 for ever (reading A13)
-  const long long c = st.c, cm = st.c + st.m[D];
-  double Msf = a.Ms_u;
-  if (MS_ARR) Msf = 0.5 * (__ldg(a.Ms + c) + __ldg(a.Ms + cm));
-  if (!(Msf > 0.0)) {
-    // non-magnetic face inside the sweep box: Maxwell update at r = 1, copy afterwards so that
-    // both Jacobi buffers hold it
-    if (FIRST) {
-      double ch = a.ch_uniform;
-      if (MU_ARR) ch = a.g.dt / (2.0 * kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + cm))));
-      a.Hc[D][c] = __ldg(a.Hn[D] + c) - ch * curl_e<D>(a.g, st, a.E);
-    } else {
-      a.Hc[D][c] = __ldg(a.Hp[D] + c);
-    }
-    return 0.0;
+// 1/(1+y), y >= 0.  For y < 6e-5 the alternating series through y^3 is exact to 1.3e-17
+// relative (y = |a|^2 is ~1e-10 at any physical field strength); otherwise the division.
+__device__ __forceinline__ double recip_1p(double y) {
+  if (y < 6.0e-5) return fma(y, fma(y, 1.0 - y, -1.0), 1.0);
+  return 1.0 / (1.0 + y);
+}
+
+// (1+x)^(-1/2) - 1 = Ms/|M^n + Delta| - 1  (PAPER.md:98, 179 applied to the increment).
+// |x| < 1e-4: Maclaurin series through x^4 (truncation 63/256 x^5 < 5e-17 relative);
+// otherwise -x / (s (1 + s)), s = sqrt(1+x) -- both free of cancellation.
+__device__ __forceinline__ double rsqrt_1p_m1(double x) {
+  if (fabs(x) < 1.0e-4)
+    return x * fma(x, fma(x, fma(x, 35.0 / 128.0, -5.0 / 16.0), 3.0 / 8.0), -0.5);
+  const double sq = sqrt(1.0 + x);
+  return -x / (sq * (1.0 + sq));
+}
+
+// The increment form of eqs. 18-20 + N(M) on one face (reading A24):
+//   b = M^n + beta,  tau = a x M^n,  Delta = (18) - M^n,  dM = M^r - M^n.
+// mn = M^n, hn = H_eff^n, he = H_eff^{r-1} (FIRST: he == hn).
+template <bool FIRST>
+__device__ __forceinline__ Vec3 llg_increment(const Vec3 &mn, const Vec3 &hn, const Vec3 &he,
+                                              double cf, double aM, double rMs) {
+  const Vec3 t0 = cross(mn, hn);
+  const Vec3 beta = {-cf * t0.x, -cf * t0.y, -cf * t0.z};                      // (20) - M^n
+  const Vec3 av = {-(cf * he.x + aM * mn.x), -(cf * he.y + aM * mn.y), -(cf * he.z + aM * mn.z)};  // (19)
+  const Vec3 axb = cross(av, beta);
+  const double ab = dot(av, beta);
+  const double rden = recip_1p(dot(av, av));
+  Vec3 De;  // (18) - M^n
+  if (FIRST) {  // tau = -beta
+    De = {(2.0 * (beta.x - axb.x) + ab * av.x) * rden, (2.0 * (beta.y - axb.y) + ab * av.y) * rden,
+          (2.0 * (beta.z - axb.z) + ab * av.z) * rden};
+  } else {
+    const Vec3 t1 = cross(mn, he);
+    const Vec3 tau = {cf * t1.x, cf * t1.y, cf * t1.z};
+    const Vec3 axt = cross(av, tau);
+    De = {(beta.x - tau.x + axt.x + ab * av.x - axb.x) * rden,
+          (beta.y - tau.y + axt.y + ab * av.y - axb.y) * rden,
+          (beta.z - tau.z + axt.z + ab * av.z - axb.z) * rden};
   }
-  double alf = a.alpha_u, gam = a.gamma_u;
+  const double x = (2.0 * dot(mn, De) + dot(De, De)) * (rMs * rMs);
+  const double sm1 = rsqrt_1p_m1(x);
+  return {De.x + sm1 * (mn.x + De.x), De.y + sm1 * (mn.y + De.y), De.z + sm1 * (mn.z + De.z)};
+}
+
+// result of one face: M^r, H^r (normal component), residual
+struct FaceOut {
+  Vec3 m;
+  double h;
+  double res;
+};
+
+// One Jacobi iterate on the D-face of the cell at offset c, BRANCH-FREE: every load is a
+// constant offset from c (always in bounds thanks to the ghost layer) and is issued
+// unconditionally, so the compiler batches all of a face's loads ahead of the arithmetic; the
+// magnetic / non-magnetic / wall decision is a select at the end.  (A non-magnetic face runs the
+// LLG arithmetic on rMs = 0 and discards it.)  The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f
+// (0 on non-magnetic faces).  Ms_c / rMs_c: this cell's Ms and its reciprocal, shared by the
+// three faces wherever Ms is locally uniform.
+template <int D, bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
+__device__ __forceinline__ FaceOut hm_face(const HMArgs &a, int c, bool wall, double Ms_c,
+                                           double rMs_c) {
+  const int cm = c - stride_of<D>(a.g);
+  // ---- loads
+  double Ms_m = Ms_c;
+  if (MS_ARR) Ms_m = __ldg(a.Ms + cm);
+  const Vec3 mn = {__ldcs(a.Mn[3 * D + 0] + c), __ldcs(a.Mn[3 * D + 1] + c),
+                   __ldcs(a.Mn[3 * D + 2] + c)};
+  Vec3 mp = mn;
+  if (!FIRST)
+    mp = {__ldcs(a.Mr[3 * D + 0] + c), __ldcs(a.Mr[3 * D + 1] + c), __ldcs(a.Mr[3 * D + 2] + c)};
+  Vec3 hn = h_em<D>(a.g, c, a.Hn);
+  Vec3 he = hn;
+  if (!FIRST) he = h_em<D>(a.g, c, a.Hp);
+  const double C = curl_e<D>(a.g, c, a.E);
+  double alf = a.alpha_u, gam = a.gamma_u, ch = a.ch_uniform;
   if (AG_ARR) {
     alf = 0.5 * (__ldg(a.alpha + c) + __ldg(a.alpha + cm));
     gam = 0.5 * (fabs(__ldg(a.gamma + c)) + fabs(__ldg(a.gamma + cm)));  // |gamma| (eqs. 19-20)
   }
+  if (MU_ARR) ch = a.g.dt / (2.0 * kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + cm))));
+  const double hn_own = comp<D>(hn), hp_own = comp<D>(he);
+
+  // ---- magnetic face: eqs. 18-21
+  const double Msf = 0.5 * (Ms_c + Ms_m);
+  const bool magnetic = !wall && Msf > 0.0;
+  double rMs = rMs_c;
+  if (MS_ARR && Ms_m != Ms_c) rMs = Msf > 0.0 ? 1.0 / Msf : 0.0;
   const double cf = kMu0 * gam * a.g.dt * 0.25;  // mu0 |gamma| dt / 4
-  const double rMs = 1.0 / Msf;
   const Vec3 hb = {a.hb[0], a.hb[1], a.hb[2]};
   const Vec3 u = {a.u[0], a.u[1], a.u[2]};
-
-  const Vec3 mn = {__ldg(a.Mn[3 * D + 0] + c), __ldg(a.Mn[3 * D + 1] + c),
-                   __ldg(a.Mn[3 * D + 2] + c)};
   // H_eff^n = H_EM^n + H_bias + H_k (M^n.u / Ms) u            (A19)
-  Vec3 hn = h_em<D>(st, a.Hn);
   hn.x += hb.x; hn.y += hb.y; hn.z += hb.z;
   if (ANISO) {
     const double p = a.hk * (dot(mn, u) * rMs);
     hn.x += p * u.x; hn.y += p * u.y; hn.z += p * u.z;
   }
   // H_eff^{r-1}, lagged; at r = 1 it is H_eff^n
-  Vec3 he = hn, mp = mn;
-  if (!FIRST) {
-    mp = {a.Mr[3 * D + 0][c], a.Mr[3 * D + 1][c], a.Mr[3 * D + 2][c]};
-    he = h_em<D>(st, a.Hp);
+  if (FIRST) {
+    he = hn;
+  } else {
     he.x += hb.x; he.y += hb.y; he.z += hb.z;
     if (ANISO) {
       const double p = a.hk * (dot(mp, u) * rMs);
       he.x += p * u.x; he.y += p * u.y; he.z += p * u.z;
     }
   }
-  // eqs. 18-20 in increment form (A24):  b = M^n + beta,  tau = a x M^n
-  const Vec3 t0 = cross(mn, hn);
-  const Vec3 beta = {-cf * t0.x, -cf * t0.y, -cf * t0.z};
-  const Vec3 t1 = cross(mn, he);
-  const Vec3 tau = {cf * t1.x, cf * t1.y, cf * t1.z};
-  const double aM = alf * rMs;
-  const Vec3 av = {-(cf * he.x + aM * mn.x), -(cf * he.y + aM * mn.y), -(cf * he.z + aM * mn.z)};  // (19)
-  const Vec3 axt = cross(av, tau), axb = cross(av, beta);
-  const double ab = dot(av, beta);
-  const double rden = 1.0 / (1.0 + dot(av, av));
-  const Vec3 De = {(beta.x - tau.x + axt.x + ab * av.x - axb.x) * rden,
-                   (beta.y - tau.y + axt.y + ab * av.y - axb.y) * rden,
-                   (beta.z - tau.z + axt.z + ab * av.z - axb.z) * rden};  // (18) - M^n
-  // renormalisation N(M) applied to the increment
-  const double x = (2.0 * dot(mn, De) + dot(De, De)) * (rMs * rMs);
-  const double sq = sqrt(1.0 + x);
-  const double sm1 = -x / (sq * (1.0 + sq));  // Ms/|M^n + Delta| - 1
-  const Vec3 dM = {De.x + sm1 * (mn.x + De.x), De.y + sm1 * (mn.y + De.y),
-                   De.z + sm1 * (mn.z + De.z)};
+  const Vec3 dM = llg_increment<FIRST>(mn, hn, he, cf, alf * rMs, rMs);
   const Vec3 mr = {mn.x + dM.x, mn.y + dM.y, mn.z + dM.z};
-  a.Mr[3 * D + 0][c] = mr.x;
-  a.Mr[3 * D + 1][c] = mr.y;
-  a.Mr[3 * D + 2][c] = mr.z;
   // eq. 21, normal component:  H^r = H^n + M^n - M^r - (dt / 2 mu0) curl E
-  const double C = curl_e<D>(a.g, st, a.E);
-  a.Hc[D][c] = __ldg(a.Hn[D] + c) - comp<D>(dM) - (a.g.dt / (2.0 * kMu0)) * C;
+  const double h_mag = hn_own - comp<D>(dM) - (a.g.dt / (2.0 * kMu0)) * C;
   // stopping test of PAPER.md:154, per face; reduced by the caller
   const double e = fmax(fmax(fabs(mr.x - mp.x), fabs(mr.y - mp.y)), fabs(mr.z - mp.z));
-  return e * rMs;
+
+  // ---- non-magnetic face inside the sweep box: Maxwell update at r = 1, copy afterwards so that
+  // both Jacobi buffers hold it.  PEC wall face: H = 0, M = 0 for ever (A13).
+  const double h_non = wall ? 0.0 : (FIRST ? hn_own - ch * C : hp_own);
+  FaceOut o;
+  o.m = {magnetic ? mr.x : 0.0, magnetic ? mr.y : 0.0, magnetic ? mr.z : 0.0};
+  o.h = magnetic ? h_mag : h_non;
+  o.res = magnetic ? e * rMs : 0.0;
+  return o;
+}
+
+template <int D>
+__device__ __forceinline__ void store_face(const HMArgs &a, int c, const FaceOut &o) {
+  __stcs(a.Mr[3 * D + 0] + c, o.m.x);
+  __stcs(a.Mr[3 * D + 1] + c, o.m.y);
+  __stcs(a.Mr[3 * D + 2] + c, o.m.z);
+  a.Hc[D][c] = o.h;
+}
+template <int D>
+__device__ __forceinline__ void store_face_images(const HMArgs &a, int i, int j, int k, int c,
+                                                  const FaceOut &o) {
+  store_images(a.Mr[3 * D + 0], a.g, i, j, k, c, o.m.x);
+  store_images(a.Mr[3 * D + 1], a.g, i, j, k, c, o.m.y);
+  store_images(a.Mr[3 * D + 2], a.g, i, j, k, c, o.m.z);
+  store_images(a.Hc[D], a.g, i, j, k, c, o.h);
 }
 
 template <bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
@@ -287,21 +442,47 @@ __global__ void __launch_bounds__(NTHREADS) k_hm_sweep(const __grid_constant__ H
   if (!FIRST) {
     if (__longlong_as_double((long long)a.resid[a.r - 1]) < a.tol) return;
   }
-  const int i = a.lo[0] + blockIdx.x * BX + threadIdx.x;
-  const int j = a.lo[1] + blockIdx.y * BY + threadIdx.y;
-  const int k = a.lo[2] + blockIdx.z * BZ + threadIdx.z;
   double res = 0.0;
-  if (i < a.hi[0] && j < a.hi[1] && k < a.hi[2]) {
-    const Stencil st = make_stencil(a.g, i, j, k);
-    res = hm_face<0, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, st);
-    res = fmax(res, hm_face<1, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, st));
-    res = fmax(res, hm_face<2, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, st));
+  for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
+    const Item w = decode_item(a.box, it);
+    const Column col = make_column(a.g, w.i, w.j);
+    int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
+    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
+    for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
+      c_tile += a.g.sz;
+      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
+      if (!w.active) continue;
+      double Ms_c = a.Ms_u, rMs_c = a.rMs_u;
+      if (MS_ARR) {
+        Ms_c = __ldg(a.Ms + c);
+        rMs_c = Ms_c > 0.0 ? 1.0 / Ms_c : 0.0;
+      }
+      const bool edge = col.edge_ij || edge_k(a.g, k);
+      {
+        const FaceOut o = hm_face<0, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, c, col.wall[0], Ms_c, rMs_c);
+        store_face<0>(a, c, o);
+        if (edge) store_face_images<0>(a, w.i, w.j, k, c, o);
+        res = fmax(res, o.res);
+      }
+      {
+        const FaceOut o = hm_face<1, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, c, col.wall[1], Ms_c, rMs_c);
+        store_face<1>(a, c, o);
+        if (edge) store_face_images<1>(a, w.i, w.j, k, c, o);
+        res = fmax(res, o.res);
+      }
+      {
+        const FaceOut o = hm_face<2, FIRST, MS_ARR, AG_ARR, MU_ARR, ANISO>(a, c, wall_k(a.g, k), Ms_c, rMs_c);
+        store_face<2>(a, c, o);
+        if (edge) store_face_images<2>(a, w.i, w.j, k, c, o);
+        res = fmax(res, o.res);
+      }
+    }
   }
   // convergence word: warp shuffles, then ONE atomic per block
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) res = fmax(res, __shfl_xor_sync(0xffffffffu, res, o));
   __shared__ double wmax[NTHREADS / 32];
-  const int tid = threadIdx.x + BX * (threadIdx.y + BY * threadIdx.z);
+  const int tid = threadIdx.x + TX * threadIdx.y;
   if ((tid & 31) == 0) wmax[tid >> 5] = res;
   __syncthreads();
   if (tid == 0) {
@@ -337,85 +518,120 @@ __global__ void k_half_end(DevState *st, unsigned long long *resid, int max_iter
 
 struct CanonArgs {
   GridP g;
+  BoxP box;
   const double *src[3];
   double *dst[3];
-  int lo[3], hi[3];
   const DevState *st;
 };
 
 __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ CanonArgs a) {
   if (!a.st->last_R_even) return;
-  const int i = a.lo[0] + blockIdx.x * BX + threadIdx.x;
-  const int j = a.lo[1] + blockIdx.y * BY + threadIdx.y;
-  const int k = a.lo[2] + blockIdx.z * BZ + threadIdx.z;
-  if (i >= a.hi[0] || j >= a.hi[1] || k >= a.hi[2]) return;
-  const long long c = (long long)i + a.g.s[1] * j + a.g.s[2] * k;
+  for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
+    const Item w = decode_item(a.box, it);
+    if (!w.active) continue;
+    const Column col = make_column(a.g, w.i, w.j);
+    int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
+    for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
+      const bool edge = col.edge_ij || edge_k(a.g, k);
 #pragma unroll
-  for (int d = 0; d < 3; ++d) a.dst[d][c] = __ldg(a.src[d] + c);
+      for (int d = 0; d < 3; ++d) {
+        const double v = __ldg(a.src[d] + c);
+        a.dst[d][c] = v;
+        if (edge) store_images(a.dst[d], a.g, w.i, w.j, k, c, v);
+      }
+    }
+  }
 }
 
 // ------------------------------------------------------------------ E update (eq. 11)
 
 struct EArgs {
   GridP g;
+  BoxP box;  // the whole grid
   double *E[3];
   const double *H[3];
   const double *eps_r, *sigma;  // cell-centred arrays or nullptr (uniform)
   double eps_u, sigma_u;        // uniform values (eps_u is eps0*eps_r)
   SourcesP src;
   const DevState *st;
+  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
+  int npf;
 };
 
-template <int D, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
-__device__ __forceinline__ void e_edge(const EArgs &a, const Stencil &st) {
-  if (wall_edge(a.g, st, D)) return;  // tangential E on a PEC wall stays 0
+// eq. 11 on the D-edge of the cell at offset c; a wall-tangential edge stays 0
+// (PAPER.md:187).  J = soft source term of this edge.
+template <int D, bool EPS_ARR, bool SIG_ARR>
+__device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, double J) {
   constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
-  const long long c = st.c;
+  const int s1 = stride_of<d1>(a.g), s2 = stride_of<d2>(a.g);
   // (curl H)_D at the D-edge: backward differences
-  const double h2 = __ldg(a.H[d2] + c), h2m = ldv(a.H[d2], c + st.m[d1], st.vm[d1]);
-  const double h1 = __ldg(a.H[d1] + c), h1m = ldv(a.H[d1], c + st.m[d2], st.vm[d2]);
-  const double curl = (h2 - h2m) * a.g.rd[d1] - (h1 - h1m) * a.g.rd[d2];
+  const double h2 = __ldg(a.H[d2] + c), h2m = __ldg(a.H[d2] + c - s1);
+  const double h1 = __ldg(a.H[d1] + c), h1m = __ldg(a.H[d1] + c - s2);
+  const double e0 = a.E[D][c];
   // four-cell means of eps, sigma at the edge
   double eps = a.eps_u, sig = a.sigma_u;
-  const long long c1 = c + st.m[d1], c2 = c + st.m[d2], c12 = c + st.m[d1] + st.m[d2];
   if (EPS_ARR)
-    eps = kEps0 * (0.25 * ((__ldg(a.eps_r + c) + __ldg(a.eps_r + c1)) +
-                           (__ldg(a.eps_r + c2) + __ldg(a.eps_r + c12))));
+    eps = kEps0 * (0.25 * ((__ldg(a.eps_r + c) + __ldg(a.eps_r + c - s1)) +
+                           (__ldg(a.eps_r + c - s2) + __ldg(a.eps_r + c - s1 - s2))));
   if (SIG_ARR)
-    sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c1)) +
-                  (__ldg(a.sigma + c2) + __ldg(a.sigma + c12)));
-  double J = 0.0;
-  if (HAS_SRC) {
-    for (int s = 0; s < a.src.count; ++s) {
-      const SourceP &S = a.src.s[s];
-      if (S.comp != D) continue;
-      if (st.idx[0] < S.lo[0] || st.idx[0] >= S.hi[0] || st.idx[1] < S.lo[1] ||
-          st.idx[1] >= S.hi[1] || st.idx[2] < S.lo[2] || st.idx[2] >= S.hi[2])
-        continue;
-      double p = 1.0;
-      if (S.profile) {
-        const long long bx = S.hi[0] - S.lo[0], by = S.hi[1] - S.lo[1];
-        p = __ldg(S.profile + (st.idx[0] - S.lo[0]) +
-                  bx * ((st.idx[1] - S.lo[1]) + by * (long long)(st.idx[2] - S.lo[2])));
-      }
-      J += a.st->src_amp[s] * p;
-    }
-  }
+    sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c - s1)) +
+                  (__ldg(a.sigma + c - s2) + __ldg(a.sigma + c - s1 - s2)));
+  const double curl = (h2 - h2m) * a.g.rd[d1] - (h1 - h1m) * a.g.rd[d2];
   const double edt = eps / a.g.dt, hs = 0.5 * sig;
-  const double e0 = a.E[D][c];
-  a.E[D][c] = (curl - (hs - edt) * e0 - J) / (hs + edt);  // eq. 11
+  const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
+  return wall ? 0.0 : e1;
+}
+
+// soft sources on the D-edge of cell (i,j,k)
+template <int D>
+__device__ __forceinline__ double source_term(const EArgs &a, int i, int j, int k) {
+  double J = 0.0;
+  for (int s = 0; s < a.src.count; ++s) {
+    const SourceP &S = a.src.s[s];
+    if (S.comp != D) continue;
+    if (i < S.lo[0] || i >= S.hi[0] || j < S.lo[1] || j >= S.hi[1] || k < S.lo[2] || k >= S.hi[2])
+      continue;
+    double p = 1.0;
+    if (S.profile) {
+      const long long bx = S.hi[0] - S.lo[0], by = S.hi[1] - S.lo[1];
+      p = __ldg(S.profile + (i - S.lo[0]) + bx * ((j - S.lo[1]) + by * (long long)(k - S.lo[2])));
+    }
+    J += a.st->src_amp[s] * p;
+  }
+  return J;
 }
 
 template <bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
 __global__ void __launch_bounds__(NTHREADS) k_e_update(const __grid_constant__ EArgs a) {
-  const int i = blockIdx.x * BX + threadIdx.x;
-  const int j = blockIdx.y * BY + threadIdx.y;
-  const int k = blockIdx.z * BZ + threadIdx.z;
-  if (i >= a.g.n[0] || j >= a.g.n[1] || k >= a.g.n[2]) return;
-  const Stencil st = make_stencil(a.g, i, j, k);
-  e_edge<0, EPS_ARR, SIG_ARR, HAS_SRC>(a, st);
-  e_edge<1, EPS_ARR, SIG_ARR, HAS_SRC>(a, st);
-  e_edge<2, EPS_ARR, SIG_ARR, HAS_SRC>(a, st);
+  for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
+    const Item w = decode_item(a.box, it);
+    const Column col = make_column(a.g, w.i, w.j);
+    int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
+    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
+    for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
+      c_tile += a.g.sz;
+      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
+      if (!w.active) continue;
+      double Jx = 0.0, Jy = 0.0, Jz = 0.0;
+      if (HAS_SRC) {
+        Jx = source_term<0>(a, w.i, w.j, k);
+        Jy = source_term<1>(a, w.i, w.j, k);
+        Jz = source_term<2>(a, w.i, w.j, k);
+      }
+      const bool wk = wall_k(a.g, k);
+      const double ex = e_edge<0, EPS_ARR, SIG_ARR>(a, c, col.wall[1] || wk, Jx);
+      const double ey = e_edge<1, EPS_ARR, SIG_ARR>(a, c, wk || col.wall[0], Jy);
+      const double ez = e_edge<2, EPS_ARR, SIG_ARR>(a, c, col.wall[0] || col.wall[1], Jz);
+      a.E[0][c] = ex;
+      a.E[1][c] = ey;
+      a.E[2][c] = ez;
+      if (col.edge_ij || edge_k(a.g, k)) {
+        store_images(a.E[0], a.g, w.i, w.j, k, c, ex);
+        store_images(a.E[1], a.g, w.i, w.j, k, c, ey);
+        store_images(a.E[2], a.g, w.i, w.j, k, c, ez);
+      }
+    }
+  }
 }
 
 // source time functions for this step: t = (n + 1/2) dt  (eq. 31)
@@ -429,6 +645,45 @@ __global__ void k_step_begin(DevState *st, const __grid_constant__ SourcesP src,
 
 // ------------------------------------------------------------------ set-up kernels
 
+__device__ __forceinline__ Cell make_cell(const GridP &g, int i, int j, int k) {
+  Cell q;
+  q.i = i; q.j = j; q.k = k;
+  q.c = g.org + i + g.sy * j + g.sz * k;
+  q.edge = false;
+  return q;
+}
+template <int D> __device__ __forceinline__ bool wall_face(const GridP &g, const Cell &q) {
+  return !g.per[D] && (D == 0 ? q.i : (D == 1 ? q.j : q.k)) == 0;
+}
+template <int D> __device__ __forceinline__ bool wall_edge(const GridP &g, const Cell &q) {
+  constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
+  const int v1 = t1 == 0 ? q.i : (t1 == 1 ? q.j : q.k), v2 = t2 == 0 ? q.i : (t2 == 1 ? q.j : q.k);
+  return (!g.per[t1] && v1 == 0) || (!g.per[t2] && v2 == 0);
+}
+
+// ghost layer of one array: periodic axes mirror the opposite interior plane, PEC ghosts are 0
+__global__ void k_fill_ghosts(double *__restrict__ a, const __grid_constant__ GridP g) {
+  const long long px = g.n[0] + 2, py = g.n[1] + 2, pz = g.n[2] + 2;
+  const long long total = px * py * pz;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const int idx[3] = {(int)(t % px) - 1, (int)((t / px) % py) - 1, (int)(t / (px * py)) - 1};
+    int src[3];
+    bool ghost = false, zero = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      src[d] = idx[d];
+      if (idx[d] < 0 || idx[d] >= g.n[d]) {
+        ghost = true;
+        if (g.per[d]) src[d] = idx[d] < 0 ? g.n[d] - 1 : 0; else zero = true;
+      }
+    }
+    if (!ghost) continue;
+    const int dst = g.org + idx[0] + g.sy * idx[1] + g.sz * idx[2];
+    a[dst] = zero ? 0.0 : a[g.org + src[0] + g.sy * src[1] + g.sz * src[2]];
+  }
+}
+
 struct FieldsP {
   GridP g;
   double *E[3];
@@ -436,22 +691,24 @@ struct FieldsP {
 };
 
 // zero tangential E and normal H on PEC walls
-__global__ void __launch_bounds__(NTHREADS) k_enforce_walls(const __grid_constant__ FieldsP a) {
-  const int i = blockIdx.x * BX + threadIdx.x;
-  const int j = blockIdx.y * BY + threadIdx.y;
-  const int k = blockIdx.z * BZ + threadIdx.z;
-  if (i >= a.g.n[0] || j >= a.g.n[1] || k >= a.g.n[2]) return;
-  const Stencil st = make_stencil(a.g, i, j, k);
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    if (wall_edge(a.g, st, d)) a.E[d][st.c] = 0.0;
-    if (wall_face(a.g, st, d)) a.H[d][st.c] = 0.0;
+__global__ void k_enforce_walls(const __grid_constant__ FieldsP a) {
+  const long long total = (long long)a.g.n[0] * a.g.n[1] * a.g.n[2];
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const Cell q = make_cell(a.g, (int)(t % a.g.n[0]), (int)((t / a.g.n[0]) % a.g.n[1]),
+                             (int)(t / ((long long)a.g.n[0] * a.g.n[1])));
+    if (wall_edge<0>(a.g, q)) a.E[0][q.c] = 0.0;
+    if (wall_edge<1>(a.g, q)) a.E[1][q.c] = 0.0;
+    if (wall_edge<2>(a.g, q)) a.E[2][q.c] = 0.0;
+    if (wall_face<0>(a.g, q)) a.H[0][q.c] = 0.0;
+    if (wall_face<1>(a.g, q)) a.H[1][q.c] = 0.0;
+    if (wall_face<2>(a.g, q)) a.H[2][q.c] = 0.0;
   }
 }
 
 struct InitMP {
   GridP g;
-  const double *Mc[3];  // cell-centred initial M (nullptr = 0)
+  const double *Mc[3];  // cell-centred initial M in the device layout, ghosts filled (nullptr = 0)
   double *M[9];         // face M out
   const double *Ms;     // array or nullptr
   double Ms_u;
@@ -460,39 +717,42 @@ struct InitMP {
 };
 
 // cell-centred M averaged to faces; renormalised to the face's Ms (A11)
-__global__ void __launch_bounds__(NTHREADS) k_init_m(const __grid_constant__ InitMP a) {
-  const int i = blockIdx.x * BX + threadIdx.x;
-  const int j = blockIdx.y * BY + threadIdx.y;
-  const int k = blockIdx.z * BZ + threadIdx.z;
-  if (i >= a.g.n[0] || j >= a.g.n[1] || k >= a.g.n[2]) return;
-  const Stencil st = make_stencil(a.g, i, j, k);
+__global__ void k_init_m(const __grid_constant__ InitMP a) {
+  const long long total = (long long)a.g.n[0] * a.g.n[1] * a.g.n[2];
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const Cell q = make_cell(a.g, (int)(t % a.g.n[0]), (int)((t / a.g.n[0]) % a.g.n[1]),
+                             (int)(t / ((long long)a.g.n[0] * a.g.n[1])));
+    const int st[3] = {1, a.g.sy, a.g.sz};
+    const bool wall[3] = {wall_face<0>(a.g, q), wall_face<1>(a.g, q), wall_face<2>(a.g, q)};
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    double m[3] = {0.0, 0.0, 0.0};
-    if (a.enable_llg && !wall_face(a.g, st, d)) {
-      const long long cm = st.c + st.m[d];
-      double Msf = a.Ms_u;
-      if (a.Ms) Msf = 0.5 * (a.Ms[st.c] + a.Ms[cm]);
-      if (Msf > 0.0) {
-        double v[3];
+    for (int d = 0; d < 3; ++d) {
+      double m[3] = {0.0, 0.0, 0.0};
+      if (a.enable_llg && !wall[d]) {
+        const int cm = q.c - st[d];
+        double Msf = a.Ms_u;
+        if (a.Ms) Msf = 0.5 * (a.Ms[q.c] + a.Ms[cm]);
+        if (Msf > 0.0) {
+          double v[3];
 #pragma unroll
-        for (int q = 0; q < 3; ++q) v[q] = a.Mc[q] ? 0.5 * (a.Mc[q][st.c] + a.Mc[q][cm]) : 0.0;
-        const double nrm = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-        if (nrm > 0.0) {
-          const double sc = Msf / nrm;
+          for (int p = 0; p < 3; ++p) v[p] = a.Mc[p] ? 0.5 * (a.Mc[p][q.c] + a.Mc[p][cm]) : 0.0;
+          const double nrm = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+          if (nrm > 0.0) {
+            const double sc = Msf / nrm;
 #pragma unroll
-          for (int q = 0; q < 3; ++q) m[q] = v[q] * sc;
-        } else {
-          a.st->init_error = 1;
+            for (int p = 0; p < 3; ++p) m[p] = v[p] * sc;
+          } else {
+            a.st->init_error = 1;
+          }
         }
       }
-    }
 #pragma unroll
-    for (int q = 0; q < 3; ++q) a.M[3 * d + q][st.c] = m[q];
+      for (int p = 0; p < 3; ++p) a.M[3 * d + p][q.c] = m[p];
+    }
   }
 }
 
-// min / max of an array: per-block partials, finished on the host
+// min / max of a COMPACT user array: per-block partials, finished on the host
 __global__ void k_minmax(const double *__restrict__ a, long long n, double *__restrict__ part) {
   double lo = INFINITY, hi = -INFINITY;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
@@ -520,17 +780,18 @@ __global__ void k_minmax(const double *__restrict__ a, long long n, double *__re
   }
 }
 
-// bounding box and count of the cells with Ms > 0: out = {lo x,y,z, hi x,y,z (inclusive)}, count
-__global__ void k_mag_box(const double *__restrict__ Ms, GridP g, int *box,
+// bounding box and count of the cells with Ms > 0 (Ms in the device layout):
+// box = {lo x,y,z, hi x,y,z (inclusive)}, count
+__global__ void k_mag_box(const double *__restrict__ Ms, const __grid_constant__ GridP g, int *box,
                           unsigned long long *count) {
   const long long n = (long long)g.n[0] * g.n[1] * g.n[2];
   int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {-1, -1, -1};
   unsigned long long cnt = 0;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
        t += (long long)gridDim.x * blockDim.x) {
-    if (Ms[t] > 0.0) {
-      const int i = (int)(t % g.n[0]), j = (int)((t / g.n[0]) % g.n[1]),
-                k = (int)(t / ((long long)g.n[0] * g.n[1]));
+    const int i = (int)(t % g.n[0]), j = (int)((t / g.n[0]) % g.n[1]),
+              k = (int)(t / ((long long)g.n[0] * g.n[1]));
+    if (Ms[g.org + i + g.sy * j + g.sz * k] > 0.0) {
       lo[0] = min(lo[0], i); lo[1] = min(lo[1], j); lo[2] = min(lo[2], k);
       hi[0] = max(hi[0], i); hi[1] = max(hi[1], j); hi[2] = max(hi[2], k);
       ++cnt;
