@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- coupled FDTD-LLG throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+
+One "step" = one full time step of the hot path (H/M half-step, E update, H/M half-step:
+PAPER.md:94, 152) over the whole synthetic grid.  Default workload: BASELINE.json configs[4],
+the 768^3 coupled grid named "throughput and HBM-roofline run" (the largest single-GPU
+configuration; configs[1] is Maxwell-only and configs[0] is the 32^3 parity case).
+
+Prints ONE JSON line: metric/value (Gcell-updates/s, inputs resident in HBM, CUDA-graph replay),
+e2e (same metric through the public API with HOST buffers: H2D of the initial fields, K steps,
+D2H of all 15 result arrays inside the timed region), roofline (dominant kernel, algorithmic
+bytes / CUDA-event duration against the measured HBM peak), cpu_baseline (the oracle as it
+stands, timed on this box's host cores on a bounded sample), clocks, gpu_launches.
+
+N > 1 (torchrun): the path is single-GPU by scope (replicas only); each
+rank advances its own replica of the grid, no data-path collective; value = all ranks' cell
+updates / max-over-ranks device time; "scaling": "weak".
+
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "coupled FDTD-LLG Gcell-updates/s (fp64)"
+UNIT = "Gcell-updates/s"
+
+# algorithmic 8-byte words per cell and launch: every array
+# read once and written once per sweep, stencil neighbours served on chip
+WORDS = {"h_update": 9,      # E 3 + H 3 read, H 3 written
+         "hm_first": 27,     # E 3 + H^n 3 + M^n 9 read, M^1 9 + H^1 3 written
+         "hm_iter": 39,      # + H^{r-1} 3 + M^{r-1} 9 read
+         "e_update": 9}      # E 3 + H 3 read, E 3 written
+
+
+def _parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5")
+    ap.add_argument("--shape", default=None, help="nx,ny,nz (default: the config's full size)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-shape", default="128,128,128")
+    ap.add_argument("--cpu-sample-steps", type=int, default=30)
+    return ap.parse_args()
+
+
+def _shape(args):
+    return tuple(int(v) for v in args.shape.split(",")) if args.shape else None
+
+
+def _workload_name(w):
+    return f"{w.name} {w.nx}x{w.ny}x{w.nz}"
+
+
+# ------------------------------------------------------------------ clocks
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU, sampled every 200 ms while running."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [c.strip() for c in line.split(",")]))
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
+    def summary(self, t0, t1):
+        rows = [r for t, r in self.rows if t0 <= t <= t1 and len(r) >= 7] or \
+               [r for _, r in self.rows[-3:] if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for q, n in enumerate(names) if any(r[3 + q].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons,
+                "samples": len(rows)}
+
+
+# ------------------------------------------------------------------ the oracle legs
+
+def _oracle_rate(cfg, shape, steps, warmup=0):
+    """Cell-updates/s of the CPU oracle (as it stands) on a reduced-shape copy of the workload."""
+    from oracle import Oracle  # noqa: F401  (the one place bench.py may execute oracle/)
+    from oracle.cpu_oracle import omp_threads
+    from paper_2103_12819_b200 import workloads as wl
+    from tests._util import oracle_from_workload
+    w = wl.make_config(cfg, shape=shape)
+    o = oracle_from_workload(w)
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return w, w.cells * steps / dt, dt, omp_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    shape = tuple(int(v) for v in args.cpu_sample_shape.split(","))
+    from paper_2103_12819_b200 import workloads as wl
+    full = wl.CONFIGS[args.config].__defaults__[0] if args.shape is None else _shape(args)
+    w, rate, dt, cores = _oracle_rate(args.config, shape, args.steps, args.warmup)
+    sample = (f"config {args.config} structure at {shape[0]}x{shape[1]}x{shape[2]} cells, "
+              f"{args.steps} steps after {args.warmup} warm-up (the full {full[0]}x{full[1]}x{full[2]} "
+              f"grid is out of the oracle's reach; the rate per cell is what is compared)")
+    val = rate * 1e-9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"cfg{args.config} {full[0]}x{full[1]}x{full[2]} (sampled)",
+                       "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ ours
+
+def _peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _ncu_traffic(kernel, workload):
+    """dram bytes per launch of `kernel` from the committed ncu capture, if it was taken on this
+    workload (profiles/traffic.csv: kernel,workload,dram_bytes_per_launch)."""
+    f = ROOT / "profiles" / "traffic.csv"
+    if not f.exists():
+        return None
+    for line in f.read_text().splitlines():
+        c = [x.strip() for x in line.split(",")]
+        if len(c) >= 3 and c[0] == kernel and c[1] == workload:
+            try:
+                return float(c[2])
+            except ValueError:
+                return None
+    return None
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2103_12819_b200 import workloads as wl
+    from paper_2103_12819_b200.binding import from_workload
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2103_12819_b200.replicas import barrier, max_over_ranks, whole_job_rate
+
+    K, W = args.steps, max(args.warmup, 0)
+    w = wl.make_config(args.config, shape=_shape(args), device=dev)
+    cells = w.cells
+    name = _workload_name(w)
+    sim = from_workload(w, device=dev)
+    stream = sim.stream
+
+    # host copies of the initial state for the end-to-end leg (pinned), before the device inputs go
+    host_in = None
+    if not args.no_e2e:
+        def pin(t):
+            return None if t is None else torch.empty(t.shape, dtype=t.dtype).pin_memory().copy_(t)
+        host_in = {"E": [pin(t) for t in w.E], "H": [pin(t) for t in w.H],
+                   "M_cell": [pin(t) for t in w.M_cell]}
+    del w
+    torch.cuda.empty_cache()
+
+    vis = [v for v in os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",") if v.strip()]
+    sampler = ClockSampler(vis[local] if local < len(vis) else local)
+    sampler.start()
+
+    # ---- device-resident throughput: CUDA-graph replay of K steps
+    sim.step(max(W, 1))
+    stream.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_a = time.perf_counter()
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    stream.synchronize()
+    torch.cuda.synchronize()
+    t_b = time.perf_counter()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), dev)
+    st = sim.stats()
+    value = whole_job_rate(cells, K, ms * 1e-3, world) * 1e-9
+    launches = K * st["launches_per_step"]
+
+    # ---- roofline of the dominant kernel: an event pair around every launch, K more steps
+    prof = sim.step_timed(K)
+    t_c = time.perf_counter()
+    peak, peak_src = _peak()
+    box = st["sweep_cells"]
+    from paper_2103_12819_b200.binding import MAT_BITS
+    mask = st["material_array_mask"]
+    extra = {"h_update": bool(mask & MAT_BITS["mu_r"]),
+             "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
+             "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
+    extra["hm_iter"] = extra["hm_first"]
+    per_class = {}
+    for cls, (cms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        ent = {"launches": cnt, "ms_total": cms, "us_per_launch": 1e3 * cms / cnt}
+        if cls in WORDS:
+            # cells one launch covers: the sweep box (LLG sweeps), the whole grid (E update), the
+            # complement of the box split over its slabs (H update, 2 half-steps per step)
+            if cls.startswith("hm_"):
+                ncell = box
+            elif cls == "e_update":
+                ncell = cells
+            else:
+                ncell = (cells - box) * 2 * K / cnt
+            ent["alg_bytes_per_launch"] = 8.0 * (WORDS[cls] + extra[cls]) * ncell
+            ent["alg_GBps"] = ent["alg_bytes_per_launch"] / (cms / cnt * 1e-3) * 1e-9
+        per_class[cls] = ent
+    timed = [c for c in per_class if "alg_GBps" in per_class[c]]
+    dom = max(timed, key=lambda c: per_class[c]["ms_total"])
+    dom_kernel = {"h_update": "k_h_update", "hm_first": "k_hm_sweep<FIRST>",
+                  "hm_iter": "k_hm_sweep<ITER>", "e_update": "k_e_update"}[dom]
+    achieved = per_class[dom]["alg_GBps"]
+    step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
+    roofline = {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": _ncu_traffic(dom_kernel, name),
+                "alg_bytes_per_launch": per_class[dom]["alg_bytes_per_launch"],
+                "us_per_launch": per_class[dom]["us_per_launch"],
+                "share_of_step": per_class[dom]["ms_total"] / sum(v["ms_total"] for v in per_class.values()),
+                "how": f"CUDA events around every launch over {K} steps (fdtd_llg_step_timed, plain launches)",
+                "whole_step": {"alg_bytes_per_step": step_bytes,
+                               "achieved": step_bytes / (ms / K * 1e-3) * 1e-9,
+                               "frac": step_bytes / (ms / K * 1e-3) * 1e-9 / peak},
+                "kernels": per_class}
+    clocks = sampler.summary(t_a, t_c)
+
+    # ---- end to end through the public API with HOST buffers
+    e2e = None
+    if host_in is not None:
+        from paper_2103_12819_b200.binding import FIELD_NAMES
+        out = {nm: torch.empty(sim.shape, dtype=torch.float64).pin_memory() for nm in FIELD_NAMES}
+        if not st["magnetic_cells"]:
+            out = {k: v for k, v in out.items() if not k.startswith("M")}
+        h2d = sum(t.numel() * 8 for g in host_in.values() for t in g if t is not None)
+        d2h = sum(t.numel() * 8 for t in out.values())
+        sim.set_fields(host_in["E"], host_in["H"], host_in["M_cell"])   # warm the path once
+        sim.step(1)
+        stream.synchronize()
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        sim.set_fields(host_in["E"], host_in["H"], host_in["M_cell"])   # H2D from pinned memory
+        sim.step(K)
+        sim.read_fields(out=out)                                         # D2H, synchronises
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0, dev)
+        barrier()
+        e2e = {"value": whole_job_rate(cells, K, dt, world) * 1e-9, "unit": UNIT,
+               "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+               "seconds": dt, "what": f"set_fields(host) + step({K}) + read_fields(host), wall clock"}
+        del out, host_in
+    sampler.stop()
+
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        shp = tuple(int(v) for v in args.cpu_sample_shape.split(","))
+        _, rate, dt, cores = _oracle_rate(args.config, shp, args.cpu_sample_steps)
+        cpu = {"value": rate * 1e-9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"config {args.config} structure at {shp[0]}x{shp[1]}x{shp[2]}, "
+                         f"{args.cpu_sample_steps} steps, {dt:.1f} s"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"],
+                           "llg_iterations_per_halfstep": st["iters_total"] / max(1, st["halfsteps"]),
+                           "parallelism": "replicas" if world > 1 else "single-gpu",
+                           "l2": "state far larger than L2 (no flush needed)" if cells * 48 > 4e8
+                                 else "state fits L2: latency-bound case, no roofline claim",
+                           "time_loop": "CUDA graph replay"},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+                "gpu_launches": launches,
+                "context": "paper: 59x node-by-node GPU speedup (8x V100 vs 32-core Haswell, "
+                           "PAPER.md:229, 277) -- another machine, context only"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = _parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

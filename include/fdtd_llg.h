@@ -86,7 +86,22 @@ typedef struct {
   long long kernel_launches;        /* kernels this handle has launched in fdtd_llg_step       */
   long long magnetic_cells;         /* cells with Ms > 0 (0 when LLG is disabled)              */
   int launches_per_step;            /* kernel nodes in one captured step                       */
+  long long sweep_cells;            /* cells of the LLG sweep box (bounding box of the magnetic
+                                       cells + 1 halo cell), what one k_hm_sweep launch covers  */
+  unsigned material_array_mask;     /* FDTD_LLG_MAT_* bits of the materials kept as device arrays
+                                       (a uniform map is folded into a scalar)                  */
 } fdtd_llg_stats;
+
+/* kernel classes of fdtd_llg_step_timed */
+enum {
+  FDTD_LLG_K_H_UPDATE = 0,   /* Maxwell H half-step outside the LLG sweep box (eq. 21, M = 0)   */
+  FDTD_LLG_K_HM_FIRST = 1,   /* LLG iterate r = 1 (eqs. 18-21)                                  */
+  FDTD_LLG_K_HM_ITER = 2,    /* LLG iterate r >= 2 that ran                                     */
+  FDTD_LLG_K_HM_SKIPPED = 3, /* LLG iterate launched after convergence (exits on the flag)      */
+  FDTD_LLG_K_E_UPDATE = 4,   /* eq. 11                                                          */
+  FDTD_LLG_K_OTHER = 5,      /* source amplitudes, half-step bookkeeping, canonical-buffer copy */
+  FDTD_LLG_K_NCLASS = 6
+};
 
 /* Fill *opt with the defaults: PEC x3, LLG on, no bias, no anisotropy (axis z), tol 1e-6
  * (PAPER.md:154), max 20 iterations, graph on. */
@@ -140,6 +155,13 @@ int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
 
 /* Advance n >= 0 time steps.  Asynchronous: only enqueues work on the stream (n graph launches). */
 int fdtd_llg_step(fdtd_llg *s, int n);
+
+/* Advance n time steps (1 <= n <= 2048) with plain launches (no graph) and a CUDA-event pair
+ * around every kernel launch; returns, per kernel class FDTD_LLG_K_*, the summed device time in
+ * milliseconds (ms_by_class[FDTD_LLG_K_NCLASS], HOST) and the number of launches
+ * (launches_by_class[FDTD_LLG_K_NCLASS], HOST).  Same arithmetic as fdtd_llg_step.  Synchronises
+ * the stream.  This is the measurement hook of bench.py's roofline block. */
+int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *launches_by_class);
 
 /* Copy the present fields out.  E[3], H[3], M[9] are HOST arrays of pointers (or NULL); each
  * non-NULL entry receives nx*ny*nz doubles in `mem_space`.  M order: x-face (Mx,My,Mz), y-face

@@ -38,15 +38,19 @@ class Stats(C.Structure):
                 ("nonconverged_halfsteps", C.c_longlong), ("resid_last", C.c_double),
                 ("halfsteps", C.c_longlong), ("courant", C.c_double),
                 ("kernel_launches", C.c_longlong), ("magnetic_cells", C.c_longlong),
-                ("launches_per_step", C.c_int)]
+                ("launches_per_step", C.c_int), ("sweep_cells", C.c_longlong),
+                ("material_array_mask", C.c_uint)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
 EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_create",
-           "fdtd_llg_set_fields", "fdtd_llg_set_source", "fdtd_llg_step", "fdtd_llg_read_fields",
+           "fdtd_llg_set_fields", "fdtd_llg_set_source", "fdtd_llg_step", "fdtd_llg_step_timed",
+           "fdtd_llg_read_fields",
            "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy")
+
+KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other")
 
 _VP = C.c_void_p
 _PP = C.POINTER(C.c_void_p)
@@ -82,6 +86,9 @@ def lib() -> C.CDLL:
         L.fdtd_llg_set_source.restype = C.c_int
         L.fdtd_llg_step.argtypes = [_VP, C.c_int]
         L.fdtd_llg_step.restype = C.c_int
+        L.fdtd_llg_step_timed.argtypes = [_VP, C.c_int, C.POINTER(C.c_double),
+                                          C.POINTER(C.c_longlong)]
+        L.fdtd_llg_step_timed.restype = C.c_int
         L.fdtd_llg_read_fields.argtypes = [_VP, _PP, _PP, _PP, C.c_int]
         L.fdtd_llg_read_fields.restype = C.c_int
         L.fdtd_llg_get_stats.argtypes = [_VP, C.POINTER(Stats)]
@@ -245,6 +252,15 @@ class FdtdLlg:
         with self._torch.cuda.device(self.device):
             rc = lib().fdtd_llg_step(self._h, int(n))
         _check(rc, self._h)
+
+    def step_timed(self, n=1) -> dict:
+        """n steps with an event pair around every launch: {class: (ms, launches)}."""
+        ms = (C.c_double * len(KERNEL_CLASSES))()
+        cnt = (C.c_longlong * len(KERNEL_CLASSES))()
+        with self._torch.cuda.device(self.device):
+            rc = lib().fdtd_llg_step_timed(self._h, int(n), ms, cnt)
+        _check(rc, self._h)
+        return {k: (ms[q], cnt[q]) for q, k in enumerate(KERNEL_CLASSES)}
 
     def read_fields(self, names=None, device=None, out=None) -> dict:
         """Fields as torch tensors shaped (nz, ny, nx).  ``device=None``: pinned host memory."""

@@ -69,6 +69,12 @@ struct fdtd_llg {
   double *profile_pool = nullptr;
   size_t profile_cap = 0, profile_used = 0;
 
+  // per-kernel timing of fdtd_llg_step_timed: an event pair around every launch
+  struct ProfRec { cudaEvent_t a, b; int cls, half, r; };
+  std::vector<ProfRec> *prof = nullptr;
+  int prof_half = 0;
+  int *r_hist = nullptr;  // device: iteration count R of half-step h at [h % R_HIST]
+
   cudaGraphExec_t graph = nullptr;
   bool graph_valid = false;
   int launches_per_step = 0;
@@ -78,6 +84,23 @@ struct fdtd_llg {
 };
 
 namespace {
+
+constexpr int R_HIST = 4096;
+
+// event pair around the launches between prof_begin and prof_end (no-ops outside step_timed)
+void prof_begin(fdtd_llg *s, int cls, int r) {
+  if (!s->prof) return;
+  fdtd_llg::ProfRec p{};
+  p.cls = cls; p.half = s->prof_half; p.r = r;
+  cudaEventCreate(&p.a);
+  cudaEventCreate(&p.b);
+  cudaEventRecord(p.a, s->stream);
+  s->prof->push_back(p);
+}
+void prof_end(fdtd_llg *s) {
+  if (!s->prof) return;
+  cudaEventRecord(s->prof->back().b, s->stream);
+}
 
 int fail(fdtd_llg *s, int code, const char *fmt, ...) {
   char buf[512];
@@ -176,6 +199,7 @@ size_t small_bytes(const fdtd_llg_options *o) {
   b += padded((size_t)(o->llg_max_iter + 2)) * 8 + 4096;      // residual words
   b += (2 * 1024 + 64) * 8;                                   // reduction scratch
   b += (size_t)1 << 20;                                       // source profiles pool (1 MiB)
+  b += (size_t)R_HIST * sizeof(int);                          // iteration counts per half-step
   return (b + 255) / 256 * 256;
 }
 
@@ -354,8 +378,10 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     h.box = s->box_out[b];
     if (h.box.items == 0) continue;
     const int grid = grid_for(s, h.box, 0);
+    prof_begin(s, FDTD_LLG_K_H_UPDATE, 0);
     if (s->mu_r.is_array) k_h_update<true><<<grid, blk, 0, s->stream>>>(h);
     else k_h_update<false><<<grid, blk, 0, s->stream>>>(h);
+    prof_end(s);
     ++*launches;
   }
   if (s->llg) {
@@ -389,13 +415,16 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
         for (int q = 0; q < 9; ++q) a.pf[a.npf++] = a.Mr[q];
       }
       if (a.Ms) a.pf[a.npf++] = a.Ms;
+      prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
       int rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
+      prof_end(s);
       if (rc) return rc;
       ++*launches;
     }
   }
-  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->opt.llg_max_iter, s->opt.llg_tol,
-                                     s->llg ? 1 : 0, last ? 1 : 0);
+  prof_begin(s, FDTD_LLG_K_OTHER, 0);
+  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->r_hist, s->opt.llg_max_iter,
+                                     s->opt.llg_tol, s->llg ? 1 : 0, last ? 1 : 0);
   ++*launches;
   if (s->llg && s->opt.llg_max_iter >= 2) {
     CanonArgs c{};
@@ -406,6 +435,8 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     k_canon<<<grid_for(s, c.box, 8), blk, 0, s->stream>>>(c);
     ++*launches;
   }
+  prof_end(s);
+  if (s->prof) s->prof_half++;
   CU(s, cudaGetLastError());
   return FDTD_LLG_OK;
 }
@@ -428,9 +459,11 @@ int enqueue_e(fdtd_llg *s, int hset, int *launches) {
   const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = s->src.count > 0;
 #define EK(EA, SA, HS)                                                        \
   if (ea == EA && sa == SA && hs == HS) k_e_update<EA, SA, HS><<<grid, blk, 0, s->stream>>>(a);
+  prof_begin(s, FDTD_LLG_K_E_UPDATE, 0);
   EK(false, false, false) EK(false, false, true) EK(false, true, false) EK(false, true, true)
   EK(true, false, false) EK(true, false, true) EK(true, true, false) EK(true, true, true)
 #undef EK
+  prof_end(s);
   ++*launches;
   CU(s, cudaGetLastError());
   return FDTD_LLG_OK;
@@ -441,7 +474,9 @@ int enqueue_e(fdtd_llg *s, int hset, int *launches) {
 int enqueue_step(fdtd_llg *s, int *launches) {
   *launches = 0;
   if (s->src.count > 0) {
+    prof_begin(s, FDTD_LLG_K_OTHER, 0);
     k_step_begin<<<1, 32, 0, s->stream>>>(s->dstate, s->src, s->dt);
+    prof_end(s);
     ++*launches;
   }
   int rc = enqueue_half(s, 0, 1, 2, 0, 1, false, launches);
@@ -571,6 +606,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->resid = reinterpret_cast<unsigned long long *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 4096;
   s->scratch = reinterpret_cast<double *>(p); p += (2 * 1024 + 64) * 8;
   s->profile_pool = reinterpret_cast<double *>(p); s->profile_cap = ((size_t)1 << 20) / 8; p += (size_t)1 << 20;
+  s->r_hist = reinterpret_cast<int *>(p); p += (size_t)R_HIST * sizeof(int);
   p = s->ws + small_bytes(&s->opt);
   double *q = reinterpret_cast<double *>(p);
   for (int d = 0; d < 3; ++d) { s->E[d] = q; q += s->stride; }
@@ -727,6 +763,46 @@ int fdtd_llg_step(fdtd_llg *s, int n) {
   return FDTD_LLG_OK;
 }
 
+int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *launches_by_class) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (n < 1 || n > R_HIST / 2) return fail(s, FDTD_LLG_EINVAL, "n must be in 1..%d", R_HIST / 2);
+  if (!ms_by_class || !launches_by_class) return fail(s, FDTD_LLG_EINVAL, "output array is NULL");
+  std::vector<fdtd_llg::ProfRec> recs;
+  DevState h0{};
+  CU(s, cudaMemcpyAsync(&h0, s->dstate, sizeof h0, cudaMemcpyDeviceToHost, s->stream));
+  CU(s, cudaStreamSynchronize(s->stream));
+  s->prof = &recs;
+  s->prof_half = 0;
+  int rc = FDTD_LLG_OK;
+  for (int t = 0; t < n && !rc; ++t) {
+    int launches = 0;
+    rc = enqueue_step(s, &launches);
+    s->launches_per_step = launches;
+  }
+  s->prof = nullptr;
+  cudaError_t e = cudaStreamSynchronize(s->stream);
+  std::vector<int> hist(R_HIST);
+  if (e == cudaSuccess)
+    e = cudaMemcpy(hist.data(), s->r_hist, sizeof(int) * R_HIST, cudaMemcpyDeviceToHost);
+  for (int c = 0; c < FDTD_LLG_K_NCLASS; ++c) { ms_by_class[c] = 0.0; launches_by_class[c] = 0; }
+  for (auto &p : recs) {
+    float ms = 0.f;
+    if (e == cudaSuccess && !rc) cudaEventElapsedTime(&ms, p.a, p.b);
+    int cls = p.cls;
+    // an LLG iterate beyond the half-step's iteration count exited on its first flag read
+    if (cls == FDTD_LLG_K_HM_ITER && p.r > hist[(h0.halfsteps + p.half) % R_HIST]) cls = FDTD_LLG_K_HM_SKIPPED;
+    ms_by_class[cls] += ms;
+    launches_by_class[cls]++;
+    cudaEventDestroy(p.a);
+    cudaEventDestroy(p.b);
+  }
+  if (rc) return rc;
+  if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "step_timed: %s", cudaGetErrorString(e));
+  s->host_steps += n;
+  s->kernel_launches += (long long)n * s->launches_per_step;
+  return FDTD_LLG_OK;
+}
+
 int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double *const *M,
                          int mem_space) {
   if (!s) return FDTD_LLG_EINVAL;
@@ -768,6 +844,14 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   out->kernel_launches = s->kernel_launches;
   out->magnetic_cells = s->magnetic_cells;
   out->launches_per_step = s->launches_per_step;
+  out->material_array_mask = (s->eps_r.is_array ? 1u : 0) | (s->sigma.is_array ? 2u : 0) |
+                             (s->mu_r.is_array ? 4u : 0) | (s->Ms.is_array ? 8u : 0) |
+                             (s->alpha.is_array ? 16u : 0) | (s->gamma.is_array ? 32u : 0);
+  out->sweep_cells = 0;
+  if (s->llg) {
+    out->sweep_cells = 1;
+    for (int d = 0; d < 3; ++d) out->sweep_cells *= (long long)(s->hi[d] - s->lo[d]);
+  }
   return FDTD_LLG_OK;
 }
 

@@ -187,9 +187,10 @@ __device__ __forceinline__ void prefetch_plane(const double *const *ptrs, int n,
   for (int q = t; q < n * TY; q += NTHREADS) {
     const int arr = q / TY, row = q % TY;
     if (row < rows) {
-      const unsigned long long addr =
-          (unsigned long long)(ptrs[arr] + c_row0 + row * sy) & ~15ull;
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(addr), "r"((width * 8 + 23) & ~15)
+      const unsigned long long raw = (unsigned long long)(ptrs[arr] + c_row0 + row * sy);
+      const unsigned long long addr = raw & ~15ull;
+      const unsigned bytes = (unsigned)((raw - addr) + width * 8 + 15) & ~15u;
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(addr), "r"(bytes)
                    : "memory");
     }
   }
@@ -494,8 +495,8 @@ __global__ void __launch_bounds__(NTHREADS) k_hm_sweep(const __grid_constant__ H
 }
 
 // 1 thread: close an (H,M) half-step
-__global__ void k_half_end(DevState *st, unsigned long long *resid, int max_iter, double tol,
-                           int any_magnetic, int last_of_step) {
+__global__ void k_half_end(DevState *st, unsigned long long *resid, int *r_hist, int max_iter,
+                           double tol, int any_magnetic, int last_of_step) {
   if (any_magnetic) {
     int R = max_iter;
     for (int r = 1; r <= max_iter; ++r)
@@ -512,6 +513,7 @@ __global__ void k_half_end(DevState *st, unsigned long long *resid, int max_iter
     st->iters_last = 0;
     st->last_R_even = 0;
   }
+  r_hist[st->halfsteps % 4096] = st->iters_last;
   st->halfsteps++;
   if (last_of_step) st->steps++;
 }
