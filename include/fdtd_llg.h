@@ -71,6 +71,8 @@ typedef struct {
   int use_graph;      /* 1 (default): the step is captured once in a CUDA Graph and replayed      */
   unsigned scalar_material_mask; /* FDTD_LLG_MAT_* bits: that material pointer addresses ONE double
                          in HOST memory, the uniform value (no nx*ny*nz array needed)            */
+  int kernel_path;    /* 0 (default): TMA-fed shared-memory pipelines wherever they apply;
+                         1: the direct-load kernels everywhere (same arithmetic; A/B checks)     */
 } fdtd_llg_options;
 
 typedef struct {

@@ -15,6 +15,7 @@
 
 #include "../../include/fdtd_llg.h"
 #include "kernels.cuh"
+#include "hm_tma.cuh"
 
 using namespace fl;
 
@@ -35,6 +36,7 @@ size_t array_stride(int nx, int ny, int nz) {
 struct MatInfo {
   bool is_array = false;  // non-uniform: kept on the device
   double uniform = 0.0;   // value when uniform
+  double maxv = 0.0;      // largest value of the map
   double *dev = nullptr;
 };
 
@@ -59,6 +61,11 @@ struct fdtd_llg {
   long long magnetic_cells = 0;
   int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
   BoxP box_llg{}, box_all{};
+  // TMA-fed sweeps (hm_tma.cuh): used when alpha, gamma, mu_r are uniform and opt.kernel_path == 0
+  bool tma_hm = false;
+  TileBox tile_llg{};
+  CUtensorMap mapH{}, mapE{}, mapS{}, mapM{};
+  int n_arrays = 0;  // arrays in the workspace tensor (4th TMA coordinate)
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
 
@@ -258,6 +265,7 @@ int take_material(fdtd_llg *s, MatInfo *m, const double *user, int mem_space, do
   if (strict_min ? !(lo > min_allowed) : !(lo >= min_allowed))
     return fail(s, FDTD_LLG_EINVAL, "%s must be %s %g everywhere (min is %g)", name,
                 strict_min ? ">" : ">=", min_allowed, lo);
+  m->maxv = hi;
   if (lo == hi) {
     m->uniform = lo;
     return FDTD_LLG_OK;
@@ -307,6 +315,7 @@ int find_sweep_box(fdtd_llg *s) {
     if (s->g.per[d] && (l < 0 || h > n)) { l = 0; h = n; }
     s->lo[d] = l < 0 ? 0 : l;
     s->hi[d] = h > n ? n : h;
+    if (d == 0) s->lo[d] &= ~1;  // even start in x: TMA box rows begin on 16-byte boundaries
   }
   s->llg = true;
   return FDTD_LLG_OK;
@@ -337,6 +346,95 @@ void make_boxes(fdtd_llg *s) {
     lo[d] = s->lo[d];
     hi[d] = s->hi[d];
   }
+}
+
+
+// ---- TMA-fed sweeps -----------------------------------------------------------------------
+
+constexpr int HM_BY = 8;  // tile rows of k_hm_tma
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+// tensor map over ALL arrays of the workspace: (x = row pitch, y = ny+2, z = nz+2, a = array),
+// box = (bx, by, 1, ba) elements
+int make_map(fdtd_llg *s, CUtensorMap *m, int bx, int by, int ba) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return fail(s, FDTD_LLG_ECUDA, "cuTensorMapEncodeTiled is not available");
+  const cuuint64_t dims[4] = {(cuuint64_t)s->g.sy, (cuuint64_t)s->g.n[1] + 2, (cuuint64_t)s->g.n[2] + 2,
+                              (cuuint64_t)s->n_arrays};
+  const cuuint64_t strides[3] = {(cuuint64_t)s->g.sy * 8, (cuuint64_t)s->g.sz * 8, (cuuint64_t)s->stride * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1u, (cuuint32_t)ba};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, s->E[0], dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(s, FDTD_LLG_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return FDTD_LLG_OK;
+}
+
+int array_index(const fdtd_llg *s, const double *p) { return (int)((p - s->E[0]) / (ptrdiff_t)s->stride); }
+
+// TW x by columns marched over kz planes; kz as long as possible while leaving >= 16 items per SM
+TileBox make_tilebox(const fdtd_llg *s, const int lo[3], const int hi[3], int by) {
+  TileBox b{};
+  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
+  b.ntx = (hi[0] - lo[0] + TW - 1) / TW;
+  b.nty = (hi[1] - lo[1] + by - 1) / by;
+  const int ez = std::max(1, hi[2] - lo[2]);
+  int kz = ez;
+  while (kz > 16 && (long long)b.ntx * b.nty * ((ez + kz - 1) / kz) < 16LL * s->num_sms) kz = (kz + 1) / 2;
+  b.kz = kz;
+  b.items = b.ntx * b.nty * ((ez + kz - 1) / kz);
+  return b;
+}
+
+template <bool FIRST>
+int launch_hm_tma(fdtd_llg *s, const HMTArgs &p) {
+  const bool ms = s->Ms.is_array, an = s->opt.ani_hk != 0.0;
+  const int grid = std::max(1, std::min(p.tb.items, s->num_sms));
+#define TK(MS, AN)                                                                          \
+  if (ms == MS && an == AN) {                                                               \
+    using L = HmLayout<HM_BY, FIRST, MS>;                                                   \
+    k_hm_tma<HM_BY, FIRST, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);     \
+    return FDTD_LLG_OK;                                                                     \
+  }
+  TK(false, false) TK(false, true) TK(true, false) TK(true, true)
+#undef TK
+  return FDTD_LLG_OK;
+}
+
+// opt in to > 48 KB of dynamic shared memory for every instantiation
+int setup_hm_tma(fdtd_llg *s) {
+#define TA(FIRST, MS, AN)                                                                   \
+  CU(s, cudaFuncSetAttribute(k_hm_tma<HM_BY, FIRST, MS, AN>,                                \
+                             cudaFuncAttributeMaxDynamicSharedMemorySize,                   \
+                             (int)HmLayout<HM_BY, FIRST, MS>::SMEM_BYTES));
+  TA(true, false, false) TA(true, false, true) TA(true, true, false) TA(true, true, true)
+  TA(false, false, false) TA(false, false, true) TA(false, true, false) TA(false, true, true)
+#undef TA
+  int rc;
+  if ((rc = make_map(s, &s->mapH, HW, HM_BY + 2, 3))) return rc;
+  if ((rc = make_map(s, &s->mapE, EW, HM_BY + 1, 3))) return rc;
+  if ((rc = make_map(s, &s->mapS, HW, HM_BY + 1, 1))) return rc;
+  if ((rc = make_map(s, &s->mapM, TW, HM_BY, 9))) return rc;
+  s->tile_llg = make_tilebox(s, s->lo, s->hi, HM_BY);
+  return FDTD_LLG_OK;
 }
 
 // ---- launching one step ----------------------------------------------------------------
@@ -393,11 +491,16 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
     a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
+    if (s->tma_hm && s->Ms.is_array) {  // k_hm_tma: the most common face value and its reciprocal
+      a.Ms_u = s->Ms.maxv;
+      a.rMs_u = 1.0 / s->Ms.maxv;
+    }
     a.ch_uniform = h.ch_uniform;
     for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
     a.hk = s->opt.ani_hk;
     a.tol = s->opt.llg_tol;
     a.resid = s->resid;
+    a.pipe_error = &s->dstate->pipe_error;
     for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
       // r <= 3 normally run: one block per item.  Later iterates almost never run: a small
       // persistent grid keeps their early exit at launch-latency cost.
@@ -416,7 +519,19 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
       }
       if (a.Ms) a.pf[a.npf++] = a.Ms;
       prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
-      int rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
+      int rc;
+      if (s->tma_hm) {
+        HMTArgs p{};
+        p.a = a;
+        p.tb = s->tile_llg;
+        p.mapH = s->mapH; p.mapE = s->mapE; p.mapS = s->mapS; p.mapM = s->mapM;
+        p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
+        p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
+        p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
+        rc = (r == 1) ? launch_hm_tma<true>(s, p) : launch_hm_tma<false>(s, p);
+      } else {
+        rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
+      }
       prof_end(s);
       if (rc) return rc;
       ++*launches;
@@ -633,6 +748,10 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   }
   if ((rc = find_sweep_box(s))) return bail(rc);
   make_boxes(s);
+  s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
+  s->tma_hm = s->llg && opt->kernel_path == 0 && !s->alpha.is_array && !s->gamma.is_array &&
+              !s->mu_r.is_array;
+  if (s->tma_hm && (rc = setup_hm_tma(s))) return bail(rc);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
   *out = s;
@@ -830,6 +949,8 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   DevState h{};
   CU(s, cudaMemcpyAsync(&h, s->dstate, sizeof h, cudaMemcpyDeviceToHost, s->stream));
   CU(s, cudaStreamSynchronize(s->stream));
+  if (h.pipe_error)
+    return fail(s, FDTD_LLG_ESTATE, "a TMA pipeline wait timed out (wait tag %d): results are invalid", h.pipe_error);
   std::memset(out, 0, sizeof *out);
   out->steps = h.steps;
   out->time = (double)h.steps * s->dt;

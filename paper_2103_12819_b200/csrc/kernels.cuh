@@ -69,6 +69,7 @@ struct DevState {
   int iters_max;
   int last_R_even;  // 1 when the last half-step ended on an even iterate (result in the pong set)
   int init_error;   // set by k_init_m when a magnetic face got a zero averaged M
+  int pipe_error;   // set by a TMA-fed kernel whose mbarrier wait timed out (tag of the wait)
   double resid_last;
   double src_amp[MAX_SOURCES];
 };
@@ -266,6 +267,7 @@ struct HMArgs {
   double hb[3], hk, u[3];
   double tol;
   unsigned long long *resid;  // [max_iter + 1] bit patterns of the residual of iterate r
+  int *pipe_error;            // &DevState::pipe_error
   int r;
   const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
   int npf;
@@ -349,42 +351,22 @@ struct FaceOut {
   double res;
 };
 
-// One Jacobi iterate on the D-face of the cell at offset c, BRANCH-FREE: every load is a
-// constant offset from c (always in bounds thanks to the ghost layer) and is issued
-// unconditionally, so the compiler batches all of a face's loads ahead of the arithmetic; the
-// magnetic / non-magnetic / wall decision is a select at the end.  (A non-magnetic face runs the
-// LLG arithmetic on rMs = 0 and discards it.)  The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f
-// (0 on non-magnetic faces).  Ms_c / rMs_c: this cell's Ms and its reciprocal, shared by the
-// three faces wherever Ms is locally uniform.
-template <int D, bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
-__device__ __forceinline__ FaceOut hm_face(const HMArgs &a, int c, bool wall, double Ms_c,
-                                           double rMs_c) {
-  const int cm = c - stride_of<D>(a.g);
-  // ---- loads
-  double Ms_m = Ms_c;
-  if (MS_ARR) Ms_m = __ldg(a.Ms + cm);
-  const Vec3 mn = {__ldcs(a.Mn[3 * D + 0] + c), __ldcs(a.Mn[3 * D + 1] + c),
-                   __ldcs(a.Mn[3 * D + 2] + c)};
-  Vec3 mp = mn;
-  if (!FIRST)
-    mp = {__ldcs(a.Mr[3 * D + 0] + c), __ldcs(a.Mr[3 * D + 1] + c), __ldcs(a.Mr[3 * D + 2] + c)};
-  Vec3 hn = h_em<D>(a.g, c, a.Hn);
-  Vec3 he = hn;
-  if (!FIRST) he = h_em<D>(a.g, c, a.Hp);
-  const double C = curl_e<D>(a.g, c, a.E);
-  double alf = a.alpha_u, gam = a.gamma_u, ch = a.ch_uniform;
-  if (AG_ARR) {
-    alf = 0.5 * (__ldg(a.alpha + c) + __ldg(a.alpha + cm));
-    gam = 0.5 * (fabs(__ldg(a.gamma + c)) + fabs(__ldg(a.gamma + cm)));  // |gamma| (eqs. 19-20)
-  }
-  if (MU_ARR) ch = a.g.dt / (2.0 * kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + cm))));
+// Arithmetic of one Jacobi iterate on a D-face, shared by every sweep kernel (whatever way its
+// operands were fetched), BRANCH-FREE: the magnetic / non-magnetic / wall decision is a select at
+// the end.  (A non-magnetic face runs the LLG arithmetic on rMs = 0 and discards it.)
+//   mn = M^n, mp = M^{r-1}, hn / he = H_EM^n / H_EM^{r-1} (own normal component + the two
+//   four-point averages), C = (curl E)_D, Msf / rMs = face Ms and its reciprocal (0 if Msf = 0),
+//   alf, gam = face alpha, |gamma|, ch = dt / (2 mu) of a non-magnetic face.
+// The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces).
+template <int D, bool FIRST, bool ANISO>
+__device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn, const Vec3 &mp_in,
+                                                Vec3 hn, Vec3 he, double C, double Msf, double rMs,
+                                                double alf, double gam, double ch, bool wall) {
+  const Vec3 mp = FIRST ? mn : mp_in;
   const double hn_own = comp<D>(hn), hp_own = comp<D>(he);
 
   // ---- magnetic face: eqs. 18-21
-  const double Msf = 0.5 * (Ms_c + Ms_m);
   const bool magnetic = !wall && Msf > 0.0;
-  double rMs = rMs_c;
-  if (MS_ARR && Ms_m != Ms_c) rMs = Msf > 0.0 ? 1.0 / Msf : 0.0;
   const double cf = kMu0 * gam * a.g.dt * 0.25;  // mu0 |gamma| dt / 4
   const Vec3 hb = {a.hb[0], a.hb[1], a.hb[2]};
   const Vec3 u = {a.u[0], a.u[1], a.u[2]};
@@ -419,6 +401,38 @@ __device__ __forceinline__ FaceOut hm_face(const HMArgs &a, int c, bool wall, do
   o.h = magnetic ? h_mag : h_non;
   o.res = magnetic ? e * rMs : 0.0;
   return o;
+}
+
+// One Jacobi iterate on the D-face of the cell at offset c, operands straight from global memory:
+// every load is a constant offset from c (always in bounds thanks to the ghost layer) and is
+// issued unconditionally, so the compiler batches all of a face's loads ahead of the arithmetic.
+// Ms_c / rMs_c: this cell's Ms and its reciprocal, shared by the three faces wherever Ms is
+// locally uniform.
+template <int D, bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
+__device__ __forceinline__ FaceOut hm_face(const HMArgs &a, int c, bool wall, double Ms_c,
+                                           double rMs_c) {
+  const int cm = c - stride_of<D>(a.g);
+  double Ms_m = Ms_c;
+  if (MS_ARR) Ms_m = __ldg(a.Ms + cm);
+  const Vec3 mn = {__ldcs(a.Mn[3 * D + 0] + c), __ldcs(a.Mn[3 * D + 1] + c),
+                   __ldcs(a.Mn[3 * D + 2] + c)};
+  Vec3 mp = mn;
+  if (!FIRST)
+    mp = {__ldcs(a.Mr[3 * D + 0] + c), __ldcs(a.Mr[3 * D + 1] + c), __ldcs(a.Mr[3 * D + 2] + c)};
+  const Vec3 hn = h_em<D>(a.g, c, a.Hn);
+  Vec3 he = hn;
+  if (!FIRST) he = h_em<D>(a.g, c, a.Hp);
+  const double C = curl_e<D>(a.g, c, a.E);
+  double alf = a.alpha_u, gam = a.gamma_u, ch = a.ch_uniform;
+  if (AG_ARR) {
+    alf = 0.5 * (__ldg(a.alpha + c) + __ldg(a.alpha + cm));
+    gam = 0.5 * (fabs(__ldg(a.gamma + c)) + fabs(__ldg(a.gamma + cm)));  // |gamma| (eqs. 19-20)
+  }
+  if (MU_ARR) ch = a.g.dt / (2.0 * kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + cm))));
+  const double Msf = 0.5 * (Ms_c + Ms_m);
+  double rMs = rMs_c;
+  if (MS_ARR && Ms_m != Ms_c) rMs = Msf > 0.0 ? 1.0 / Msf : 0.0;
+  return hm_face_core<D, FIRST, ANISO>(a, mn, mp, hn, he, C, Msf, rMs, alf, gam, ch, wall);
 }
 
 template <int D>
