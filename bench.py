@@ -58,6 +58,8 @@ def _parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-shape", default="128,128,128")
     ap.add_argument("--cpu-sample-steps", type=int, default=30)
+    ap.add_argument("--kernel-path", type=int, default=0,
+                    help="fdtd_llg_options.kernel_path: 0 = default kernels, 1 = direct-load kernels (A/B)")
     return ap.parse_args()
 
 
@@ -203,7 +205,7 @@ def run_ours(args):
     w = wl.make_config(args.config, shape=_shape(args), device=dev)
     cells = w.cells
     name = _workload_name(w)
-    sim = from_workload(w, device=dev)
+    sim = from_workload(w, device=dev, kernel_path=args.kernel_path)
     stream = sim.stream
 
     # host copies of the initial state for the end-to-end leg (pinned), before the device inputs go
@@ -331,7 +333,7 @@ def run_ours(args):
                            "parallelism": "replicas" if world > 1 else "single-gpu",
                            "l2": "state far larger than L2 (no flush needed)" if cells * 48 > 4e8
                                  else "state fits L2: latency-bound case, no roofline claim",
-                           "time_loop": "CUDA graph replay"},
+                           "time_loop": "CUDA graph replay", "kernel_path": args.kernel_path},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
                 "gpu_launches": launches,
                 "context": "paper: 59x node-by-node GPU speedup (8x V100 vs 32-core Haswell, "
