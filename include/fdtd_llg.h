@@ -71,8 +71,11 @@ typedef struct {
   int use_graph;      /* 1 (default): the step is captured once in a CUDA Graph and replayed      */
   unsigned scalar_material_mask; /* FDTD_LLG_MAT_* bits: that material pointer addresses ONE double
                          in HOST memory, the uniform value (no nx*ny*nz array needed)            */
-  int kernel_path;    /* 0 (default): TMA-fed shared-memory pipelines wherever they apply;
-                         1: the direct-load kernels everywhere (same arithmetic; A/B checks)     */
+  int kernel_path;    /* which LLG sweep kernel runs (same arithmetic in all: bitwise-equal results).
+                         0 (default): staged sweep, tile 32x16 (TMA-fed shared-memory ring for the
+                         neighbour operands) wherever it applies (alpha, gamma, mu_r uniform);
+                         1: direct-load kernels everywhere; 2: the all-TMA sweep, warp = (face,
+                         row); 3: staged sweep, tile 32x7, two blocks per SM.  1-3: A/B checks    */
 } fdtd_llg_options;
 
 typedef struct {

@@ -16,6 +16,7 @@
 #include "../../include/fdtd_llg.h"
 #include "kernels.cuh"
 #include "hm_tma.cuh"
+#include "hm_stage.cuh"
 
 using namespace fl;
 
@@ -66,11 +67,17 @@ struct fdtd_llg {
   TileBox tile_llg{};
   CUtensorMap mapH{}, mapE{}, mapS{}, mapM{};
   int n_arrays = 0;  // arrays in the workspace tensor (4th TMA coordinate)
+  // staged sweeps (hm_stage.cuh): kernel_path 0 (tile rows 16) and 3 (tile rows 7)
+  int stage_by = 0;  // 0 = not used
+  StBox st_box{};
+  CUtensorMap mapT{}, mapPM{};
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
 
   DevState *dstate = nullptr;
   unsigned long long *resid = nullptr;
+  unsigned *work = nullptr;  // [max_iter + 1] item counters of the staged sweeps
+  int tune = 3, m_ahead = 0;
   double *scratch = nullptr;  // 2*1024 doubles for reductions + 8 ints
   SourcesP src{};
   double *profile_pool = nullptr;
@@ -203,7 +210,7 @@ bool valid_opts(const fdtd_llg_options *o, const char **why) {
 size_t small_bytes(const fdtd_llg_options *o) {
   size_t b = 0;
   b += 4096;                                                  // DevState
-  b += padded((size_t)(o->llg_max_iter + 2)) * 8 + 4096;      // residual words
+  b += 2 * padded((size_t)(o->llg_max_iter + 2)) * 8 + 4096;  // residual words, item counters
   b += (2 * 1024 + 64) * 8;                                   // reduction scratch
   b += (size_t)1 << 20;                                       // source profiles pool (1 MiB)
   b += (size_t)R_HIST * sizeof(int);                          // iteration counts per half-step
@@ -437,6 +444,60 @@ int setup_hm_tma(fdtd_llg *s) {
   return FDTD_LLG_OK;
 }
 
+// ---- staged sweeps (hm_stage.cuh) ----------------------------------------------------------
+
+// SW x by columns marched over kz planes; a persistent grid of `grid` blocks draws the items
+// dynamically.  kz: as long as possible (every item loads one extra stage) while leaving >= 24
+// items per block, so that the last items of the sweep are a small fraction of it; >= 32 planes.
+StBox make_stbox(const int lo[3], const int hi[3], int by, int grid) {
+  StBox b{};
+  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
+  b.ntx = (hi[0] - lo[0] + SW - 1) / SW;
+  b.nty = (hi[1] - lo[1] + by - 1) / by;
+  const int ez = std::max(1, hi[2] - lo[2]);
+  const long long cols = (long long)b.ntx * b.nty;
+  int nc = 1;
+  while (cols * nc < 24LL * grid && (ez + nc) / (nc + 1) >= 32) ++nc;
+  b.kz = (ez + nc - 1) / nc;
+  b.items = (int)(cols * ((ez + b.kz - 1) / b.kz));
+  return b;
+}
+
+template <int BY, bool FIRST>
+int launch_hm_stage_by(fdtd_llg *s, const HMSArgs &p) {
+  const bool ms = s->Ms.is_array, an = s->opt.ani_hk != 0.0;
+  const int grid = std::max(1, std::min(p.tb.items, s->num_sms * StLayout<BY, FIRST, true>::BPS));
+#define SK(MS, AN)                                                                          \
+  if (ms == MS && an == AN) {                                                               \
+    using L = StLayout<BY, FIRST, MS>;                                                      \
+    k_hm_stage<BY, FIRST, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);      \
+    return FDTD_LLG_OK;                                                                     \
+  }
+  SK(false, false) SK(false, true) SK(true, false) SK(true, true)
+#undef SK
+  return FDTD_LLG_OK;
+}
+template <bool FIRST>
+int launch_hm_stage(fdtd_llg *s, const HMSArgs &p) {
+  return s->stage_by == 16 ? launch_hm_stage_by<16, FIRST>(s, p) : launch_hm_stage_by<7, FIRST>(s, p);
+}
+
+template <int BY>
+int setup_hm_stage_by(fdtd_llg *s) {
+#define SA(FIRST, MS, AN)                                                                   \
+  CU(s, cudaFuncSetAttribute(k_hm_stage<BY, FIRST, MS, AN>,                                 \
+                             cudaFuncAttributeMaxDynamicSharedMemorySize,                   \
+                             (int)StLayout<BY, FIRST, MS>::SMEM_BYTES));
+  SA(true, false, false) SA(true, false, true) SA(true, true, false) SA(true, true, true)
+  SA(false, false, false) SA(false, false, true) SA(false, true, false) SA(false, true, true)
+#undef SA
+  int rc;
+  if ((rc = make_map(s, &s->mapT, SROW, BY + 1, 1))) return rc;
+  if ((rc = make_map(s, &s->mapPM, SW, BY, 9))) return rc;
+  s->st_box = make_stbox(s->lo, s->hi, BY, s->num_sms * StLayout<BY, true, true>::BPS);
+  return FDTD_LLG_OK;
+}
+
 // ---- launching one step ----------------------------------------------------------------
 
 template <bool FIRST>
@@ -491,7 +552,7 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
     a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
-    if (s->tma_hm && s->Ms.is_array) {  // k_hm_tma: the most common face value and its reciprocal
+    if ((s->tma_hm || s->stage_by) && s->Ms.is_array) {  // the most common face value and its reciprocal
       a.Ms_u = s->Ms.maxv;
       a.rMs_u = 1.0 / s->Ms.maxv;
     }
@@ -520,7 +581,19 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
       if (a.Ms) a.pf[a.npf++] = a.Ms;
       prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
       int rc;
-      if (s->tma_hm) {
+      if (s->stage_by) {
+        HMSArgs p{};
+        p.a = a;
+        p.tb = s->st_box;
+        p.mapT = s->mapT; p.mapM = s->mapPM;
+        p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
+        p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
+        p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
+        p.work = s->work + r;
+        p.tune = s->tune;
+        p.m_ahead = s->m_ahead;
+        rc = (r == 1) ? launch_hm_stage<true>(s, p) : launch_hm_stage<false>(s, p);
+      } else if (s->tma_hm) {
         HMTArgs p{};
         p.a = a;
         p.tb = s->tile_llg;
@@ -538,7 +611,7 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     }
   }
   prof_begin(s, FDTD_LLG_K_OTHER, 0);
-  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->r_hist, s->opt.llg_max_iter,
+  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->r_hist, s->opt.llg_max_iter,
                                      s->opt.llg_tol, s->llg ? 1 : 0, last ? 1 : 0);
   ++*launches;
   if (s->llg && s->opt.llg_max_iter >= 2) {
@@ -718,7 +791,8 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   // carve the workspace: small state first, then the big arrays
   char *p = s->ws;
   s->dstate = reinterpret_cast<DevState *>(p); p += 4096;
-  s->resid = reinterpret_cast<unsigned long long *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 4096;
+  s->resid = reinterpret_cast<unsigned long long *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8;
+  s->work = reinterpret_cast<unsigned *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 4096;
   s->scratch = reinterpret_cast<double *>(p); p += (2 * 1024 + 64) * 8;
   s->profile_pool = reinterpret_cast<double *>(p); s->profile_cap = ((size_t)1 << 20) / 8; p += (size_t)1 << 20;
   s->r_hist = reinterpret_cast<int *>(p); p += (size_t)R_HIST * sizeof(int);
@@ -749,9 +823,13 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   if ((rc = find_sweep_box(s))) return bail(rc);
   make_boxes(s);
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
-  s->tma_hm = s->llg && opt->kernel_path == 0 && !s->alpha.is_array && !s->gamma.is_array &&
-              !s->mu_r.is_array;
+  const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
+  s->tma_hm = smem_ok && opt->kernel_path == 2;
   if (s->tma_hm && (rc = setup_hm_tma(s))) return bail(rc);
+  if (const char *e = getenv("FDTD_LLG_TUNE")) sscanf(e, "%d,%d", &s->tune, &s->m_ahead);
+  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
+  if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
+  if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
   *out = s;
@@ -786,6 +864,7 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
   // reset run state
   CU(s, cudaMemsetAsync(s->dstate, 0, sizeof(DevState), s->stream));
   CU(s, cudaMemsetAsync(s->resid, 0, (size_t)(s->opt.llg_max_iter + 2) * 8, s->stream));
+  CU(s, cudaMemsetAsync(s->work, 0, (size_t)(s->opt.llg_max_iter + 2) * 4, s->stream));
   if (s->opt.enable_llg) {
     InitMP a{};
     a.g = s->g;

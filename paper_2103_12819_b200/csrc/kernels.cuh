@@ -442,13 +442,33 @@ __device__ __forceinline__ void store_face(const HMArgs &a, int c, const FaceOut
   __stcs(a.Mr[3 * D + 2] + c, o.m.z);
   a.Hc[D][c] = o.h;
 }
+// periodic ghost images of an interior value, inlined (no call: a call would wait for every load
+// the caller has in flight).  Up to two shifts per axis (both when the axis is one cell long).
+__device__ __forceinline__ void store_images_inl(double *a, const GridP &g, int i, int j, int k,
+                                                 int c, double v) {
+  const int sx[3] = {0, (g.per[0] && i == 0) ? g.n[0] : 0, (g.per[0] && i == g.n[0] - 1) ? -g.n[0] : 0};
+  const int sy[3] = {0, (g.per[1] && j == 0) ? g.n[1] * g.sy : 0,
+                     (g.per[1] && j == g.n[1] - 1) ? -g.n[1] * g.sy : 0};
+  const int sz[3] = {0, (g.per[2] && k == 0) ? g.n[2] * g.sz : 0,
+                     (g.per[2] && k == g.n[2] - 1) ? -g.n[2] * g.sz : 0};
+#pragma unroll
+  for (int x = 0; x < 3; ++x)
+#pragma unroll
+    for (int y = 0; y < 3; ++y)
+#pragma unroll
+      for (int z = 0; z < 3; ++z) {
+        if (!(x | y | z)) continue;
+        if ((x && !sx[x]) || (y && !sy[y]) || (z && !sz[z])) continue;
+        a[c + sx[x] + sy[y] + sz[z]] = v;
+      }
+}
+
+// Only H is ever read through a ghost (the four-point averages and curl H); M is read by the
+// thread that owns the face, so its ghosts need no refresh.
 template <int D>
 __device__ __forceinline__ void store_face_images(const HMArgs &a, int i, int j, int k, int c,
                                                   const FaceOut &o) {
-  store_images(a.Mr[3 * D + 0], a.g, i, j, k, c, o.m.x);
-  store_images(a.Mr[3 * D + 1], a.g, i, j, k, c, o.m.y);
-  store_images(a.Mr[3 * D + 2], a.g, i, j, k, c, o.m.z);
-  store_images(a.Hc[D], a.g, i, j, k, c, o.h);
+  store_images_inl(a.Hc[D], a.g, i, j, k, c, o.h);
 }
 
 template <bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
@@ -509,7 +529,7 @@ __global__ void __launch_bounds__(NTHREADS) k_hm_sweep(const __grid_constant__ H
 }
 
 // 1 thread: close an (H,M) half-step
-__global__ void k_half_end(DevState *st, unsigned long long *resid, int *r_hist, int max_iter,
+__global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, int *r_hist, int max_iter,
                            double tol, int any_magnetic, int last_of_step) {
   if (any_magnetic) {
     int R = max_iter;
@@ -522,7 +542,7 @@ __global__ void k_half_end(DevState *st, unsigned long long *resid, int *r_hist,
     if (R > st->iters_max) st->iters_max = R;
     st->resid_last = res;
     st->last_R_even = ((R & 1) == 0);
-    for (int r = 1; r <= max_iter; ++r) resid[r] = 0ull;
+    for (int r = 1; r <= max_iter; ++r) { resid[r] = 0ull; work[r] = 0u; }
   } else {
     st->iters_last = 0;
     st->last_R_even = 0;

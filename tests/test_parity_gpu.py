@@ -112,21 +112,23 @@ def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
 
 @pytest.mark.parametrize("cfg,shape", [(1, (32, 32, 32)), (4, (44, 36, 40)), (5, (40, 44, 36)),
                                        (5, (70, 19, 23)), (4, (33, 8, 50))])
-def test_tma_pipeline_equals_direct_load_kernels_bitwise(cfg, shape):
-    """kernel_path 0 (TMA-fed shared-memory rings) and 1 (direct global loads) share the
-    arithmetic (hm_face_core): every field and the iteration counts agree bit for bit, on shapes
-    with ragged tiles in x and y and several z chunks."""
+def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
+    """kernel_path 0 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell), 2 (all-TMA
+    sweep, warp = (face, row)) and 1 (direct global loads) share the arithmetic (hm_face_core):
+    every field and the iteration counts agree bit for bit, on shapes with ragged tiles in x and
+    y and several z chunks."""
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(cfg, shape=shape)
     outs, stats = [], []
-    for path in (0, 1):
+    for path in (1, 0, 2, 3):
         sim = from_workload(w, kernel_path=path)
         sim.step(25)
         outs.append(_gpu_fields(sim))
         stats.append(sim.stats())
-    for n in outs[0]:
-        assert np.array_equal(outs[0][n], outs[1][n]), n
-    assert stats[0]["iters_total"] == stats[1]["iters_total"] > 0
+    for other, st in zip(outs[1:], stats[1:]):
+        for n in outs[0]:
+            assert np.array_equal(outs[0][n], other[n]), n
+        assert stats[0]["iters_total"] == st["iters_total"] > 0
 
 
 def test_device_resident_inputs_equal_host_inputs():
