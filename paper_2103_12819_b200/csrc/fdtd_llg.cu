@@ -54,7 +54,8 @@ struct fdtd_llg {
   char *ws = nullptr;
   size_t ws_bytes = 0;
 
-  double *E[3]{};
+  double *E[3]{};   // E set 0 (time n when host_steps is even)
+  double *E2[3]{};  // E set 1: the E update is out of place, the two sets alternate
   double *Hset[3][3]{};  // three H sets (time-n, ping, pong), statically rotated per half-step
   double *Mset[2][9]{};  // two M sets
   MatInfo eps_r, sigma, mu_r, Ms, alpha, gamma;
@@ -77,7 +78,6 @@ struct fdtd_llg {
   DevState *dstate = nullptr;
   unsigned long long *resid = nullptr;
   unsigned *work = nullptr;  // [max_iter + 1] item counters of the staged sweeps
-  int tune = 3, m_ahead = 0;
   double *scratch = nullptr;  // 2*1024 doubles for reductions + 8 ints
   SourcesP src{};
   double *profile_pool = nullptr;
@@ -89,8 +89,8 @@ struct fdtd_llg {
   int prof_half = 0;
   int *r_hist = nullptr;  // device: iteration count R of half-step h at [h % R_HIST]
 
-  cudaGraphExec_t graph = nullptr;
-  bool graph_valid = false;
+  cudaGraphExec_t graph[2] = {nullptr, nullptr};  // one captured step per E parity
+  bool graph_valid[2] = {false, false};
   int launches_per_step = 0;
   long long kernel_launches = 0;
   long long host_steps = 0;
@@ -522,17 +522,14 @@ int launch_sweep(fdtd_llg *s, const HMArgs &a, int grid) {
 
 // (H,M) half-step: time-n set `in`, result in set `out`, `tmp` is the other Jacobi buffer.
 // M: time-n set `min`, result in set `mout`.
-int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool last,
+int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int min, int mout, bool last,
                  int *launches) {
   const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
-  for (int d = 0; d < 3; ++d) { h.E[d] = s->E[d]; h.Hn[d] = s->Hset[in][d]; h.Hc[d] = s->Hset[out][d]; }
+  for (int d = 0; d < 3; ++d) { h.E[d] = E[d]; h.Hn[d] = s->Hset[in][d]; h.Hc[d] = s->Hset[out][d]; }
   h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
   h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
-  h.npf = 0;
-  for (int d = 0; d < 3; ++d) { h.pf[h.npf++] = s->E[d]; h.pf[h.npf++] = s->Hset[in][d]; }
-  if (h.mu_r) h.pf[h.npf++] = h.mu_r;
   for (int b = 0; b < s->n_out; ++b) {
     h.box = s->box_out[b];
     if (h.box.items == 0) continue;
@@ -547,7 +544,7 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
     HMArgs a{};
     a.g = s->g;
     a.box = s->box_llg;
-    for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.Hn[d] = s->Hset[in][d]; }
+    for (int d = 0; d < 3; ++d) { a.E[d] = E[d]; a.Hn[d] = s->Hset[in][d]; }
     for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
@@ -571,14 +568,6 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
       const int to = (r & 1) ? out : tmp;
       for (int d = 0; d < 3; ++d) { a.Hp[d] = s->Hset[from][d]; a.Hc[d] = s->Hset[to][d]; }
       a.r = r;
-      a.npf = 0;
-      for (int d = 0; d < 3; ++d) { a.pf[a.npf++] = a.E[d]; a.pf[a.npf++] = a.Hn[d]; }
-      for (int q = 0; q < 9; ++q) a.pf[a.npf++] = a.Mn[q];
-      if (r > 1) {
-        for (int d = 0; d < 3; ++d) a.pf[a.npf++] = a.Hp[d];
-        for (int q = 0; q < 9; ++q) a.pf[a.npf++] = a.Mr[q];
-      }
-      if (a.Ms) a.pf[a.npf++] = a.Ms;
       prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
       int rc;
       if (s->stage_by) {
@@ -590,8 +579,6 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
         p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
         p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
         p.work = s->work + r;
-        p.tune = s->tune;
-        p.m_ahead = s->m_ahead;
         rc = (r == 1) ? launch_hm_stage<true>(s, p) : launch_hm_stage<false>(s, p);
       } else if (s->tma_hm) {
         HMTArgs p{};
@@ -629,21 +616,17 @@ int enqueue_half(fdtd_llg *s, int in, int out, int tmp, int min, int mout, bool 
   return FDTD_LLG_OK;
 }
 
-int enqueue_e(fdtd_llg *s, int hset, int *launches) {
+int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int *launches) {
   const dim3 blk(TX, TY, 1);
   EArgs a{};
   a.g = s->g;
   a.box = s->box_all;
-  for (int d = 0; d < 3; ++d) { a.E[d] = s->E[d]; a.H[d] = s->Hset[hset][d]; }
+  for (int d = 0; d < 3; ++d) { a.E[d] = Ein[d]; a.Eo[d] = Eout[d]; a.H[d] = s->Hset[hset][d]; }
   a.eps_r = s->eps_r.dev; a.sigma = s->sigma.dev;
   a.eps_u = kEps0 * s->eps_r.uniform; a.sigma_u = s->sigma.uniform;
   a.src = s->src;
   a.st = s->dstate;
   const int grid = grid_for(s, a.box, 0);
-  a.npf = 0;
-  for (int d = 0; d < 3; ++d) { a.pf[a.npf++] = a.E[d]; a.pf[a.npf++] = a.H[d]; }
-  if (a.eps_r) a.pf[a.npf++] = a.eps_r;
-  if (a.sigma) a.pf[a.npf++] = a.sigma;
   const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = s->src.count > 0;
 #define EK(EA, SA, HS)                                                        \
   if (ea == EA && sa == SA && hs == HS) k_e_update<EA, SA, HS><<<grid, blk, 0, s->stream>>>(a);
@@ -659,36 +642,38 @@ int enqueue_e(fdtd_llg *s, int hset, int *launches) {
 
 // one full time step: HM half (curl E^n), E update, HM half (curl E^{n+1}).
 // H sets: state in 0 -> half 1 result in 1 -> half 2 result back in 0.  M sets: 0 -> 1 -> 0.
-int enqueue_step(fdtd_llg *s, int *launches) {
+// one time step; par = parity of the step: E^n is in E set `par`, E^{n+1} goes to the other set
+int enqueue_step(fdtd_llg *s, int par, int *launches) {
   *launches = 0;
+  double *const *Ea = par ? s->E2 : s->E, *const *Eb = par ? s->E : s->E2;
   if (s->src.count > 0) {
     prof_begin(s, FDTD_LLG_K_OTHER, 0);
     k_step_begin<<<1, 32, 0, s->stream>>>(s->dstate, s->src, s->dt);
     prof_end(s);
     ++*launches;
   }
-  int rc = enqueue_half(s, 0, 1, 2, 0, 1, false, launches);
+  int rc = enqueue_half(s, Ea, 0, 1, 2, 0, 1, false, launches);
   if (rc) return rc;
-  rc = enqueue_e(s, 1, launches);
+  rc = enqueue_e(s, Ea, Eb, 1, launches);
   if (rc) return rc;
-  return enqueue_half(s, 1, 0, 2, 1, 0, true, launches);
+  return enqueue_half(s, Eb, 1, 0, 2, 1, 0, true, launches);
 }
 
-int build_graph(fdtd_llg *s) {
-  if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
-  s->graph_valid = false;
+int build_graph(fdtd_llg *s, int par) {
+  if (s->graph[par]) { cudaGraphExecDestroy(s->graph[par]); s->graph[par] = nullptr; }
+  s->graph_valid[par] = false;
   cudaGraph_t g = nullptr;
   CU(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
   int launches = 0;
-  int rc = enqueue_step(s, &launches);
+  int rc = enqueue_step(s, par, &launches);
   cudaError_t e = cudaStreamEndCapture(s->stream, &g);
   if (rc) { if (g) cudaGraphDestroy(g); return rc; }
   if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
-  e = cudaGraphInstantiate(&s->graph, g, 0);
+  e = cudaGraphInstantiate(&s->graph[par], g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
   s->launches_per_step = launches;
-  s->graph_valid = true;
+  s->graph_valid[par] = true;
   return FDTD_LLG_OK;
 }
 
@@ -720,8 +705,8 @@ size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *
                                 unsigned material_mask) {
   if (nx < 1 || ny < 1 || nz < 1 || !opt) return 0;
   const size_t stride = array_stride(nx, ny, nz);
-  size_t arrays = 6;                       // E, H
-  if (opt->enable_llg) arrays += 6 + 18;   // two more H sets, two M sets
+  size_t arrays = 12;                      // two E sets, two H sets (every update is out of place)
+  if (opt->enable_llg) arrays += 3 + 18;   // the Jacobi H buffer, two M sets
   for (unsigned b = 0; b < 6; ++b)
     if (material_mask & (1u << b)) ++arrays;
   return arrays * stride * sizeof(double) + small_bytes(opt);
@@ -799,16 +784,16 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   p = s->ws + small_bytes(&s->opt);
   double *q = reinterpret_cast<double *>(p);
   for (int d = 0; d < 3; ++d) { s->E[d] = q; q += s->stride; }
-  const int nh = opt->enable_llg ? 3 : 1;
+  for (int d = 0; d < 3; ++d) { s->E2[d] = q; q += s->stride; }
+  const int nh = opt->enable_llg ? 3 : 2;  // every update is out of place
   for (int h = 0; h < nh; ++h)
     for (int d = 0; d < 3; ++d) { s->Hset[h][d] = q; q += s->stride; }
   if (!opt->enable_llg)
-    for (int h = 1; h < 3; ++h)
-      for (int d = 0; d < 3; ++d) s->Hset[h][d] = s->Hset[0][d];  // Maxwell only: in place
+    for (int d = 0; d < 3; ++d) s->Hset[2][d] = s->Hset[1][d];  // Maxwell only: no Jacobi buffer
   if (opt->enable_llg)
     for (int m = 0; m < 2; ++m)
       for (int c = 0; c < 9; ++c) { s->Mset[m][c] = q; q += s->stride; }
-  const size_t state_arrays = 3 + 3 * nh + (opt->enable_llg ? 18 : 0);
+  const size_t state_arrays = 6 + 3 * nh + (opt->enable_llg ? 18 : 0);
   CUB(cudaMemsetAsync(s->ws, 0, small_bytes(&s->opt) + state_arrays * s->stride * sizeof(double), s->stream));
 
   int rc;
@@ -826,7 +811,6 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
   s->tma_hm = smem_ok && opt->kernel_path == 2;
   if (s->tma_hm && (rc = setup_hm_tma(s))) return bail(rc);
-  if (const char *e = getenv("FDTD_LLG_TUNE")) sscanf(e, "%d,%d", &s->tune, &s->m_ahead);
   s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
   if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
   if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
@@ -934,7 +918,7 @@ int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
     s->profile_used += padded(nb);
   }
   s->src.count++;
-  s->graph_valid = false;  // the step's kernel arguments changed
+  s->graph_valid[0] = s->graph_valid[1] = false;  // the step's kernel arguments changed
   return FDTD_LLG_OK;
 }
 
@@ -943,15 +927,18 @@ int fdtd_llg_step(fdtd_llg *s, int n) {
   if (n < 0) return fail(s, FDTD_LLG_EINVAL, "n must be >= 0");
   if (n == 0) return FDTD_LLG_OK;
   if (s->opt.use_graph) {
-    if (!s->graph_valid) {
-      int rc = build_graph(s);
-      if (rc) return rc;
+    for (int t = 0; t < n; ++t) {
+      const int par = (int)((s->host_steps + t) & 1);
+      if (!s->graph_valid[par]) {
+        int rc = build_graph(s, par);
+        if (rc) return rc;
+      }
+      CU(s, cudaGraphLaunch(s->graph[par], s->stream));
     }
-    for (int t = 0; t < n; ++t) CU(s, cudaGraphLaunch(s->graph, s->stream));
   } else {
     for (int t = 0; t < n; ++t) {
       int launches = 0;
-      int rc = enqueue_step(s, &launches);
+      int rc = enqueue_step(s, (int)((s->host_steps + t) & 1), &launches);
       if (rc) return rc;
       s->launches_per_step = launches;
     }
@@ -974,7 +961,7 @@ int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *laun
   int rc = FDTD_LLG_OK;
   for (int t = 0; t < n && !rc; ++t) {
     int launches = 0;
-    rc = enqueue_step(s, &launches);
+    rc = enqueue_step(s, (int)((s->host_steps + t) & 1), &launches);
     s->launches_per_step = launches;
   }
   s->prof = nullptr;
@@ -1009,7 +996,7 @@ int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double
   const size_t bytes = s->ncell * sizeof(double);
   int rc;
   for (int d = 0; d < 3; ++d) {
-    if (E && E[d] && (rc = copy_out(s, E[d], s->E[d], mem_space))) return rc;
+    if (E && E[d] && (rc = copy_out(s, E[d], ((s->host_steps & 1) ? s->E2 : s->E)[d], mem_space))) return rc;
     if (H && H[d] && (rc = copy_out(s, H[d], s->Hset[0][d], mem_space))) return rc;
   }
   if (M)
@@ -1061,7 +1048,8 @@ const char *fdtd_llg_last_error(const fdtd_llg *s) {
 
 void fdtd_llg_destroy(fdtd_llg *s) {
   if (!s) return;
-  if (s->graph) cudaGraphExecDestroy(s->graph);
+  for (int p = 0; p < 2; ++p)
+    if (s->graph[p]) cudaGraphExecDestroy(s->graph[p]);
   delete s;
 }
 

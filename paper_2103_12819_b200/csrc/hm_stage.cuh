@@ -65,8 +65,6 @@ struct HMSArgs {
   CUtensorMap mapM;  // box (SW, BY, 1, 9): L2 prefetch of an M set's plane
   int aE, aHn, aHp, aMn, aMp, aMs;  // array indices (4th tensor coordinate)
   unsigned *work;  // item counter of this iterate (zero at launch; k_half_end re-arms it)
-  int tune;        // bit 0: L2 prefetch of the next stage's boxes, bit 1: of the M planes
-  int m_ahead;     // M plane prefetched when stage pz is issued: pz + m_ahead
 };
 
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int c0, int c1, int c2, int c3) {
@@ -185,16 +183,12 @@ __device__ __forceinline__ void s_load_m(const HMArgs &a, int c, Vec3 &mn, Vec3 
 }
 
 // the TMA loads of stage pz of the tile at (x0, y0): tensor coordinates x = PADL + i, y = j + 1,
-// z = k + 1 (one ghost layer).  PREFETCH: the same boxes as L2 prefetches.
-template <class L, bool FIRST, bool MS_ARR, bool PREFETCH>
+// z = k + 1 (one ghost layer)
+template <class L, bool FIRST, bool MS_ARR>
 __device__ __forceinline__ void s_issue_stage(const HMSArgs &p, double *dst, uint64_t *bar, int x0,
                                               int y0, int pz) {
   const int xa = PADL + x0, xb = PADL + x0 - 2, ya = y0 + 1, yb = y0, z = pz + 1;
-#define S_BOX(slot, cx, cy, cz, arr)                                         \
-  do {                                                                       \
-    if (PREFETCH) tma_prefetch_4d(&p.mapT, cx, cy, cz, arr);                 \
-    else tma_load_4d(dst + (slot), &p.mapT, bar, cx, cy, cz, arr);           \
-  } while (0)
+#define S_BOX(slot, cx, cy, cz, arr) tma_load_4d(dst + (slot), &p.mapT, bar, cx, cy, cz, arr)
   S_BOX(L::HN + 0 * L::SLOT, xa, yb, z, p.aHn + 0);
   S_BOX(L::HN + 1 * L::SLOT, xb, ya, z, p.aHn + 1);
   S_BOX(L::HN + 2 * L::SLOT, xb, yb, z + 1, p.aHn + 2);
@@ -262,12 +256,9 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
         const int it = (int)atomicAdd(p.work, 1u);
         const bool end = it >= T.items;
         const StItem w = st_decode(T, end ? 0 : it, BY);
-        if (!end) {  // the first planes of a fresh column, towards L2
-          if (p.tune & 1) s_issue_stage<L, FIRST, MS_ARR, true>(p, nullptr, nullptr, w.x0, w.y0, w.k0 - 1);
-          if (p.tune & 2) {
-            tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMn);
-            if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMp);
-          }
+        if (!end) {  // the first M plane of a fresh column, towards L2
+          tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMn);
+          if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMp);
         }
         for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1); ++pz, ++n) {
           const unsigned s = n % L::NS, u = n / L::NS;
@@ -278,14 +269,12 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
             break;
           }
           mbar_expect_tx(full + s, L::BYTES);
-          s_issue_stage<L, FIRST, MS_ARR, false>(p, ring + s * L::STAGE, full + s, w.x0, w.y0, pz);
-          // towards L2, one step ahead of their use: the next stage's boxes, and the M planes the
-          // compute warps load while they work on plane pz - 1
-          if ((p.tune & 1) && pz + 1 < w.k1)
-            s_issue_stage<L, FIRST, MS_ARR, true>(p, nullptr, nullptr, w.x0, w.y0, pz + 1);
-          if ((p.tune & 2) && pz + p.m_ahead >= w.k0 && pz + p.m_ahead < w.k1) {
-            tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + p.m_ahead + 1, p.aMn);
-            if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + p.m_ahead + 1, p.aMp);
+          s_issue_stage<L, FIRST, MS_ARR>(p, ring + s * L::STAGE, full + s, w.x0, w.y0, pz);
+          // towards L2: the M planes the compute warps will load while they work on plane pz - 1
+          // (about one plane time ahead: long enough to cover HBM latency, short enough to survive in L2)
+          if (pz >= w.k0) {
+            tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + 1, p.aMn);
+            if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + 1, p.aMp);
           }
         }
         if (end) break;

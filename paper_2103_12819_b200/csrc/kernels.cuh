@@ -36,7 +36,6 @@ constexpr int PADL = 16;         // doubles left of i = 0 in a row (ghost i = -1
 constexpr int TX = 32, TY = 8;   // thread block = TX x TY columns
 constexpr int NTHREADS = TX * TY;
 constexpr int KZ_MAX = 16;       // planes marched per work item (fewer on small grids)
-constexpr int MAX_PF = 32;       // arrays a kernel can prefetch
 
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kMu0 = 4.0e-7 * kPi;
@@ -116,25 +115,26 @@ __device__ __forceinline__ bool edge_k(const GridP &g, int k) {
 }
 __device__ __forceinline__ bool wall_k(const GridP &g, int k) { return !g.per[2] && k == 0; }
 
-// slow path of a store: the periodic ghost images of an interior value
-__device__ __noinline__ void store_images(double *a, const GridP &g, int i, int j, int k, int c,
-                                          double v) {
-  const int idx[3] = {i, j, k};
-  const int st[3] = {1, g.sy, g.sz};
-  int sh[3][3], cnt[3];
+// slow path of a store: the periodic ghost images of an interior value, inlined
+// (no call: a call would wait for every load
+// the caller has in flight).  Up to two shifts per axis (both when the axis is one cell long).
+__device__ __forceinline__ void store_images_inl(double *a, const GridP &g, int i, int j, int k,
+                                                 int c, double v) {
+  const int sx[3] = {0, (g.per[0] && i == 0) ? g.n[0] : 0, (g.per[0] && i == g.n[0] - 1) ? -g.n[0] : 0};
+  const int sy[3] = {0, (g.per[1] && j == 0) ? g.n[1] * g.sy : 0,
+                     (g.per[1] && j == g.n[1] - 1) ? -g.n[1] * g.sy : 0};
+  const int sz[3] = {0, (g.per[2] && k == 0) ? g.n[2] * g.sz : 0,
+                     (g.per[2] && k == g.n[2] - 1) ? -g.n[2] * g.sz : 0};
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    cnt[d] = 0;
-    sh[d][cnt[d]++] = 0;
-    if (g.per[d]) {
-      if (idx[d] == 0) sh[d][cnt[d]++] = g.n[d] * st[d];            // ghost at index n
-      if (idx[d] == g.n[d] - 1) sh[d][cnt[d]++] = -g.n[d] * st[d];  // ghost at index -1
-    }
-  }
-  for (int x = 0; x < cnt[0]; ++x)
-    for (int y = 0; y < cnt[1]; ++y)
-      for (int z = 0; z < cnt[2]; ++z)
-        if (x | y | z) a[c + sh[0][x] + sh[1][y] + sh[2][z]] = v;
+  for (int x = 0; x < 3; ++x)
+#pragma unroll
+    for (int y = 0; y < 3; ++y)
+#pragma unroll
+      for (int z = 0; z < 3; ++z) {
+        if (!(x | y | z)) continue;
+        if ((x && !sx[x]) || (y && !sy[y]) || (z && !sz[z])) continue;
+        a[c + sx[x] + sy[y] + sz[z]] = v;
+      }
 }
 
 // (curl E)_D at the D-face: forward differences (standard Yee)
@@ -159,42 +159,18 @@ __device__ __forceinline__ double avg4(const GridP &g, int c, const double *__re
 // work-item decode shared by the sweeping kernels
 struct Item {
   int i, j, k0, k1;
-  int i0, j0, rows, width;  // tile origin and its valid extent (for the plane prefetch)
   bool active;
 };
 __device__ __forceinline__ Item decode_item(const BoxP &b, int it) {
   const int tx = it % b.ntx, r = it / b.ntx;
   const int ty = r % b.nty, tz = r / b.nty;
   Item w;
-  w.i0 = b.lo[0] + tx * TX;
-  w.j0 = b.lo[1] + ty * TY;
-  w.i = w.i0 + (int)threadIdx.x;
-  w.j = w.j0 + (int)threadIdx.y;
-  w.rows = min(TY, b.hi[1] - w.j0);
-  w.width = min(TX, b.hi[0] - w.i0);
+  w.i = b.lo[0] + tx * TX + (int)threadIdx.x;
+  w.j = b.lo[1] + ty * TY + (int)threadIdx.y;
   w.k0 = b.lo[2] + tz * b.kz;
   w.k1 = min(w.k0 + b.kz, b.hi[2]);
   w.active = w.i < b.hi[0] && w.j < b.hi[1];
   return w;
-}
-
-// L2 prefetch of the NEXT z-plane of this block's tile: one cp.async.bulk.prefetch per
-// (array, row), issued by one thread each, so that the z march finds its streamed operands in
-// L2 instead of paying the HBM latency.  A hint only: rows are widened to 16-byte alignment.
-// ptrs[n]: the arrays; c_row0: offset of (tile x0, tile y0, k+1); rows: valid rows of the tile.
-__device__ __forceinline__ void prefetch_plane(const double *const *ptrs, int n, int c_row0, int sy,
-                                               int rows, int width) {
-  const int t = threadIdx.x + TX * threadIdx.y;
-  for (int q = t; q < n * TY; q += NTHREADS) {
-    const int arr = q / TY, row = q % TY;
-    if (row < rows) {
-      const unsigned long long raw = (unsigned long long)(ptrs[arr] + c_row0 + row * sy);
-      const unsigned long long addr = raw & ~15ull;
-      const unsigned bytes = (unsigned)((raw - addr) + width * 8 + 15) & ~15u;
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(addr), "r"(bytes)
-                   : "memory");
-    }
-  }
 }
 
 // ------------------------------------------------------------------ Maxwell H half-step
@@ -207,8 +183,6 @@ struct HArgs {
   double *Hc[3];
   const double *mu_r;  // cell-centred array or nullptr (uniform)
   double ch_uniform;   // dt / (2 mu0 mu_r) when uniform
-  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
-  int npf;
 };
 
 // eq. 21 with M = 0 and the local mu; a PEC wall face stays 0
@@ -230,12 +204,9 @@ __global__ void __launch_bounds__(NTHREADS) k_h_update(const __grid_constant__ H
   for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
     const Item w = decode_item(a.box, it);
     const Column col = make_column(a.g, w.i, w.j);
+    if (!w.active) continue;
     int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
-    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
     for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
-      c_tile += a.g.sz;
-      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
-      if (!w.active) continue;
       const double hx = h_face<0, MU_ARR>(a, c, col.wall[0]);
       const double hy = h_face<1, MU_ARR>(a, c, col.wall[1]);
       const double hz = h_face<2, MU_ARR>(a, c, wall_k(a.g, k));
@@ -243,9 +214,9 @@ __global__ void __launch_bounds__(NTHREADS) k_h_update(const __grid_constant__ H
       a.Hc[1][c] = hy;
       a.Hc[2][c] = hz;
       if (col.edge_ij || edge_k(a.g, k)) {
-        store_images(a.Hc[0], a.g, w.i, w.j, k, c, hx);
-        store_images(a.Hc[1], a.g, w.i, w.j, k, c, hy);
-        store_images(a.Hc[2], a.g, w.i, w.j, k, c, hz);
+        store_images_inl(a.Hc[0], a.g, w.i, w.j, k, c, hx);
+        store_images_inl(a.Hc[1], a.g, w.i, w.j, k, c, hy);
+        store_images_inl(a.Hc[2], a.g, w.i, w.j, k, c, hz);
       }
     }
   }
@@ -269,8 +240,6 @@ struct HMArgs {
   unsigned long long *resid;  // [max_iter + 1] bit patterns of the residual of iterate r
   int *pipe_error;            // &DevState::pipe_error
   int r;
-  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
-  int npf;
 };
 
 struct Vec3 { double x, y, z; };
@@ -442,27 +411,6 @@ __device__ __forceinline__ void store_face(const HMArgs &a, int c, const FaceOut
   __stcs(a.Mr[3 * D + 2] + c, o.m.z);
   a.Hc[D][c] = o.h;
 }
-// periodic ghost images of an interior value, inlined (no call: a call would wait for every load
-// the caller has in flight).  Up to two shifts per axis (both when the axis is one cell long).
-__device__ __forceinline__ void store_images_inl(double *a, const GridP &g, int i, int j, int k,
-                                                 int c, double v) {
-  const int sx[3] = {0, (g.per[0] && i == 0) ? g.n[0] : 0, (g.per[0] && i == g.n[0] - 1) ? -g.n[0] : 0};
-  const int sy[3] = {0, (g.per[1] && j == 0) ? g.n[1] * g.sy : 0,
-                     (g.per[1] && j == g.n[1] - 1) ? -g.n[1] * g.sy : 0};
-  const int sz[3] = {0, (g.per[2] && k == 0) ? g.n[2] * g.sz : 0,
-                     (g.per[2] && k == g.n[2] - 1) ? -g.n[2] * g.sz : 0};
-#pragma unroll
-  for (int x = 0; x < 3; ++x)
-#pragma unroll
-    for (int y = 0; y < 3; ++y)
-#pragma unroll
-      for (int z = 0; z < 3; ++z) {
-        if (!(x | y | z)) continue;
-        if ((x && !sx[x]) || (y && !sy[y]) || (z && !sz[z])) continue;
-        a[c + sx[x] + sy[y] + sz[z]] = v;
-      }
-}
-
 // Only H is ever read through a ghost (the four-point averages and curl H); M is read by the
 // thread that owns the face, so its ghosts need no refresh.
 template <int D>
@@ -481,12 +429,9 @@ __global__ void __launch_bounds__(NTHREADS) k_hm_sweep(const __grid_constant__ H
   for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
     const Item w = decode_item(a.box, it);
     const Column col = make_column(a.g, w.i, w.j);
+    if (!w.active) continue;
     int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
-    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
     for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
-      c_tile += a.g.sz;
-      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
-      if (!w.active) continue;
       double Ms_c = a.Ms_u, rMs_c = a.rMs_u;
       if (MS_ARR) {
         Ms_c = __ldg(a.Ms + c);
@@ -573,7 +518,7 @@ __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ Cano
       for (int d = 0; d < 3; ++d) {
         const double v = __ldg(a.src[d] + c);
         a.dst[d][c] = v;
-        if (edge) store_images(a.dst[d], a.g, w.i, w.j, k, c, v);
+        if (edge) store_images_inl(a.dst[d], a.g, w.i, w.j, k, c, v);
       }
     }
   }
@@ -584,26 +529,23 @@ __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ Cano
 struct EArgs {
   GridP g;
   BoxP box;  // the whole grid
-  double *E[3];
+  const double *E[3];  // E^n
+  double *Eo[3];       // E^{n+1}: the other E set (out of place)
   const double *H[3];
   const double *eps_r, *sigma;  // cell-centred arrays or nullptr (uniform)
   double eps_u, sigma_u;        // uniform values (eps_u is eps0*eps_r)
   SourcesP src;
   const DevState *st;
-  const double *pf[MAX_PF];  // streamed arrays, prefetched one plane ahead
-  int npf;
 };
 
 // eq. 11 on the D-edge of the cell at offset c; a wall-tangential edge stays 0
-// (PAPER.md:187).  J = soft source term of this edge.
+// (PAPER.md:187).  J = soft source term of this edge; e0 = E^n on the edge; (curl H)_D at the edge
+// by backward differences: h2 - h2m along d1 = D+1, h1 - h1m along d2 = D+2.
 template <int D, bool EPS_ARR, bool SIG_ARR>
-__device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, double J) {
+__device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, double J, double e0,
+                                         double h2, double h2m, double h1, double h1m) {
   constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
   const int s1 = stride_of<d1>(a.g), s2 = stride_of<d2>(a.g);
-  // (curl H)_D at the D-edge: backward differences
-  const double h2 = __ldg(a.H[d2] + c), h2m = __ldg(a.H[d2] + c - s1);
-  const double h1 = __ldg(a.H[d1] + c), h1m = __ldg(a.H[d1] + c - s2);
-  const double e0 = a.E[D][c];
   // four-cell means of eps, sigma at the edge
   double eps = a.eps_u, sig = a.sigma_u;
   if (EPS_ARR)
@@ -616,6 +558,24 @@ __device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, doubl
   const double edt = eps / a.g.dt, hs = 0.5 * sig;
   const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
   return wall ? 0.0 : e1;
+}
+
+// everything the three edges of one cell read
+struct EOps {
+  double e0, e1, e2;
+  double hx, hy, hz;
+  double hx_my, hz_my;  // at j-1
+  double hy_mx, hz_mx;  // at i-1
+  double hx_mz, hy_mz;  // at k-1
+};
+__device__ __forceinline__ EOps e_load(const EArgs &a, int c) {
+  EOps o;
+  o.e0 = __ldg(a.E[0] + c); o.e1 = __ldg(a.E[1] + c); o.e2 = __ldg(a.E[2] + c);
+  o.hx = __ldg(a.H[0] + c); o.hy = __ldg(a.H[1] + c); o.hz = __ldg(a.H[2] + c);
+  o.hx_my = __ldg(a.H[0] + c - a.g.sy); o.hz_my = __ldg(a.H[2] + c - a.g.sy);
+  o.hy_mx = __ldg(a.H[1] + c - 1); o.hz_mx = __ldg(a.H[2] + c - 1);
+  o.hx_mz = __ldg(a.H[0] + c - a.g.sz); o.hy_mz = __ldg(a.H[1] + c - a.g.sz);
+  return o;
 }
 
 // soft sources on the D-edge of cell (i,j,k)
@@ -638,16 +598,14 @@ __device__ __forceinline__ double source_term(const EArgs &a, int i, int j, int 
 }
 
 template <bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
-__global__ void __launch_bounds__(NTHREADS) k_e_update(const __grid_constant__ EArgs a) {
+__global__ void __launch_bounds__(NTHREADS, 4) k_e_update(const __grid_constant__ EArgs a) {
   for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
     const Item w = decode_item(a.box, it);
+    if (!w.active) continue;
     const Column col = make_column(a.g, w.i, w.j);
     int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
-    int c_tile = a.g.org + w.i0 + a.g.sy * w.j0 + a.g.sz * w.k0;
     for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
-      c_tile += a.g.sz;
-      if (k + 1 < w.k1) prefetch_plane(a.pf, a.npf, c_tile, a.g.sy, w.rows, w.width);
-      if (!w.active) continue;
+      const EOps o = e_load(a, c);
       double Jx = 0.0, Jy = 0.0, Jz = 0.0;
       if (HAS_SRC) {
         Jx = source_term<0>(a, w.i, w.j, k);
@@ -655,16 +613,16 @@ __global__ void __launch_bounds__(NTHREADS) k_e_update(const __grid_constant__ E
         Jz = source_term<2>(a, w.i, w.j, k);
       }
       const bool wk = wall_k(a.g, k);
-      const double ex = e_edge<0, EPS_ARR, SIG_ARR>(a, c, col.wall[1] || wk, Jx);
-      const double ey = e_edge<1, EPS_ARR, SIG_ARR>(a, c, wk || col.wall[0], Jy);
-      const double ez = e_edge<2, EPS_ARR, SIG_ARR>(a, c, col.wall[0] || col.wall[1], Jz);
-      a.E[0][c] = ex;
-      a.E[1][c] = ey;
-      a.E[2][c] = ez;
+      const double ex = e_edge<0, EPS_ARR, SIG_ARR>(a, c, col.wall[1] || wk, Jx, o.e0, o.hz, o.hz_my, o.hy, o.hy_mz);
+      const double ey = e_edge<1, EPS_ARR, SIG_ARR>(a, c, wk || col.wall[0], Jy, o.e1, o.hx, o.hx_mz, o.hz, o.hz_mx);
+      const double ez = e_edge<2, EPS_ARR, SIG_ARR>(a, c, col.wall[0] || col.wall[1], Jz, o.e2, o.hy, o.hy_mx, o.hx, o.hx_my);
+      a.Eo[0][c] = ex;
+      a.Eo[1][c] = ey;
+      a.Eo[2][c] = ez;
       if (col.edge_ij || edge_k(a.g, k)) {
-        store_images(a.E[0], a.g, w.i, w.j, k, c, ex);
-        store_images(a.E[1], a.g, w.i, w.j, k, c, ey);
-        store_images(a.E[2], a.g, w.i, w.j, k, c, ez);
+        store_images_inl(a.Eo[0], a.g, w.i, w.j, k, c, ex);
+        store_images_inl(a.Eo[1], a.g, w.i, w.j, k, c, ey);
+        store_images_inl(a.Eo[2], a.g, w.i, w.j, k, c, ez);
       }
     }
   }
