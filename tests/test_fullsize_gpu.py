@@ -1,0 +1,187 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default
+kernel path, CUDA-graph replay).
+
+* configs 2 and 3 (256^3, 512x128x128): the oracle runs the whole grid for a few steps; every
+  element is compared.
+* configs 4 and 5 (384^3, 768^3): the oracle cannot hold the grid (or would take minutes), so it
+  computes SAMPLED outputs instead: a sub-box of the same seeded inputs is cut out and advanced by
+  the oracle; the scheme has a finite domain of dependence (per step: R + 1 cells per (H,M)
+  half-step through the four-point averages and curl E, 1 cell for the E update, i.e. 2R + 3 cells
+  with R LLG iterations), so the core of the sub-box is exactly what the
+  full grid holds there, whatever boundary the cut faces get.  Windows are placed on the structure
+  that matters: the magnetic / non-magnetic interface, a PEC wall, the source plane.
+* config 5 additionally: properties that hold at any size, on the whole 768^3 grid -- |M| = Ms on
+  magnetic faces, M = 0 exactly on non-magnetic faces, div(H + M) unchanged (P8), the
+  iteration counts.
+"""
+import numpy as np
+import pytest
+import torch
+
+from tests._util import FIELD_GROUPS
+from oracle import Oracle
+from paper_2103_12819_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-9
+ALL = FIELD_GROUPS["E"] + FIELD_GROUPS["H"] + FIELD_GROUPS["M"]
+
+
+def _need_gb(gb):
+    free, _ = torch.cuda.mem_get_info(0)
+    if free < gb * 1e9:
+        pytest.skip(f"needs {gb} GB of free device memory, {free / 1e9:.0f} GB available")
+
+
+def _scalar_or_slice(v, sl):
+    if v is None or isinstance(v, (int, float)):
+        return v
+    return v[sl].detach().cpu().numpy().copy()
+
+
+def _window_oracle(w, lo, n, steps, bc):
+    """The oracle on the sub-box [lo, lo+n) of workload w (inputs sliced from the full arrays)."""
+    sl = tuple(slice(lo[d], lo[d] + n[d]) for d in (2, 1, 0))   # arrays are (z, y, x)
+    mats = {k: _scalar_or_slice(v, sl) for k, v in w.materials.items()}
+    full = lambda v: np.full((n[2], n[1], n[0]), float(v)) if isinstance(v, (int, float)) else v
+    o = Oracle(n[0], n[1], n[2], w.dx, w.dy, w.dz, w.dt,
+               eps_r=full(mats.get("eps_r")), sigma=full(mats.get("sigma")), mu_r=full(mats.get("mu_r")),
+               Ms=full(mats.get("Ms")), alpha=full(mats.get("alpha")), gamma=full(mats.get("gamma")),
+               bc=bc, enable_llg=w.enable_llg, h_bias=w.h_bias, ani_hk=w.ani_hk, ani_axis=w.ani_axis,
+               llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter)
+    cut = lambda ts: [None if t is None else t[sl].detach().cpu().numpy().copy() for t in ts]
+    o.set_fields(cut(w.E), cut(w.H), cut(w.M_cell))
+    for s in w.sources:
+        # the part of the source box inside the window, in window coordinates
+        slo = [max(s.lo[d], lo[d]) - lo[d] for d in range(3)]
+        shi = [min(s.hi[d], lo[d] + n[d]) - lo[d] for d in range(3)]
+        if any(a >= b for a, b in zip(slo, shi)):
+            continue
+        prof = None
+        if s.profile is not None:
+            p = s.profile.detach().cpu().numpy()
+            off = [slo[d] + lo[d] - s.lo[d] for d in range(3)]
+            prof = p[off[2]:off[2] + shi[2] - slo[2], off[1]:off[1] + shi[1] - slo[1],
+                     off[0]:off[0] + shi[0] - slo[0]].copy()
+        o.set_source(s.comp, slo, shi, prof, s.amplitude, s.f0, s.t0, s.tp)
+    o.step(steps)
+    return o.read_fields(), o.stats()
+
+
+def _gpu_window(sim, names, lo, n):
+    """Sub-box of the named result arrays, read one array at a time (device -> slice -> host)."""
+    out = {}
+    for nm in names:
+        t = sim.read_fields(names=(nm,), device="cuda:0")[nm]
+        out[nm] = t[lo[2]:lo[2] + n[2], lo[1]:lo[1] + n[1], lo[0]:lo[0] + n[0]].cpu().numpy().copy()
+        del t
+    return out
+
+
+def _scales(ref, groups):
+    return {g: max(float(np.max(np.abs(ref[nm]))) for nm in FIELD_GROUPS[g]) or 1.0 for g in groups}
+
+
+@pytest.mark.parametrize("cfg,steps", [(2, 10), (3, 10)])
+def test_full_size_every_element(cfg, steps):
+    """configs 2, 3 at full size: the oracle runs the whole grid."""
+    from paper_2103_12819_b200.binding import from_workload
+    from tests._util import oracle_from_workload, rel_linf
+    w = wl.make_config(cfg)
+    o = oracle_from_workload(w)
+    o.step(steps)
+    ref = o.read_fields()
+    sim = from_workload(w)
+    sim.step(steps)
+    got = {k: v.numpy() for k, v in sim.read_fields(names=FIELD_GROUPS["E"] + FIELD_GROUPS["H"]).items()}
+    for g in ("E", "H"):
+        assert rel_linf(got, ref, g) <= TOL, (g, rel_linf(got, ref, g))
+    assert sim.stats()["steps"] == steps
+
+
+def test_config4_full_size_windows():
+    """384^3 tunable filter: windows on the slab top (k = 32) under the source plane (k = 48), and
+    on the PEC corner at the origin inside the magnetic slab."""
+    _need_gb(20)
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(4, device="cuda:0")
+    sim = from_workload(w)
+    steps, R = 3, 3
+    sim.step(steps)
+    st = sim.stats()
+    assert st["steps"] == steps and st["nonconverged_halfsteps"] == 0
+    assert st["iters_max"] <= R, st   # the margin below assumes at most R iterations per half-step
+    m = steps * (2 * R + 3)
+    # (window origin, window size, axes whose LOW side is the real PEC wall: no margin there)
+    for lo, n, wall_lo in [
+        ((160, 150, 4), (72, 72, 72), (False, False, False)),     # slab top + source plane
+        ((0, 0, 0), (64, 64, 30 + m), (True, True, True)),         # PEC corner inside the slab
+    ]:
+        ref, ost = _window_oracle(w, lo, n, steps, (0, 0, 0))
+        assert int(ost["iters_total"]) <= 2 * steps * R
+        got = _gpu_window(sim, ALL, lo, n)
+        core = tuple(slice(0 if wall_lo[d] else m, n[d] - m) for d in (2, 1, 0))
+        sc = _scales(ref, ("E", "H", "M"))
+        for g in ("E", "H", "M"):
+            num = max(float(np.max(np.abs(got[nm][core] - ref[nm][core]))) for nm in FIELD_GROUPS[g])
+            assert num / sc[g] <= TOL, (lo, g, num / sc[g])
+
+
+def test_config5_full_size_windows_and_invariants():
+    """768^3 (the bench workload): oracle windows on the magnetic interface (k = 384) and on the
+    lower PEC wall, then whole-grid properties."""
+    _need_gb(165)
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(5, device="cuda:0")
+    nx, ny, nz = w.nx, w.ny, w.nz
+    sim = from_workload(w)
+    Ms = 8e5
+
+    def slab(nm, k0, k1):
+        t = sim.read_fields(names=(nm,), device="cuda:0")[nm]
+        s = t[k0:k1].clone()
+        del t
+        return s
+
+    def div_b(k0, k1):
+        """discrete div(H + M_normal) of the cells k0..k1-1 (periodic x, y): needs planes k0..k1"""
+        bx = slab("Hx", k0, k1) + slab("Mxx", k0, k1)
+        d = (torch.roll(bx, -1, 2) - bx) / w.dx
+        del bx
+        by = slab("Hy", k0, k1) + slab("Myy", k0, k1)
+        d += (torch.roll(by, -1, 1) - by) / w.dy
+        del by
+        bz = slab("Hz", k0, k1 + 1) + slab("Mzz", k0, k1 + 1)
+        d += (bz[1:] - bz[:-1]) / w.dz
+        return d
+
+    K0, K1 = 370, 398          # straddles the interface at k = 384
+    div0 = div_b(K0, K1)
+    steps, R = 2, 3
+    sim.step(steps)
+    st = sim.stats()
+    assert st["steps"] == steps and st["nonconverged_halfsteps"] == 0
+    assert st["iters_max"] <= R and st["iters_total"] == 2 * steps * R, st
+    # ---- property: div(H + M) is unchanged by the step (eq. 21 adds a discrete curl only)
+    div1 = div_b(K0, K1)
+    assert float((div1 - div0).abs().max()) <= 1e-9 * Ms / w.dx
+    del div0, div1
+    # ---- property: |M| = Ms on faces inside the magnetic half, exactly 0 above the interface
+    for f in "xyz":
+        sq = sum(slab("M" + f + c, 1, 383) ** 2 for c in "xyz")
+        assert float((sq.sqrt() / Ms - 1.0).abs().max()) <= 1e-12, f
+        del sq
+        for c in "xyz":
+            assert float(slab("M" + f + c, 386, nz).abs().max()) == 0.0
+    # ---- sampled outputs: oracle windows
+    m = steps * (2 * R + 3)
+    n = (2 * m + 20, 2 * m + 20, 2 * m + 20)
+    for lo, zlow_is_wall in [((300, 420, 384 - n[2] // 2), False), ((nx - n[0], 5, 0), True)]:
+        ref, ost = _window_oracle(w, lo, n, steps, (0, 0, 0))
+        got = _gpu_window(sim, ALL, lo, n)
+        core = (slice(0 if zlow_is_wall else m, n[2] - m), slice(m, n[1] - m), slice(m, n[0] - m))
+        sc = _scales(ref, ("E", "H", "M"))
+        for g in ("E", "H", "M"):
+            num = max(float(np.max(np.abs(got[nm][core] - ref[nm][core]))) for nm in FIELD_GROUPS[g])
+            assert num / sc[g] <= TOL, (lo, g, num / sc[g])
