@@ -42,8 +42,12 @@ UNIT = "Gcell-updates/s"
 # read once and written once per sweep, stencil neighbours served on chip
 WORDS = {"h_update": 9,      # E 3 + H 3 read, H 3 written
          "hm_first": 27,     # E 3 + H^n 3 + M^n 9 read, M^1 9 + H^1 3 written
-         "hm_iter": 39,      # + H^{r-1} 3 + M^{r-1} 9 read
+         "hm_second": 39,    # + H^1 3 + M^1 9 read, M^2 9 + H^2 3 written
+         "hm_iter": 39,      # r >= 3: as r = 2
          "e_update": 9}      # E 3 + H 3 read, E 3 written
+# staged sweeps (kernel_path 0, 3): M^1 never goes to memory -- r = 1 writes H^1 only and r = 2
+# recomputes M^1 from M^n, H^n (hm_stage.cuh)
+WORDS_STAGED = dict(WORDS, hm_first=18, hm_second=30)
 
 
 def _parse():
@@ -251,13 +255,15 @@ def run_ours(args):
     extra = {"h_update": bool(mask & MAT_BITS["mu_r"]),
              "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
              "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
-    extra["hm_iter"] = extra["hm_first"]
+    extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
+    uniform_agm = not any(mask & MAT_BITS[m] for m in ("alpha", "gamma", "mu_r"))   # the staged sweeps' condition
+    words = WORDS_STAGED if (args.kernel_path in (0, 3) and st["magnetic_cells"] and uniform_agm) else WORDS
     per_class = {}
     for cls, (cms, cnt) in prof.items():
         if cnt == 0:
             continue
         ent = {"launches": cnt, "ms_total": cms, "us_per_launch": 1e3 * cms / cnt}
-        if cls in WORDS:
+        if cls in words:
             # cells one launch covers: the sweep box (LLG sweeps), the whole grid (E update), the
             # complement of the box split over its slabs (H update, 2 half-steps per step)
             if cls.startswith("hm_"):
@@ -266,13 +272,17 @@ def run_ours(args):
                 ncell = cells
             else:
                 ncell = (cells - box) * 2 * K / cnt
-            ent["alg_bytes_per_launch"] = 8.0 * (WORDS[cls] + extra[cls]) * ncell
+            ent["alg_bytes_per_launch"] = 8.0 * (words[cls] + extra[cls]) * ncell
             ent["alg_GBps"] = ent["alg_bytes_per_launch"] / (cms / cnt * 1e-3) * 1e-9
         per_class[cls] = ent
     timed = [c for c in per_class if "alg_GBps" in per_class[c]]
     dom = max(timed, key=lambda c: per_class[c]["ms_total"])
-    dom_kernel = {"h_update": "k_h_update", "hm_first": "k_hm_sweep<FIRST>",
-                  "hm_iter": "k_hm_sweep<ITER>", "e_update": "k_e_update"}[dom]
+    staged = words is WORDS_STAGED
+    dom_kernel = {"h_update": "k_h_update",
+                  "hm_first": "k_hm_stage<FIRST_H>" if staged else "k_hm_sweep<FIRST>",
+                  "hm_second": "k_hm_stage<ITER_RE>" if staged else "k_hm_sweep<ITER>",
+                  "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
+                  "e_update": "k_e_update"}[dom]
     achieved = per_class[dom]["alg_GBps"]
     step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
     roofline = {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak,

@@ -74,8 +74,8 @@ typedef struct {
   int kernel_path;    /* which LLG sweep kernel runs (same arithmetic in all: bitwise-equal results).
                          0 (default): staged sweep, tile 32x16 (TMA-fed shared-memory ring for the
                          neighbour operands) wherever it applies (alpha, gamma, mu_r uniform);
-                         1: direct-load kernels everywhere; 2: the all-TMA sweep, warp = (face,
-                         row); 3: staged sweep, tile 32x7, two blocks per SM.  1-3: A/B checks    */
+                         1: direct-load kernels everywhere; 3: staged sweep, tile 32x7, two blocks
+                         per SM.  1, 3: A/B checks                                               */
 } fdtd_llg_options;
 
 typedef struct {
@@ -101,11 +101,12 @@ typedef struct {
 enum {
   FDTD_LLG_K_H_UPDATE = 0,   /* Maxwell H half-step outside the LLG sweep box (eq. 21, M = 0)   */
   FDTD_LLG_K_HM_FIRST = 1,   /* LLG iterate r = 1 (eqs. 18-21)                                  */
-  FDTD_LLG_K_HM_ITER = 2,    /* LLG iterate r >= 2 that ran                                     */
+  FDTD_LLG_K_HM_ITER = 2,    /* LLG iterate r >= 3 that ran                                     */
   FDTD_LLG_K_HM_SKIPPED = 3, /* LLG iterate launched after convergence (exits on the flag)      */
   FDTD_LLG_K_E_UPDATE = 4,   /* eq. 11                                                          */
   FDTD_LLG_K_OTHER = 5,      /* source amplitudes, half-step bookkeeping, canonical-buffer copy */
-  FDTD_LLG_K_NCLASS = 6
+  FDTD_LLG_K_HM_SECOND = 6,  /* LLG iterate r = 2 that ran (the staged sweep recomputes M^1 there) */
+  FDTD_LLG_K_NCLASS = 7
 };
 
 /* Fill *opt with the defaults: PEC x3, LLG on, no bias, no anisotropy (axis z), tol 1e-6

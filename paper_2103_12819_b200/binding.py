@@ -50,7 +50,7 @@ EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_cre
            "fdtd_llg_read_fields",
            "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy")
 
-KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other")
+KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other", "hm_second")
 
 _VP = C.c_void_p
 _PP = C.POINTER(C.c_void_p)

@@ -15,7 +15,6 @@
 
 #include "../../include/fdtd_llg.h"
 #include "kernels.cuh"
-#include "hm_tma.cuh"
 #include "hm_stage.cuh"
 
 using namespace fl;
@@ -63,10 +62,6 @@ struct fdtd_llg {
   long long magnetic_cells = 0;
   int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
   BoxP box_llg{}, box_all{};
-  // TMA-fed sweeps (hm_tma.cuh): used when alpha, gamma, mu_r are uniform and opt.kernel_path == 0
-  bool tma_hm = false;
-  TileBox tile_llg{};
-  CUtensorMap mapH{}, mapE{}, mapS{}, mapM{};
   int n_arrays = 0;  // arrays in the workspace tensor (4th TMA coordinate)
   // staged sweeps (hm_stage.cuh): kernel_path 0 (tile rows 16) and 3 (tile rows 7)
   int stage_by = 0;  // 0 = not used
@@ -356,9 +351,8 @@ void make_boxes(fdtd_llg *s) {
 }
 
 
-// ---- TMA-fed sweeps -----------------------------------------------------------------------
+// ---- tensor maps for the staged sweeps -------------------------------------------------------
 
-constexpr int HM_BY = 8;  // tile rows of k_hm_tma
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
                                   const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
@@ -397,53 +391,6 @@ int make_map(fdtd_llg *s, CUtensorMap *m, int bx, int by, int ba) {
 
 int array_index(const fdtd_llg *s, const double *p) { return (int)((p - s->E[0]) / (ptrdiff_t)s->stride); }
 
-// TW x by columns marched over kz planes; kz as long as possible while leaving >= 16 items per SM
-TileBox make_tilebox(const fdtd_llg *s, const int lo[3], const int hi[3], int by) {
-  TileBox b{};
-  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
-  b.ntx = (hi[0] - lo[0] + TW - 1) / TW;
-  b.nty = (hi[1] - lo[1] + by - 1) / by;
-  const int ez = std::max(1, hi[2] - lo[2]);
-  int kz = ez;
-  while (kz > 16 && (long long)b.ntx * b.nty * ((ez + kz - 1) / kz) < 16LL * s->num_sms) kz = (kz + 1) / 2;
-  b.kz = kz;
-  b.items = b.ntx * b.nty * ((ez + kz - 1) / kz);
-  return b;
-}
-
-template <bool FIRST>
-int launch_hm_tma(fdtd_llg *s, const HMTArgs &p) {
-  const bool ms = s->Ms.is_array, an = s->opt.ani_hk != 0.0;
-  const int grid = std::max(1, std::min(p.tb.items, s->num_sms));
-#define TK(MS, AN)                                                                          \
-  if (ms == MS && an == AN) {                                                               \
-    using L = HmLayout<HM_BY, FIRST, MS>;                                                   \
-    k_hm_tma<HM_BY, FIRST, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);     \
-    return FDTD_LLG_OK;                                                                     \
-  }
-  TK(false, false) TK(false, true) TK(true, false) TK(true, true)
-#undef TK
-  return FDTD_LLG_OK;
-}
-
-// opt in to > 48 KB of dynamic shared memory for every instantiation
-int setup_hm_tma(fdtd_llg *s) {
-#define TA(FIRST, MS, AN)                                                                   \
-  CU(s, cudaFuncSetAttribute(k_hm_tma<HM_BY, FIRST, MS, AN>,                                \
-                             cudaFuncAttributeMaxDynamicSharedMemorySize,                   \
-                             (int)HmLayout<HM_BY, FIRST, MS>::SMEM_BYTES));
-  TA(true, false, false) TA(true, false, true) TA(true, true, false) TA(true, true, true)
-  TA(false, false, false) TA(false, false, true) TA(false, true, false) TA(false, true, true)
-#undef TA
-  int rc;
-  if ((rc = make_map(s, &s->mapH, HW, HM_BY + 2, 3))) return rc;
-  if ((rc = make_map(s, &s->mapE, EW, HM_BY + 1, 3))) return rc;
-  if ((rc = make_map(s, &s->mapS, HW, HM_BY + 1, 1))) return rc;
-  if ((rc = make_map(s, &s->mapM, TW, HM_BY, 9))) return rc;
-  s->tile_llg = make_tilebox(s, s->lo, s->hi, HM_BY);
-  return FDTD_LLG_OK;
-}
-
 // ---- staged sweeps (hm_stage.cuh) ----------------------------------------------------------
 
 // SW x by columns marched over kz planes; a persistent grid of `grid` blocks draws the items
@@ -463,33 +410,34 @@ StBox make_stbox(const int lo[3], const int hi[3], int by, int grid) {
   return b;
 }
 
-template <int BY, bool FIRST>
+template <int BY, int MODE>
 int launch_hm_stage_by(fdtd_llg *s, const HMSArgs &p) {
   const bool ms = s->Ms.is_array, an = s->opt.ani_hk != 0.0;
-  const int grid = std::max(1, std::min(p.tb.items, s->num_sms * StLayout<BY, FIRST, true>::BPS));
+  const int grid = std::max(1, std::min(p.tb.items, s->num_sms * StLayout<BY, st_first(MODE), true>::BPS));
 #define SK(MS, AN)                                                                          \
   if (ms == MS && an == AN) {                                                               \
-    using L = StLayout<BY, FIRST, MS>;                                                      \
-    k_hm_stage<BY, FIRST, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);      \
+    using L = StLayout<BY, st_first(MODE), MS>;                                             \
+    k_hm_stage<BY, MODE, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);       \
     return FDTD_LLG_OK;                                                                     \
   }
   SK(false, false) SK(false, true) SK(true, false) SK(true, true)
 #undef SK
   return FDTD_LLG_OK;
 }
-template <bool FIRST>
+template <int MODE>
 int launch_hm_stage(fdtd_llg *s, const HMSArgs &p) {
-  return s->stage_by == 16 ? launch_hm_stage_by<16, FIRST>(s, p) : launch_hm_stage_by<7, FIRST>(s, p);
+  return s->stage_by == 16 ? launch_hm_stage_by<16, MODE>(s, p) : launch_hm_stage_by<7, MODE>(s, p);
 }
 
 template <int BY>
 int setup_hm_stage_by(fdtd_llg *s) {
-#define SA(FIRST, MS, AN)                                                                   \
-  CU(s, cudaFuncSetAttribute(k_hm_stage<BY, FIRST, MS, AN>,                                 \
+#define SA(MODE, MS, AN)                                                                    \
+  CU(s, cudaFuncSetAttribute(k_hm_stage<BY, MODE, MS, AN>,                                  \
                              cudaFuncAttributeMaxDynamicSharedMemorySize,                   \
-                             (int)StLayout<BY, FIRST, MS>::SMEM_BYTES));
-  SA(true, false, false) SA(true, false, true) SA(true, true, false) SA(true, true, true)
-  SA(false, false, false) SA(false, false, true) SA(false, true, false) SA(false, true, true)
+                             (int)StLayout<BY, st_first(MODE), MS>::SMEM_BYTES));
+#define SA4(MODE) SA(MODE, false, false) SA(MODE, false, true) SA(MODE, true, false) SA(MODE, true, true)
+  SA4(ST_FIRST) SA4(ST_ITER) SA4(ST_FIRST_H) SA4(ST_ITER_RE)
+#undef SA4
 #undef SA
   int rc;
   if ((rc = make_map(s, &s->mapT, SROW, BY + 1, 1))) return rc;
@@ -549,7 +497,7 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
     a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
-    if ((s->tma_hm || s->stage_by) && s->Ms.is_array) {  // the most common face value and its reciprocal
+    if (s->stage_by && s->Ms.is_array) {  // the most common face value and its reciprocal
       a.Ms_u = s->Ms.maxv;
       a.rMs_u = 1.0 / s->Ms.maxv;
     }
@@ -579,16 +527,28 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
         p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
         p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
         p.work = s->work + r;
-        rc = (r == 1) ? launch_hm_stage<true>(s, p) : launch_hm_stage<false>(s, p);
-      } else if (s->tma_hm) {
-        HMTArgs p{};
-        p.a = a;
-        p.tb = s->tile_llg;
-        p.mapH = s->mapH; p.mapE = s->mapE; p.mapS = s->mapS; p.mapM = s->mapM;
-        p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
-        p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
-        p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
-        rc = (r == 1) ? launch_hm_tma<true>(s, p) : launch_hm_tma<false>(s, p);
+        p.cond = r > 1;
+        // With >= 2 iterations allowed, M^1 never goes to memory: r = 1 stores H^1 only and r = 2
+        // recomputes M^1 from the operands it reads anyway (18 words/cell less traffic).  Should
+        // iterate 1 already pass the stopping test, M^1 IS the result: the full r = 1 sweep then
+        // runs after all (cond 2; otherwise it exits on its first flag read).
+        const bool lean = s->opt.llg_max_iter >= 2;
+        if (r == 1 && lean) {
+          rc = launch_hm_stage<ST_FIRST_H>(s, p);
+          prof_end(s);
+          if (rc) return rc;
+          ++*launches;
+          prof_begin(s, FDTD_LLG_K_HM_ITER, s->opt.llg_max_iter + 1);  // counted as skipped unless it ran
+          p.work = s->work;
+          p.cond = 2;
+          rc = launch_hm_stage<ST_FIRST>(s, p);
+        } else if (r == 1) {
+          rc = launch_hm_stage<ST_FIRST>(s, p);
+        } else if (r == 2) {
+          rc = launch_hm_stage<ST_ITER_RE>(s, p);
+        } else {
+          rc = launch_hm_stage<ST_ITER>(s, p);
+        }
       } else {
         rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
       }
@@ -809,8 +769,6 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   make_boxes(s);
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
   const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
-  s->tma_hm = smem_ok && opt->kernel_path == 2;
-  if (s->tma_hm && (rc = setup_hm_tma(s))) return bail(rc);
   s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
   if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
   if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
@@ -976,6 +934,7 @@ int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *laun
     int cls = p.cls;
     // an LLG iterate beyond the half-step's iteration count exited on its first flag read
     if (cls == FDTD_LLG_K_HM_ITER && p.r > hist[(h0.halfsteps + p.half) % R_HIST]) cls = FDTD_LLG_K_HM_SKIPPED;
+    else if (cls == FDTD_LLG_K_HM_ITER && p.r == 2) cls = FDTD_LLG_K_HM_SECOND;
     ms_by_class[cls] += ms;
     launches_by_class[cls]++;
     cudaEventDestroy(p.a);

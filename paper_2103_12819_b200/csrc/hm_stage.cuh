@@ -33,6 +33,15 @@ struct StBox {
   int ntx, nty, kz, items;
 };
 
+// what one launch of the staged sweep does
+enum StMode {
+  ST_FIRST = 0,    // r = 1, stores M^1 and H^1
+  ST_ITER = 1,     // r >= 2, reads M^{r-1}, H^{r-1}, stores M^r, H^r
+  ST_FIRST_H = 2,  // r = 1, stores H^1 only: the r = 2 sweep recomputes M^1 (9 words less written)
+  ST_ITER_RE = 3   // r = 2 after ST_FIRST_H: M^1 recomputed from M^n, H^n (9 words less read)
+};
+__host__ __device__ constexpr bool st_first(int mode) { return mode == ST_FIRST || mode == ST_FIRST_H; }
+
 template <int BY, bool FIRST, bool MS_ARR>
 struct StLayout {
   static constexpr int ROWS = BY + 1;
@@ -64,7 +73,9 @@ struct HMSArgs {
   CUtensorMap mapT;  // box (SROW, BY+1, 1, 1) of the workspace tensor
   CUtensorMap mapM;  // box (SW, BY, 1, 9): L2 prefetch of an M set's plane
   int aE, aHn, aHp, aMn, aMp, aMs;  // array indices (4th tensor coordinate)
-  unsigned *work;  // item counter of this iterate (zero at launch; k_half_end re-arms it)
+  unsigned *work;  // item counter of this launch (zero at launch; k_half_end re-arms it)
+  int cond;        // 0: always run; 1: run iff iterate r-1 was not converged; 2: run iff iterate 1
+                   // WAS converged (the full r = 1 sweep after ST_FIRST_H, when M^1 is the result)
 };
 
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int c0, int c1, int c2, int c3) {
@@ -157,7 +168,7 @@ __device__ __forceinline__ double s_curl(const GridP &g, const double *A, const 
 }
 
 // One Jacobi iterate on the D-face of this thread's cell, neighbour operands from the ring
-template <class L, int D, bool FIRST, bool MS_ARR, bool ANISO>
+template <class L, int D, bool FIRST, bool MS_ARR, bool ANISO, bool RECOMP>
 __device__ __forceinline__ FaceOut s_face(const HMArgs &a, const double *A, const double *B, int t,
                                           const Vec3 &mn, const Vec3 &mp, bool wall) {
   double Msf = a.Ms_u, rMs = a.rMs_u;
@@ -171,14 +182,14 @@ __device__ __forceinline__ FaceOut s_face(const HMArgs &a, const double *A, cons
   Vec3 he = hn;
   if (!FIRST) he = s_hem<L, L::HP, D>(A, B, t);
   const double C = s_curl<L, D>(a.g, A, B, t);
-  return hm_face_core<D, FIRST, ANISO>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.gamma_u,
-                                       a.ch_uniform, wall);
+  return hm_face_core<D, FIRST, ANISO, RECOMP>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.gamma_u,
+                                               a.ch_uniform, wall);
 }
 
-template <int D, bool FIRST>
+template <int D, bool LOAD_MP>
 __device__ __forceinline__ void s_load_m(const HMArgs &a, int c, Vec3 &mn, Vec3 &mp) {
   mn = {__ldcs(a.Mn[3 * D + 0] + c), __ldcs(a.Mn[3 * D + 1] + c), __ldcs(a.Mn[3 * D + 2] + c)};
-  if (!FIRST)
+  if (LOAD_MP)
     mp = {__ldcs(a.Mr[3 * D + 0] + c), __ldcs(a.Mr[3 * D + 1] + c), __ldcs(a.Mr[3 * D + 2] + c)};
 }
 
@@ -220,18 +231,23 @@ __device__ __forceinline__ StItem st_decode(const StBox &T, int it, int by) {
 // Work items are handed out dynamically (one atomic per item on p.work): SMs do not all stream at
 // the same rate, and a static split leaves the fast ones idle at the end.  The producer publishes
 // the item of every stage in meta[slot] before arming the stage's barrier; item < 0 ends the march.
-template <int BY, bool FIRST, bool MS_ARR, bool ANISO>
+template <int BY, int MODE, bool MS_ARR, bool ANISO>
 __global__ void __maxnreg__(st_maxreg(BY))
 k_hm_stage(const __grid_constant__ HMSArgs p) {
+  constexpr bool FIRST = st_first(MODE);        // no H^{r-1} set, H_eff^{r-1} = H_eff^n
+  constexpr bool LOAD_MP = MODE == ST_ITER;     // M^{r-1} read from memory
+  constexpr bool RECOMP = MODE == ST_ITER_RE;   // M^1 recomputed
+  constexpr bool STORE_M = MODE != ST_FIRST_H;
   using L = StLayout<BY, FIRST, MS_ARR>;
   const HMArgs &a = p.a;
-  // the whole grid takes the same decision: iterate r runs iff iterate r-1 was not converged
-  if (!FIRST) {
-    if (__longlong_as_double((long long)a.resid[a.r - 1]) < a.tol) return;
-  }
-  extern __shared__ unsigned char smem_raw[];
-  double *const ring =
-      reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+  // the whole grid takes the same decision (the stopping test is global)
+  if (p.cond == 1 && __longlong_as_double((long long)a.resid[a.r - 1]) < a.tol) return;
+  if (p.cond == 2 && !(__longlong_as_double((long long)a.resid[1]) < a.tol)) return;
+  // dynamic shared memory starts on a 1 KB boundary of the CTA's window (no static shared memory in
+  // this kernel); keeping the pointer a plain offset of the __shared__ array lets the compiler
+  // address the ring with LDS instead of generic loads
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double *const ring = reinterpret_cast<double *>(smem_raw);
   uint64_t *const full = reinterpret_cast<uint64_t *>(ring + L::NS * L::STAGE);
   uint64_t *const empty = full + L::NS;
   double *const wmax = reinterpret_cast<double *>(empty + L::NS);
@@ -258,7 +274,7 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
         const StItem w = st_decode(T, end ? 0 : it, BY);
         if (!end) {  // the first M plane of a fresh column, towards L2
           tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMn);
-          if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMp);
+          if (LOAD_MP) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMp);
         }
         for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1); ++pz, ++n) {
           const unsigned s = n % L::NS, u = n / L::NS;
@@ -274,7 +290,7 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
           // (about one plane time ahead: long enough to cover HBM latency, short enough to survive in L2)
           if (pz >= w.k0) {
             tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + 1, p.aMn);
-            if (!FIRST) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + 1, p.aMp);
+            if (LOAD_MP) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, pz + 1, p.aMp);
           }
         }
         if (end) break;
@@ -297,9 +313,9 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
       // plane k+1 are issued as soon as the face of plane k has consumed its registers
       Vec3 mn0{}, mp0{}, mn1{}, mp1{}, mn2{}, mp2{};
       if (valid) {
-        s_load_m<0, FIRST>(a, c, mn0, mp0);
-        s_load_m<1, FIRST>(a, c, mn1, mp1);
-        s_load_m<2, FIRST>(a, c, mn2, mp2);
+        s_load_m<0, LOAD_MP>(a, c, mn0, mp0);
+        s_load_m<1, LOAD_MP>(a, c, mn1, mp1);
+        s_load_m<2, LOAD_MP>(a, c, mn2, mp2);
       }
       for (int k = w.k0; k < w.k1; ++k, c += a.g.sz, ++n) {
         const double *A = ring + (n % L::NS) * L::STAGE;
@@ -309,23 +325,26 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
           const bool edge = col.edge_ij || edge_k(a.g, k);
           const bool more = k + 1 < w.k1;
           {
-            const FaceOut o = s_face<L, 0, FIRST, MS_ARR, ANISO>(a, A, B, t, mn0, FIRST ? mn0 : mp0, col.wall[0]);
-            if (more) s_load_m<0, FIRST>(a, c + a.g.sz, mn0, mp0);
-            store_face<0>(a, c, o);
+            const FaceOut o = s_face<L, 0, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn0, LOAD_MP ? mp0 : mn0, col.wall[0]);
+            if (more) s_load_m<0, LOAD_MP>(a, c + a.g.sz, mn0, mp0);
+            if (STORE_M) store_face<0>(a, c, o);
+            else a.Hc[0][c] = o.h;
             if (edge) store_face_images<0>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }
           {
-            const FaceOut o = s_face<L, 1, FIRST, MS_ARR, ANISO>(a, A, B, t, mn1, FIRST ? mn1 : mp1, col.wall[1]);
-            if (more) s_load_m<1, FIRST>(a, c + a.g.sz, mn1, mp1);
-            store_face<1>(a, c, o);
+            const FaceOut o = s_face<L, 1, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn1, LOAD_MP ? mp1 : mn1, col.wall[1]);
+            if (more) s_load_m<1, LOAD_MP>(a, c + a.g.sz, mn1, mp1);
+            if (STORE_M) store_face<1>(a, c, o);
+            else a.Hc[1][c] = o.h;
             if (edge) store_face_images<1>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }
           {
-            const FaceOut o = s_face<L, 2, FIRST, MS_ARR, ANISO>(a, A, B, t, mn2, FIRST ? mn2 : mp2, wall_k(a.g, k));
-            if (more) s_load_m<2, FIRST>(a, c + a.g.sz, mn2, mp2);
-            store_face<2>(a, c, o);
+            const FaceOut o = s_face<L, 2, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn2, LOAD_MP ? mp2 : mn2, wall_k(a.g, k));
+            if (more) s_load_m<2, LOAD_MP>(a, c + a.g.sz, mn2, mp2);
+            if (STORE_M) store_face<2>(a, c, o);
+            else a.Hc[2][c] = o.h;
             if (edge) store_face_images<2>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }

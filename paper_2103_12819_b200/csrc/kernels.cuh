@@ -327,11 +327,13 @@ struct FaceOut {
 //   four-point averages), C = (curl E)_D, Msf / rMs = face Ms and its reciprocal (0 if Msf = 0),
 //   alf, gam = face alpha, |gamma|, ch = dt / (2 mu) of a non-magnetic face.
 // The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces).
-template <int D, bool FIRST, bool ANISO>
+// RECOMP (an iterate r = 2 only): M^1 is not read but recomputed from M^n and H_eff^n -- the very
+// expression the r = 1 sweep evaluated, so the value is the one it would have stored.
+template <int D, bool FIRST, bool ANISO, bool RECOMP = false>
 __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn, const Vec3 &mp_in,
                                                 Vec3 hn, Vec3 he, double C, double Msf, double rMs,
                                                 double alf, double gam, double ch, bool wall) {
-  const Vec3 mp = FIRST ? mn : mp_in;
+  Vec3 mp = FIRST ? mn : mp_in;
   const double hn_own = comp<D>(hn), hp_own = comp<D>(he);
 
   // ---- magnetic face: eqs. 18-21
@@ -344,6 +346,10 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
   if (ANISO) {
     const double p = a.hk * (dot(mn, u) * rMs);
     hn.x += p * u.x; hn.y += p * u.y; hn.z += p * u.z;
+  }
+  if (RECOMP) {
+    const Vec3 d1 = llg_increment<true>(mn, hn, hn, cf, alf * rMs, rMs);
+    mp = {mn.x + d1.x, mn.y + d1.y, mn.z + d1.z};
   }
   // H_eff^{r-1}, lagged; at r = 1 it is H_eff^n
   if (FIRST) {
@@ -488,6 +494,7 @@ __global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *wo
     st->resid_last = res;
     st->last_R_even = ((R & 1) == 0);
     for (int r = 1; r <= max_iter; ++r) { resid[r] = 0ull; work[r] = 0u; }
+    work[0] = 0u;
   } else {
     st->iters_last = 0;
     st->last_R_even = 0;
