@@ -45,9 +45,9 @@ WORDS = {"h_update": 9,      # E 3 + H 3 read, H 3 written
          "hm_second": 39,    # + H^1 3 + M^1 9 read, M^2 9 + H^2 3 written
          "hm_iter": 39,      # r >= 3: as r = 2
          "e_update": 9}      # E 3 + H 3 read, E 3 written
-# staged sweeps (kernel_path 0, 3): M^1 never goes to memory -- r = 1 writes H^1 only and r = 2
-# recomputes M^1 from M^n, H^n (hm_stage.cuh)
-WORDS_STAGED = dict(WORDS, hm_first=18, hm_second=30)
+# kernel_path 4: M^1 never goes to memory -- r = 1 writes H^1 only and r = 2 recomputes M^1 from
+# M^n, H^n (hm_stage.cuh)
+WORDS_LEAN = dict(WORDS, hm_first=18, hm_second=30)
 
 
 def _parse():
@@ -63,7 +63,8 @@ def _parse():
     ap.add_argument("--cpu-sample-shape", default="128,128,128")
     ap.add_argument("--cpu-sample-steps", type=int, default=30)
     ap.add_argument("--kernel-path", type=int, default=0,
-                    help="fdtd_llg_options.kernel_path: 0 = default kernels, 1 = direct-load kernels (A/B)")
+                    help="fdtd_llg_options.kernel_path: 0 = staged sweeps (default), 1 = direct-load kernels, "
+                         "3 = staged 32x7 tiles, 4 = staged + M^1 recomputed (fewer bytes, more flops)")
     return ap.parse_args()
 
 
@@ -257,7 +258,11 @@ def run_ours(args):
              "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
     extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
     uniform_agm = not any(mask & MAT_BITS[m] for m in ("alpha", "gamma", "mu_r"))   # the staged sweeps' condition
-    words = WORDS_STAGED if (args.kernel_path in (0, 3) and st["magnetic_cells"] and uniform_agm) else WORDS
+    words = WORDS_LEAN if (args.kernel_path == 4 and st["magnetic_cells"] and uniform_agm) else WORDS
+    if words is WORDS and "hm_second" in prof:   # r = 2 and r >= 3 are the same kernel: one class
+        prof = dict(prof)
+        a2, b2 = prof.pop("hm_second"), prof["hm_iter"]
+        prof["hm_iter"] = (a2[0] + b2[0], a2[1] + b2[1])
     per_class = {}
     for cls, (cms, cnt) in prof.items():
         if cnt == 0:
@@ -277,10 +282,11 @@ def run_ours(args):
         per_class[cls] = ent
     timed = [c for c in per_class if "alg_GBps" in per_class[c]]
     dom = max(timed, key=lambda c: per_class[c]["ms_total"])
-    staged = words is WORDS_STAGED
+    lean = words is WORDS_LEAN
+    staged = args.kernel_path in (0, 3, 4) and st["magnetic_cells"] and uniform_agm
     dom_kernel = {"h_update": "k_h_update",
-                  "hm_first": "k_hm_stage<FIRST_H>" if staged else "k_hm_sweep<FIRST>",
-                  "hm_second": "k_hm_stage<ITER_RE>" if staged else "k_hm_sweep<ITER>",
+                  "hm_first": "k_hm_stage<FIRST_H>" if lean else "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
+                  "hm_second": "k_hm_stage<ITER_RE>" if lean else "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
                   "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
                   "e_update": "k_e_update"}[dom]
     achieved = per_class[dom]["alg_GBps"]

@@ -75,7 +75,8 @@ typedef struct {
                          0 (default): staged sweep, tile 32x16 (TMA-fed shared-memory ring for the
                          neighbour operands) wherever it applies (alpha, gamma, mu_r uniform);
                          1: direct-load kernels everywhere; 3: staged sweep, tile 32x7, two blocks
-                         per SM.  1, 3: A/B checks                                               */
+                         per SM; 4: staged sweep that never writes M^1 (r = 1 stores H^1 only, r = 2
+                         recomputes M^1: 18 words/cell less traffic, one more LLG evaluation)     */
 } fdtd_llg_options;
 
 typedef struct {

@@ -63,8 +63,9 @@ struct fdtd_llg {
   int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
   BoxP box_llg{}, box_all{};
   int n_arrays = 0;  // arrays in the workspace tensor (4th TMA coordinate)
-  // staged sweeps (hm_stage.cuh): kernel_path 0 (tile rows 16) and 3 (tile rows 7)
+  // staged sweeps (hm_stage.cuh): kernel_path 0, 4 (tile rows 16) and 3 (tile rows 7)
   int stage_by = 0;  // 0 = not used
+  bool stage_lean = false;  // kernel_path 4: M^1 recomputed at r = 2 instead of stored at r = 1
   StBox st_box{};
   CUtensorMap mapT{}, mapPM{};
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
@@ -528,11 +529,11 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
         p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
         p.work = s->work + r;
         p.cond = r > 1;
-        // With >= 2 iterations allowed, M^1 never goes to memory: r = 1 stores H^1 only and r = 2
+        // kernel_path 4: M^1 never goes to memory: r = 1 stores H^1 only and r = 2
         // recomputes M^1 from the operands it reads anyway (18 words/cell less traffic).  Should
         // iterate 1 already pass the stopping test, M^1 IS the result: the full r = 1 sweep then
         // runs after all (cond 2; otherwise it exits on its first flag read).
-        const bool lean = s->opt.llg_max_iter >= 2;
+        const bool lean = s->stage_lean && s->opt.llg_max_iter >= 2;
         if (r == 1 && lean) {
           rc = launch_hm_stage<ST_FIRST_H>(s, p);
           prof_end(s);
@@ -544,7 +545,7 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
           rc = launch_hm_stage<ST_FIRST>(s, p);
         } else if (r == 1) {
           rc = launch_hm_stage<ST_FIRST>(s, p);
-        } else if (r == 2) {
+        } else if (r == 2 && lean) {
           rc = launch_hm_stage<ST_ITER_RE>(s, p);
         } else {
           rc = launch_hm_stage<ST_ITER>(s, p);
@@ -769,7 +770,8 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   make_boxes(s);
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
   const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
-  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
+  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 || opt->kernel_path == 4 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
+  s->stage_lean = opt->kernel_path == 4;
   if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
   if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
   CUB(cudaStreamSynchronize(s->stream));

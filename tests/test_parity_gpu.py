@@ -113,14 +113,15 @@ def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
 @pytest.mark.parametrize("cfg,shape", [(1, (32, 32, 32)), (4, (44, 36, 40)), (5, (40, 44, 36)),
                                        (5, (70, 19, 23)), (4, (33, 8, 50))])
 def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
-    """kernel_path 0 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell; M^1 recomputed
-    at r = 2 instead of stored) and 1 (direct global loads) share the arithmetic (hm_face_core):
+    """kernel_path 0 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell), 4 (the same
+    with M^1 recomputed at r = 2 instead of stored) and 1 (direct global loads) share the
+    arithmetic (hm_face_core):
     every field and the iteration counts agree bit for bit, on shapes with ragged tiles in x and
     y and several z chunks."""
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(cfg, shape=shape)
     outs, stats = [], []
-    for path in (1, 0, 3):
+    for path in (1, 0, 3, 4):
         sim = from_workload(w, kernel_path=path)
         sim.step(25)
         outs.append(_gpu_fields(sim))
