@@ -83,7 +83,7 @@ class Oracle:
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, *, eps_r=None, sigma=None, mu_r=None,
                  Ms=None, alpha=None, gamma=None, bc=(0, 0, 0), enable_llg=True,
                  h_bias=(0.0, 0.0, 0.0), ani_hk=0.0, ani_axis=(0.0, 0.0, 1.0),
-                 llg_tol=1e-12, llg_max_iter=20, kind="f64"):
+                 llg_tol=1e-12, llg_max_iter=20, kind="f64", time_scheme=0):
         self._lib, self._p = _lib(kind)
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
@@ -102,6 +102,12 @@ class Oracle:
         if not self._h:
             raise ValueError("oracle_create rejected its arguments")
         self._h = C.c_void_p(self._h)
+        if time_scheme:   # 1: the first-order scheme of PAPER.md:102-150
+            g = self._fn("set_scheme")
+            g.restype = C.c_int
+            g.argtypes = [C.c_void_p, C.c_int]
+            if g(self._h, int(time_scheme)):
+                raise ValueError("oracle_set_scheme rejected the scheme")
 
     def _fn(self, name):
         return getattr(self._lib, self._p + name)

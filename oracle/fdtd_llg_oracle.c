@@ -90,6 +90,7 @@ typedef struct {
   int enable_llg;
   REAL hbias[3], hk, axis[3], tol;
   int max_iter;
+  int scheme;          /* 0: second order, eqs. 15-21 (default); 1: first order, eqs. 6-9, 12-14 */
   size_t ncell;
   REAL *eps_r, *sigma, *mu_r, *Ms, *alpha, *gamma; /* cell centred */
   REAL *E[3], *H[3], *M[3][3];
@@ -476,6 +477,31 @@ static REAL llg_iterate(const REAL mn[3], const REAL hn[3], const REAL he[3], RE
 #endif
 }
 
+/* First-order scheme, Step 1 / Step 3: forward Euler on eq. 6,
+ *   M' = M + (dt/2) [ mu0 gamma_L (M x H_eff) + (alpha mu0 gamma_L / Ms) M x (M x H_eff) ],
+ * gamma_L = gamma / (1 + alpha^2), then N(M').  The paper prints the step of eqs. 7 and 12 as
+ * dt; both advance HALF a step (eqs. 8-9, 13-14 divide by dt/2), so dt/2 is used (DESIGN.md
+ * A22).  gamma < 0 for the electron: mu0 gamma_L = -mu0 |gamma| / (1 + alpha^2).
+ * Evaluated, like the second-order scheme, as an increment (A24).
+ *   out: mr = M' (renormalised), returns M_d - M'_d  (the term of eqs. 9, 14). */
+static REAL llg_euler(const REAL mn[3], const REAL hn[3], REAL gabs, REAL alpha_f, REAL Msf,
+                      REAL half_dt, int d, REAL mr[3]) {
+  REAL mxh[3], mxmxh[3], Delta[3], dM[3];
+  const REAL gl = MU0 * gabs / (1 + alpha_f * alpha_f); /* mu0 |gamma_L| */
+  cross(mn, hn, mxh);
+  cross(mn, mxh, mxmxh);
+  for (int q = 0; q < 3; ++q)
+    Delta[q] = half_dt * (-gl * mxh[q] - (alpha_f * gl / Msf) * mxmxh[q]);
+  REAL x = (2 * dot(mn, Delta) + dot(Delta, Delta)) / (Msf * Msf);
+  REAL sq = SQRT(1 + x);
+  REAL sm1 = -x / (sq * (1 + sq)); /* Ms/|M+Delta| - 1 */
+  for (int q = 0; q < 3; ++q) {
+    dM[q] = Delta[q] + sm1 * (mn[q] + Delta[q]);
+    mr[q] = mn[q] + dM[q];
+  }
+  return -dM[d];
+}
+
 /* (H,M) advanced over dt/2 with curl E fixed. */
 static void hm_half(oracle_t *o) {
   const int nx = o->n[0], ny = o->n[1], nz = o->n[2];
@@ -549,7 +575,9 @@ static void hm_half(oracle_t *o) {
             }
             h_eff(o, o->Hn, mn, Msf, d, c, hn);
             h_eff(o, o->Hp, mp, Msf, d, c, he);
-            REAL dMn = llg_iterate(mn, hn, he, cf, alpha_f, Msf, d, mr);
+            REAL dMn = o->scheme == 1
+                           ? llg_euler(mn, hn, face_mean_abs(o, o->gamma, d, c), alpha_f, Msf, half_dt, d, mr)
+                           : llg_iterate(mn, hn, he, cf, alpha_f, Msf, d, mr);
             /* eq. 21: H^r = H^n + M^n - M^r - (dt/2mu0) curl E, normal component */
             o->Hc[d][id] = o->Hn[d][id] + dMn - (half_dt / MU0) * o->C[d][id];
             for (int q = 0; q < 3; ++q) {
@@ -570,6 +598,7 @@ static void hm_half(oracle_t *o) {
             for (int q = 0; q < 3; ++q) o->Mp[d][q][id] = o->M[d][q][id];
           }
         }
+    if (o->scheme == 1) { delta = 0; break; } /* explicit: one sweep, no stopping test */
     if (delta < o->tol) break; /* PAPER.md:154 */
   }
   if (r > o->max_iter) {
@@ -592,6 +621,13 @@ int ORC(step)(void *h, int n) {
     hm_half(o);
     o->steps++;
   }
+  return 0;
+}
+
+/* 0: second-order scheme (default); 1: first-order scheme of PAPER.md:102-150 */
+int ORC(set_scheme)(void *h, int scheme) {
+  if (scheme != 0 && scheme != 1) return -1;
+  ((oracle_t *)h)->scheme = scheme;
   return 0;
 }
 

@@ -42,7 +42,7 @@ def shift(a, d, off, periodic):
 
 class BruteForce:
     def __init__(self, shape_xyz, d, dt, bc, eps_r, sigma, mu_r, Ms, alpha, gamma, enable_llg,
-                 h_bias, hk, axis, iters):
+                 h_bias, hk, axis, iters, scheme=0):
         self.n = shape_xyz
         self.d = [LD(v) for v in d]
         self.dt = LD(dt)
@@ -85,6 +85,9 @@ class BruteForce:
         self.hk = LD(hk)
         self.u = [LD(v) for v in axis]
         self.iters = iters
+        self.scheme = scheme   # 1: first-order scheme, eqs. 6-9, 12-14
+        # electron gyromagnetic ratio: negative; gamma_L = gamma / (1 + alpha^2)
+        self.gl_f = [-m2(np.abs(gamma), dd) / (1 + m2(alpha, dd) ** 2) for dd in range(3)]
         self.E = [np.zeros(self.shp, LD) for _ in range(3)]
         self.H = [np.zeros(self.shp, LD) for _ in range(3)]
         self.M = [[np.zeros(self.shp, LD) for _ in range(3)] for _ in range(3)]
@@ -163,6 +166,25 @@ class BruteForce:
             return
         cr = lambda a, b: [a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2],
                            a[0] * b[1] - a[1] * b[0]]
+        if self.scheme == 1:
+            # eq. 7 / 12 exactly as printed (with the half step dt/2), N(M), then eq. 9 / 14
+            Hcur, Mcur = [], []
+            for dd in range(3):
+                Msf = np.where(self.mag[dd], self.Ms_f[dd], 1)
+                hn = self.heff(Hn, Mn[dd], dd)
+                mxh = cr(Mn[dd], hn)
+                mxmxh = cr(Mn[dd], mxh)
+                g = MU0 * self.gl_f[dd]
+                m = [Mn[dd][q] + (self.dt / 2) * (g * mxh[q] + self.al_f[dd] * g / Msf * mxmxh[q])
+                     for q in range(3)]
+                nrm = np.sqrt(m[0] ** 2 + m[1] ** 2 + m[2] ** 2)
+                nrm = np.where(self.mag[dd], nrm, 1)
+                m = [np.where(self.mag[dd], m[q] * Msf / nrm, 0) for q in range(3)]
+                h = Hn[dd] + Mn[dd][dd] - m[dd] - (self.dt / 2 / MU0) * C[dd]
+                Hcur.append(np.where(self.mag[dd], h, Hnon[dd]))
+                Mcur.append(m)
+            self.H, self.M = Hcur, Mcur
+            return
         for _ in range(self.iters):
             Hcur, Mcur = [], []
             for dd in range(3):
