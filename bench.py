@@ -65,6 +65,8 @@ def _parse():
     ap.add_argument("--kernel-path", type=int, default=0,
                     help="fdtd_llg_options.kernel_path: 0 = staged sweeps (default), 1 = direct-load kernels, "
                          "3 = staged 32x7 tiles, 4 = staged + M^1 recomputed (fewer bytes, more flops)")
+    ap.add_argument("--time-scheme", type=int, default=0,
+                    help="0 = second-order scheme (the BASELINE metric), 1 = first-order scheme (PAPER.md:102-150)")
     return ap.parse_args()
 
 
@@ -119,14 +121,14 @@ class ClockSampler:
 
 # ------------------------------------------------------------------ the oracle legs
 
-def _oracle_rate(cfg, shape, steps, warmup=0):
+def _oracle_rate(cfg, shape, steps, warmup=0, time_scheme=0):
     """Cell-updates/s of the CPU oracle (as it stands) on a reduced-shape copy of the workload."""
     from oracle import Oracle  # noqa: F401  (the one place bench.py may execute oracle/)
     from oracle.cpu_oracle import omp_threads
     from paper_2103_12819_b200 import workloads as wl
     from tests._util import oracle_from_workload
     w = wl.make_config(cfg, shape=shape)
-    o = oracle_from_workload(w)
+    o = oracle_from_workload(w, time_scheme=time_scheme)
     if warmup:
         o.step(warmup)
     t0 = time.perf_counter()
@@ -142,7 +144,7 @@ def run_reference(args):
     shape = tuple(int(v) for v in args.cpu_sample_shape.split(","))
     from paper_2103_12819_b200 import workloads as wl
     full = wl.CONFIGS[args.config].__defaults__[0] if args.shape is None else _shape(args)
-    w, rate, dt, cores = _oracle_rate(args.config, shape, args.steps, args.warmup)
+    w, rate, dt, cores = _oracle_rate(args.config, shape, args.steps, args.warmup, args.time_scheme)
     sample = (f"config {args.config} structure at {shape[0]}x{shape[1]}x{shape[2]} cells, "
               f"{args.steps} steps after {args.warmup} warm-up (the full {full[0]}x{full[1]}x{full[2]} "
               f"grid is out of the oracle's reach; the rate per cell is what is compared)")
@@ -210,7 +212,7 @@ def run_ours(args):
     w = wl.make_config(args.config, shape=_shape(args), device=dev)
     cells = w.cells
     name = _workload_name(w)
-    sim = from_workload(w, device=dev, kernel_path=args.kernel_path)
+    sim = from_workload(w, device=dev, kernel_path=args.kernel_path, time_scheme=args.time_scheme)
     stream = sim.stream
 
     # host copies of the initial state for the end-to-end leg (pinned), before the device inputs go
@@ -335,7 +337,7 @@ def run_ours(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         shp = tuple(int(v) for v in args.cpu_sample_shape.split(","))
-        _, rate, dt, cores = _oracle_rate(args.config, shp, args.cpu_sample_steps)
+        _, rate, dt, cores = _oracle_rate(args.config, shp, args.cpu_sample_steps, time_scheme=args.time_scheme)
         cpu = {"value": rate * 1e-9, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"config {args.config} structure at {shp[0]}x{shp[1]}x{shp[2]}, "
                          f"{args.cpu_sample_steps} steps, {dt:.1f} s"}
@@ -349,7 +351,8 @@ def run_ours(args):
                            "parallelism": "replicas" if world > 1 else "single-gpu",
                            "l2": "state far larger than L2 (no flush needed)" if cells * 48 > 4e8
                                  else "state fits L2: latency-bound case, no roofline claim",
-                           "time_loop": "CUDA graph replay", "kernel_path": args.kernel_path},
+                           "time_loop": "CUDA graph replay", "kernel_path": args.kernel_path,
+                           "time_scheme": "first-order" if args.time_scheme else "second-order"},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
                 "gpu_launches": launches,
                 "context": "paper: 59x node-by-node GPU speedup (8x V100 vs 32-core Haswell, "

@@ -77,6 +77,10 @@ typedef struct {
                          1: direct-load kernels everywhere; 3: staged sweep, tile 32x7, two blocks
                          per SM; 4: staged sweep that never writes M^1 (r = 1 stores H^1 only, r = 2
                          recomputes M^1: 18 words/cell less traffic, one more LLG evaluation)     */
+  int time_scheme;    /* 0 (default): the second-order scheme, iterated trapezoidal LLG;
+                         1: the first-order scheme: one forward-Euler sweep of
+                         eq. 7 / 12 per (H,M) half-step (advancing dt/2), N(M), then eq. 9 / 14;
+                         llg_tol and llg_max_iter are not used                                   */
 } fdtd_llg_options;
 
 typedef struct {

@@ -189,6 +189,7 @@ int fill_ghosts(fdtd_llg *s, double *dev) {
 bool valid_opts(const fdtd_llg_options *o, const char **why) {
   for (int d = 0; d < 3; ++d)
     if (o->bc[d] != FDTD_LLG_PEC && o->bc[d] != FDTD_LLG_PERIODIC) { *why = "bc must be 0 (PEC) or 1 (periodic)"; return false; }
+  if (o->time_scheme != 0 && o->time_scheme != 1) { *why = "time_scheme must be 0 (second order) or 1 (first order)"; return false; }
   if (o->enable_llg) {
     if (!(o->llg_tol > 0) || !std::isfinite(o->llg_tol)) { *why = "llg_tol must be > 0"; return false; }
     if (o->llg_max_iter < 1 || o->llg_max_iter > 1000) { *why = "llg_max_iter must be in 1..1000"; return false; }
@@ -506,6 +507,7 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
     a.hk = s->opt.ani_hk;
     a.tol = s->opt.llg_tol;
+    a.euler = s->opt.time_scheme == 1;
     a.resid = s->resid;
     a.pipe_error = &s->dstate->pipe_error;
     for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
@@ -719,6 +721,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   }
   s->opt = *opt;
   if (!opt->enable_llg) { s->opt.llg_max_iter = 1; s->opt.llg_tol = 1.0; }
+  if (opt->time_scheme == 1) s->opt.llg_max_iter = 1;  // explicit: one sweep per half-step, no iteration
   s->stream = static_cast<cudaStream_t>(cuda_stream);
   if (!cuda_stream) s->opt.use_graph = 0;  // the legacy default stream cannot be captured
   s->ws = static_cast<char *>(dev_workspace);

@@ -237,6 +237,7 @@ struct HMArgs {
   double Ms_u, rMs_u, alpha_u, gamma_u, ch_uniform;
   double hb[3], hk, u[3];
   double tol;
+  int euler;  // 1: first-order scheme: the r = 1 sweep is a forward-Euler step
   unsigned long long *resid;  // [max_iter + 1] bit patterns of the residual of iterate r
   int *pipe_error;            // &DevState::pipe_error
   int r;
@@ -313,6 +314,21 @@ __device__ __forceinline__ Vec3 llg_increment(const Vec3 &mn, const Vec3 &hn, co
   return {De.x + sm1 * (mn.x + De.x), De.y + sm1 * (mn.y + De.y), De.z + sm1 * (mn.z + De.z)};
 }
 
+// First-order scheme, Step 1 / Step 3 (eqs. 7 and 12 advance half a step, A22):
+//   M' = M + (dt/2) [ mu0 gamma_L (M x H_eff) + (alpha mu0 gamma_L / Ms) M x (M x H_eff) ],
+// gamma_L = gamma / (1 + alpha^2) with the electron's negative gamma, then N(M') applied to the
+// increment as in llg_increment.  g2 = mu0 |gamma_L| dt / 2.  Returns dM = M' - M.
+__device__ __forceinline__ Vec3 llg_euler(const Vec3 &mn, const Vec3 &hn, double g2, double alf,
+                                          double rMs) {
+  const Vec3 p = cross(mn, hn);
+  const Vec3 q = cross(mn, p);
+  const double ar = alf * rMs;
+  const Vec3 De = {-g2 * (p.x + ar * q.x), -g2 * (p.y + ar * q.y), -g2 * (p.z + ar * q.z)};
+  const double x = (2.0 * dot(mn, De) + dot(De, De)) * (rMs * rMs);
+  const double sm1 = rsqrt_1p_m1(x);
+  return {De.x + sm1 * (mn.x + De.x), De.y + sm1 * (mn.y + De.y), De.z + sm1 * (mn.z + De.z)};
+}
+
 // result of one face: M^r, H^r (normal component), residual
 struct FaceOut {
   Vec3 m;
@@ -361,7 +377,11 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
       he.x += p * u.x; he.y += p * u.y; he.z += p * u.z;
     }
   }
-  const Vec3 dM = llg_increment<FIRST>(mn, hn, he, cf, alf * rMs, rMs);
+  Vec3 dM;
+  if (FIRST && !RECOMP && a.euler)
+    dM = llg_euler(mn, hn, 2.0 * cf / (1.0 + alf * alf), alf, rMs);
+  else
+    dM = llg_increment<FIRST>(mn, hn, he, cf, alf * rMs, rMs);
   const Vec3 mr = {mn.x + dM.x, mn.y + dM.y, mn.z + dM.z};
   // eq. 21, normal component:  H^r = H^n + M^n - M^r - (dt / 2 mu0) curl E
   const double h_mag = hn_own - comp<D>(dM) - (a.g.dt / (2.0 * kMu0)) * C;
@@ -374,7 +394,7 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
   FaceOut o;
   o.m = {magnetic ? mr.x : 0.0, magnetic ? mr.y : 0.0, magnetic ? mr.z : 0.0};
   o.h = magnetic ? h_mag : h_non;
-  o.res = magnetic ? e * rMs : 0.0;
+  o.res = (magnetic && !(FIRST && a.euler)) ? e * rMs : 0.0;  // an explicit sweep has no stopping test
   return o;
 }
 

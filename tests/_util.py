@@ -12,14 +12,15 @@ FIELD_GROUPS = {
 }
 
 
-def oracle_from_workload(w, kind="f64") -> Oracle:
+def oracle_from_workload(w, kind="f64", time_scheme=0) -> Oracle:
     a = w.numpy()
     m = a["materials"]
     o = Oracle(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt,
                eps_r=m.get("eps_r"), sigma=m.get("sigma"), mu_r=m.get("mu_r"),
                Ms=m.get("Ms"), alpha=m.get("alpha"), gamma=m.get("gamma"),
                bc=w.bc, enable_llg=w.enable_llg, h_bias=w.h_bias, ani_hk=w.ani_hk,
-               ani_axis=w.ani_axis, llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, kind=kind)
+               ani_axis=w.ani_axis, llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, kind=kind,
+               time_scheme=time_scheme)
     o.set_fields(a["E"], a["H"], a["M_cell"])
     for s in w.sources:
         prof = None if s.profile is None else s.profile.detach().cpu().numpy()

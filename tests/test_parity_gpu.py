@@ -132,6 +132,33 @@ def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
         assert stats[0]["iters_total"] == st["iters_total"] > 0
 
 
+@pytest.mark.parametrize("cfg", [1, 4, 5])
+def test_first_order_scheme_parity_100_steps(cfg):
+    """time_scheme = 1: one forward-Euler sweep per (H,M) half-step.  Same bar
+    as the second-order scheme; every kernel path agrees bit for bit."""
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
+    o = oracle_from_workload(w, time_scheme=1)
+    o.step(100)
+    ref = o.read_fields()
+    outs = []
+    for path in (0, 1, 3):
+        sim = from_workload(w, kernel_path=path, time_scheme=1)
+        sim.step(100)
+        outs.append(_gpu_fields(sim))
+        st = sim.stats()
+        assert st["iters_total"] == int(o.stats()["iters_total"]) == 200   # one sweep per half-step
+        assert st["nonconverged_halfsteps"] == 0
+    _assert_parity(outs[0], ref, True)
+    for other in outs[1:]:
+        for n in outs[0]:
+            assert np.array_equal(outs[0][n], other[n]), n
+    # and it is not the second-order result
+    o2 = oracle_from_workload(w)
+    o2.step(100)
+    assert rel_linf(o2.read_fields(), ref, "M") > 1e-9
+
+
 def test_device_resident_inputs_equal_host_inputs():
     from paper_2103_12819_b200.binding import from_workload
     wh = wl.make_config(5, shape=wl.SMALL_SHAPES[5])
