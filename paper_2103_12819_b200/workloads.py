@@ -302,6 +302,39 @@ def config5(shape=(768, 768, 768), device="cpu", steps=200, e_fields=True) -> Wo
     return w
 
 
+def paper_convergence_test(n: int, steps: int, device="cpu") -> Workload:
+    """The paper's own convergence test (eqs. 22-28), not a BASELINE config:
+    fully periodic cube of side L = 0.1 m centred at the origin on an n^3 grid, plane-wave-like
+    E, H (eqs. 22-23, sampled at the Yee locations), Gaussian bumps of sigma, eps, Ms, alpha,
+    gamma around the origin (eqs. 24-28, sampled at cell centres), M = (Ms, 0, 0), no bias,
+    CFL 0.9 on the vacuum speed of light, the paper's tolerance 1e-6."""
+    L = 0.1
+    h = L / n
+    w = Workload(f"paper_convergence_{n}", n, n, n, h, h, h, courant_dt(0.9, h, h, h),
+                 (PERIODIC, PERIODIC, PERIODIC), steps, enable_llg=True, llg_tol=1e-6,
+                 llg_max_iter=50)
+    idx = torch.arange(n, device=device, dtype=torch.float64)
+    cen = -L / 2 + (idx + 0.5) * h      # cell centres / face and edge mid-points
+    nod = -L / 2 + idx * h              # nodes
+    ax = lambda v, a: v.view([n if q == a else 1 for q in range(3)]).expand(n, n, n).contiguous()
+    # tensor axes: 0 = z, 1 = y, 2 = x
+    r2 = ax(cen, 0) ** 2 + ax(cen, 1) ** 2 + ax(cen, 2) ** 2
+    g = torch.exp(-1000.0 * r2)
+    w.materials = {"eps_r": 1.0 + g, "sigma": 0.1 * g, "Ms": 1e4 * (1.0 + g),
+                   "alpha": 0.5 * (1.0 + g), "gamma": -1.759e11 * (1.0 + g)}
+    k20 = 20.0 * math.pi
+    a0 = 1e6
+    w.E = [a0 * torch.cos(k20 * ax(nod, 0)),    # Ex(z) on the x-edge (i+1/2, j, k): z is a node
+           a0 * torch.cos(k20 * ax(nod, 2)),    # Ey(x) on (i, j+1/2, k)
+           a0 * torch.cos(k20 * ax(nod, 1))]    # Ez(y) on (i, j, k+1/2)
+    b0 = a0 / (120.0 * math.pi)
+    w.H = [b0 * torch.cos(k20 * ax(cen, 1)),    # Hx(y) on the x-face (i, j+1/2, k+1/2)
+           b0 * torch.cos(k20 * ax(cen, 0)),    # Hy(z) on (i+1/2, j, k+1/2)
+           b0 * torch.cos(k20 * ax(cen, 2))]    # Hz(x) on (i+1/2, j+1/2, k)
+    w.M_cell = [w.materials["Ms"].clone(), None, None]
+    return w
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 # shapes the oracle finishes in seconds: several tiles of the kernels plus a ragged tail

@@ -96,3 +96,26 @@ def test_full_size_configs_are_the_baseline_json_ones():
                       4: (384, 384, 384), 5: (768, 768, 768)}
     steps = {n: inspect.signature(f).parameters["steps"].default for n, f in wl.CONFIGS.items()}
     assert steps == {1: 100, 2: 1000, 3: 2000, 4: 2000, 5: 200}
+
+
+def test_paper_convergence_workload_samples_eqs_22_to_28():
+    """values at hand-computed points of a 16^3 grid (h = 0.1/16)."""
+    import math
+    w = wl.paper_convergence_test(16, 5)
+    h = 0.1 / 16
+    assert w.bc == (1, 1, 1) and w.llg_tol == 1e-6 and abs(w.dt - wl.courant_dt(0.9, h, h, h)) < 1e-30
+    # Ex(z) at the node z_k = -0.05 + k h, whatever i, j (array index [k, j, i])
+    assert abs(float(w.E[0][3, 5, 7]) - 1e6 * math.cos(20 * math.pi * (-0.05 + 3 * h))) < 1e-6
+    assert abs(float(w.E[1][3, 5, 7]) - 1e6 * math.cos(20 * math.pi * (-0.05 + 7 * h))) < 1e-6
+    # Hx(y) at the face centre y = -0.05 + (j + 1/2) h; E/H = 120 pi (PAPER.md:249)
+    hx = 1e6 / (120 * math.pi) * math.cos(20 * math.pi * (-0.05 + 5.5 * h))
+    assert abs(float(w.H[0][3, 5, 7]) - hx) < 1e-9
+    # material bumps at the cell centre nearest the origin: r^2 = 3 (h/2)^2
+    g = math.exp(-1000 * 3 * (h / 2) ** 2)
+    m = w.materials
+    assert abs(float(m["sigma"][8, 8, 8]) - 0.1 * g) < 1e-15
+    assert abs(float(m["eps_r"][8, 8, 8]) - (1 + g)) < 1e-15
+    assert abs(float(m["Ms"][7, 8, 7]) - 1e4 * (1 + g)) < 1e-9
+    assert abs(float(m["alpha"][8, 7, 7]) - 0.5 * (1 + g)) < 1e-15
+    assert abs(float(m["gamma"][8, 8, 8]) + 1.759e11 * (1 + g)) < 1e-3
+    assert w.M_cell[1] is None and float((w.M_cell[0] - m["Ms"]).abs().max()) == 0.0
