@@ -121,16 +121,17 @@ class Oracle:
         if rc:
             raise ValueError(f"oracle_set_fields failed ({rc})")
 
-    def set_source(self, comp, lo, hi, profile=None, amplitude=1.0, f0=0.0, t0=0.0, tp=1.0):
-        f = self._fn("set_source")
+    def set_source(self, comp, lo, hi, profile=None, amplitude=1.0, f0=0.0, t0=0.0, tp=1.0, kind=0):
+        """kind 0 soft E (J of eq. 11), 1 hard E, 2 soft H, 3 hard H (see the C file)."""
+        f = self._fn("add_source")
         f.restype = C.c_int
-        f.argtypes = [C.c_void_p, C.c_int, _IP, _IP, _DP] + [C.c_double] * 4
+        f.argtypes = [C.c_void_p, C.c_int, C.c_int, _IP, _IP, _DP] + [C.c_double] * 4
         nb = int(np.prod([h - l for l, h in zip(lo, hi)]))
         prof = _as_f64(profile, nb)
-        rc = f(self._h, int(comp), (C.c_int * 3)(*lo), (C.c_int * 3)(*hi), _dptr(prof),
+        rc = f(self._h, int(kind), int(comp), (C.c_int * 3)(*lo), (C.c_int * 3)(*hi), _dptr(prof),
                float(amplitude), float(f0), float(t0), float(tp))
         if rc:
-            raise ValueError(f"oracle_set_source failed ({rc})")
+            raise ValueError(f"oracle_add_source failed ({rc})")
 
     def step(self, n=1):
         f = self._fn("step")

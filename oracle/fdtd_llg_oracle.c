@@ -77,7 +77,8 @@ static const long double PI_LD = 3.14159265358979323846264338327950288L;
 #define EPS0 ((REAL)(1.0L / (4.0L * PI_LD * 1e-7L * 299792458.0L * 299792458.0L)))
 
 typedef struct {
-  int comp;            /* 0,1,2 = Jx,Jy,Jz */
+  int kind;            /* 0 soft E (J in eq. 11), 1 hard E, 2 soft H, 3 hard H */
+  int comp;            /* 0,1,2 = x,y,z component */
   int lo[3], hi[3];    /* edge-index box, lo inclusive, hi exclusive */
   REAL *profile;       /* box-sized, x fastest, or NULL = 1 */
   REAL amplitude, f0, t0, tp;
@@ -362,9 +363,19 @@ int ORC(set_fields)(void *h, const double *Ex, const double *Ey, const double *E
 /* Soft current source entering eq. 11:
  * J_comp(t) = amplitude * exp(-(t-t0)^2/(2 tp^2)) * cos(2 pi f0 t) * profile
  * on the box lo <= index < hi of comp-edges; envelope of eq. 31 (A15). */
-int ORC(set_source)(void *h, int comp, const int *lo, const int *hi, const double *profile,
-                    double amplitude, double f0, double t0, double tp) {
+/* External excitations: "soft sources [are defined] in terms of the time-rate of
+ * field change, and are applied at the beginning of the time step.  Hard sources are enforced
+ * directly for the corresponding fields after their updates at each time step."  The paper prints
+ * no formulas; the reading taken (A25), g(t) the envelope of eq. 31:
+ *   kind 0  soft E: the current J_src^{n+1/2} of eq. 11, t = (n+1/2) dt
+ *   kind 1  hard E: after the E update of step n, E_comp = A g((n+1) dt) profile on the box
+ *   kind 2  soft H: before the first (H,M) half-step of step n, H_comp += dt A g(n dt) profile
+ *   kind 3  hard H: after the second (H,M) half-step, H_comp = A g((n+1) dt) profile
+ * Wall-tangential E edges and wall faces of H stay 0; M is never touched. */
+int ORC(add_source)(void *h, int kind, int comp, const int *lo, const int *hi,
+                    const double *profile, double amplitude, double f0, double t0, double tp) {
   oracle_t *o = (oracle_t *)h;
+  if (kind < 0 || kind > 3) return -1;
   if (o->nsrc >= MAX_SOURCES || comp < 0 || comp > 2 || !(tp > 0)) return -1;
   source_t *s = &o->src[o->nsrc];
   size_t nb = 1;
@@ -374,6 +385,7 @@ int ORC(set_source)(void *h, int comp, const int *lo, const int *hi, const doubl
     s->hi[d] = hi[d];
     nb *= (size_t)(hi[d] - lo[d]);
   }
+  s->kind = kind;
   s->comp = comp;
   s->profile = profile ? alloc_fill(nb, profile, 0.0) : NULL;
   s->amplitude = (REAL)amplitude;
@@ -384,11 +396,16 @@ int ORC(set_source)(void *h, int comp, const int *lo, const int *hi, const doubl
   return 0;
 }
 
+int ORC(set_source)(void *h, int comp, const int *lo, const int *hi, const double *profile,
+                    double amplitude, double f0, double t0, double tp) {
+  return ORC(add_source)(h, 0, comp, lo, hi, profile, amplitude, f0, t0, tp);
+}
+
 static REAL source_at(const oracle_t *o, int comp, const int c[3], REAL t) {
   REAL J = 0;
   for (int s = 0; s < o->nsrc; ++s) {
     const source_t *S = &o->src[s];
-    if (S->comp != comp) continue;
+    if (S->kind != 0 || S->comp != comp) continue;
     int in = 1;
     for (int d = 0; d < 3; ++d) in = in && c[d] >= S->lo[d] && c[d] < S->hi[d];
     if (!in) continue;
@@ -613,12 +630,41 @@ static void hm_half(oracle_t *o) {
 }
 
 /* n time steps:  HM half (curl E^n) ; E update ; HM half (curl E^{n+1}) */
+/* sources of one kind applied to E (kinds 1) or H (kinds 2, 3) at time t */
+static void apply_field_sources(oracle_t *o, int kind, REAL t) {
+  for (int q = 0; q < o->nsrc; ++q) {
+    const source_t *S = &o->src[q];
+    if (S->kind != kind) continue;
+    REAL u = (t - S->t0) / S->tp;
+    REAL g = (REAL)expl((long double)(-(REAL)0.5 * u * u)) *
+             (REAL)cosl((long double)((REAL)2 * (REAL)PI_LD * S->f0 * t));
+    REAL *F = (kind == 1) ? o->E[S->comp] : o->H[S->comp];
+    size_t bx = (size_t)(S->hi[0] - S->lo[0]), by = (size_t)(S->hi[1] - S->lo[1]);
+    for (int k = S->lo[2]; k < S->hi[2]; ++k)
+      for (int j = S->lo[1]; j < S->hi[1]; ++j)
+        for (int i = S->lo[0]; i < S->hi[0]; ++i) {
+          int c[3] = {i, j, k};
+          if (kind == 1 ? wall_edge(o, S->comp, c) : wall_face(o, S->comp, c)) continue;
+          REAL p = S->profile ? S->profile[(size_t)(i - S->lo[0]) +
+                                           bx * ((size_t)(j - S->lo[1]) + by * (size_t)(k - S->lo[2]))]
+                              : 1;
+          REAL v = S->amplitude * g * p;
+          size_t id = cidx(o, i, j, k);
+          if (kind == 2) F[id] += o->dt * v;
+          else F[id] = v;
+        }
+  }
+}
+
 int ORC(step)(void *h, int n) {
   oracle_t *o = (oracle_t *)h;
   for (int s = 0; s < n; ++s) {
+    apply_field_sources(o, 2, (REAL)o->steps * o->dt);        /* soft H, beginning of the step */
     hm_half(o);
     e_update(o);
+    apply_field_sources(o, 1, (REAL)(o->steps + 1) * o->dt);  /* hard E, after its update     */
     hm_half(o);
+    apply_field_sources(o, 3, (REAL)(o->steps + 1) * o->dt);  /* hard H, after its update     */
     o->steps++;
   }
   return 0;

@@ -108,7 +108,7 @@ class BruteForce:
             for q in range(3):
                 self.M[dd][q] = np.where(self.mag[dd], m[q] * self.Ms_f[dd] / safe, 0)
 
-    def add_source(self, comp, lo, hi, profile, amplitude, f0, t0, tp):
+    def add_source(self, comp, lo, hi, profile, amplitude, f0, t0, tp, kind=0):
         mask = np.ones(self.shp, bool)
         for dd in range(3):
             mask &= (self.pos[dd] >= lo[dd]) & (self.pos[dd] < hi[dd])
@@ -118,7 +118,8 @@ class BruteForce:
         else:
             box = (hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0])
             prof[lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]] = np.asarray(profile, np.float64).reshape(box)
-        self.sources.append((comp, prof, LD(amplitude), LD(f0), LD(t0), LD(tp)))
+        # (kinds 1-3: hard E, soft H, hard H act on the field arrays themselves)
+        self.sources.append((comp, prof, LD(amplitude), LD(f0), LD(t0), LD(tp), kind, mask))
 
     # -- operators ---------------------------------------------------------------------
     def curl_faces(self, E):
@@ -212,18 +213,33 @@ class BruteForce:
         cH = self.curl_edges(self.H)
         for dd in range(3):
             J = np.zeros(self.shp, LD)
-            for comp, prof, A, f0, t0, tp in self.sources:
-                if comp == dd:
+            for comp, prof, A, f0, t0, tp, kind, _ in self.sources:
+                if comp == dd and kind == 0:
                     J = J + A * np.exp(-((t - t0) ** 2) / (2 * tp * tp)) * np.cos(2 * PI * f0 * t) * prof
             s, e = self.sig_e[dd], self.eps_e[dd]
             new = (cH[dd] - (s / 2 - e / self.dt) * self.E[dd] - J) / (s / 2 + e / self.dt)   # (11)
             self.E[dd] = np.where(self.edge_ok[dd], new, 0)
 
+    def field_sources(self, kind, t):
+        for comp, prof, A, f0, t0, tp, knd, mask in self.sources:
+            if knd != kind:
+                continue
+            v = A * np.exp(-((t - t0) ** 2) / (2 * tp * tp)) * np.cos(2 * PI * f0 * t) * prof
+            if kind == 1:
+                m = mask & self.edge_ok[comp]
+                self.E[comp] = np.where(m, v, self.E[comp])
+            else:
+                m = mask & self.face_ok[comp]
+                self.H[comp] = np.where(m, self.H[comp] + self.dt * v if kind == 2 else v, self.H[comp])
+
     def step(self, n=1):
         for _ in range(n):
+            self.field_sources(2, LD(self.steps) * self.dt)          # soft H: start of the step
             self.hm_half()
             self.e_update()
+            self.field_sources(1, LD(self.steps + 1) * self.dt)      # hard E: after its update
             self.hm_half()
+            self.field_sources(3, LD(self.steps + 1) * self.dt)      # hard H: after its update
             self.steps += 1
 
     def fields(self):
