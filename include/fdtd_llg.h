@@ -164,6 +164,22 @@ int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
                         const double *profile, int mem_space, double amplitude, double f0,
                         double t0, double tp);
 
+/* External excitations of both fields ("soft sources [are defined] in terms of the
+ * time-rate of field change, and are applied at the beginning of the time step.  Hard sources are
+ * enforced directly for the corresponding fields after their updates at each time step").  The
+ * paper prints no formulas; the reading taken (A25), g(t) the envelope above:
+ *   FDTD_LLG_SRC_SOFT_E  the current of fdtd_llg_set_source (A/m^2), t = (n+1/2) dt
+ *   FDTD_LLG_SRC_HARD_E  after the E update of step n:   E_comp  = amplitude g((n+1) dt) profile
+ *   FDTD_LLG_SRC_SOFT_H  before the first (H,M) half-step: H_comp += dt amplitude g(n dt) profile
+ *   FDTD_LLG_SRC_HARD_H  after the second (H,M) half-step: H_comp = amplitude g((n+1) dt) profile
+ * on the comp-edges (E) / comp-faces (H) of the box.  Wall-tangential E and wall-normal H stay 0;
+ * M is never touched.  The 8 sources of a handle are shared by all kinds.  Other arguments and
+ * errors as fdtd_llg_set_source (which is kind FDTD_LLG_SRC_SOFT_E). */
+enum { FDTD_LLG_SRC_SOFT_E = 0, FDTD_LLG_SRC_HARD_E = 1, FDTD_LLG_SRC_SOFT_H = 2, FDTD_LLG_SRC_HARD_H = 3 };
+int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const int *hi,
+                        const double *profile, int mem_space, double amplitude, double f0,
+                        double t0, double tp);
+
 /* Advance n >= 0 time steps.  Asynchronous: only enqueues work on the stream (n graph launches). */
 int fdtd_llg_step(fdtd_llg *s, int n);
 

@@ -47,7 +47,7 @@ class Stats(C.Structure):
 
 
 EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_create",
-           "fdtd_llg_set_fields", "fdtd_llg_set_source", "fdtd_llg_step", "fdtd_llg_step_timed",
+           "fdtd_llg_set_fields", "fdtd_llg_set_source", "fdtd_llg_add_source", "fdtd_llg_step", "fdtd_llg_step_timed",
            "fdtd_llg_read_fields",
            "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy")
 
@@ -85,6 +85,9 @@ def lib() -> C.CDLL:
         L.fdtd_llg_set_source.argtypes = [_VP, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int),
                                           _VP, C.c_int] + [C.c_double] * 4
         L.fdtd_llg_set_source.restype = C.c_int
+        L.fdtd_llg_add_source.argtypes = [_VP, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                          _VP, C.c_int] + [C.c_double] * 4
+        L.fdtd_llg_add_source.restype = C.c_int
         L.fdtd_llg_step.argtypes = [_VP, C.c_int]
         L.fdtd_llg_step.restype = C.c_int
         L.fdtd_llg_step_timed.argtypes = [_VP, C.c_int, C.POINTER(C.c_double),
@@ -234,7 +237,8 @@ class FdtdLlg:
                                            _ptr_array(M, 3), space)
         _check(rc, self._h)
 
-    def set_source(self, comp, lo, hi, profile=None, amplitude=1.0, f0=0.0, t0=0.0, tp=1.0):
+    def set_source(self, comp, lo, hi, profile=None, amplitude=1.0, f0=0.0, t0=0.0, tp=1.0, kind=0):
+        """kind: 0 soft E (the current of eq. 11), 1 hard E, 2 soft H, 3 hard H (fdtd_llg_add_source)."""
         prof = None
         if profile is not None:
             torch = self._torch
@@ -243,7 +247,7 @@ class FdtdLlg:
         space = DEVICE if (prof is not None and prof.is_cuda) else HOST
         self._sync_in()
         with self._torch.cuda.device(self.device):
-            rc = lib().fdtd_llg_set_source(self._h, int(comp), (C.c_int * 3)(*lo),
+            rc = lib().fdtd_llg_add_source(self._h, int(kind), int(comp), (C.c_int * 3)(*lo),
                                            (C.c_int * 3)(*hi), _ptr(prof), space,
                                            float(amplitude), float(f0), float(t0), float(tp))
         _check(rc, self._h)
@@ -317,5 +321,6 @@ def from_workload(w, device="cuda:0", use_graph=True, stream=None, fields_device
                   time_scheme=time_scheme)
     sim.set_fields(w.E, w.H, w.M_cell)
     for s in w.sources:
-        sim.set_source(s.comp, s.lo, s.hi, s.profile, s.amplitude, s.f0, s.t0, s.tp)
+        sim.set_source(s.comp, s.lo, s.hi, s.profile, s.amplitude, s.f0, s.t0, s.tp,
+                       kind=getattr(s, "kind", 0))
     return sim

@@ -579,6 +579,12 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
   return FDTD_LLG_OK;
 }
 
+int count_sources(const fdtd_llg *s, int kind) {
+  int n = 0;
+  for (int q = 0; q < s->src.count; ++q) n += s->src.s[q].kind == kind;
+  return n;
+}
+
 int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int *launches) {
   const dim3 blk(TX, TY, 1);
   EArgs a{};
@@ -590,7 +596,7 @@ int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, in
   a.src = s->src;
   a.st = s->dstate;
   const int grid = grid_for(s, a.box, 0);
-  const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = s->src.count > 0;
+  const bool ea = s->eps_r.is_array, sa = s->sigma.is_array, hs = count_sources(s, FDTD_LLG_SRC_SOFT_E) > 0;
 #define EK(EA, SA, HS)                                                        \
   if (ea == EA && sa == SA && hs == HS) k_e_update<EA, SA, HS><<<grid, blk, 0, s->stream>>>(a);
   prof_begin(s, FDTD_LLG_K_E_UPDATE, 0);
@@ -605,6 +611,28 @@ int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, in
 
 // one full time step: HM half (curl E^n), E update, HM half (curl E^{n+1}).
 // H sets: state in 0 -> half 1 result in 1 -> half 2 result back in 0.  M sets: 0 -> 1 -> 0.
+// hard E / soft H / hard H sources of one kind: a small kernel per source on its box
+int enqueue_box_sources(fdtd_llg *s, int kind, double *const *F, int *launches) {
+  for (int q = 0; q < s->src.count; ++q) {
+    const SourceP &S = s->src.s[q];
+    if (S.kind != kind) continue;
+    BoxSrcArgs a{};
+    a.g = s->g;
+    a.S = S;
+    a.idx = q;
+    a.F = F[S.comp];
+    a.st = s->dstate;
+    long long n = 1;
+    for (int d = 0; d < 3; ++d) n *= S.hi[d] - S.lo[d];
+    prof_begin(s, FDTD_LLG_K_OTHER, 0);
+    k_box_source<<<grid_1d(s, n), 256, 0, s->stream>>>(a);
+    prof_end(s);
+    ++*launches;
+  }
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
 // one time step; par = parity of the step: E^n is in E set `par`, E^{n+1} goes to the other set
 int enqueue_step(fdtd_llg *s, int par, int *launches) {
   *launches = 0;
@@ -615,13 +643,18 @@ int enqueue_step(fdtd_llg *s, int par, int *launches) {
     prof_end(s);
     ++*launches;
   }
-  int rc = enqueue_half(s, Ea, 0, 1, 2, 0, 1, false, launches);
+  int rc = enqueue_box_sources(s, FDTD_LLG_SRC_SOFT_H, s->Hset[0], launches);  // beginning of the step
+  if (rc) return rc;
+  rc = enqueue_half(s, Ea, 0, 1, 2, 0, 1, false, launches);
   if (rc) return rc;
   rc = enqueue_e(s, Ea, Eb, 1, launches);
   if (rc) return rc;
-  return enqueue_half(s, Eb, 1, 0, 2, 1, 0, true, launches);
+  rc = enqueue_box_sources(s, FDTD_LLG_SRC_HARD_E, Eb, launches);              // after the E update
+  if (rc) return rc;
+  rc = enqueue_half(s, Eb, 1, 0, 2, 1, 0, true, launches);
+  if (rc) return rc;
+  return enqueue_box_sources(s, FDTD_LLG_SRC_HARD_H, s->Hset[0], launches);    // after the H update
 }
-
 int build_graph(fdtd_llg *s, int par) {
   if (s->graph[par]) { cudaGraphExecDestroy(s->graph[par]); s->graph[par] = nullptr; }
   s->graph_valid[par] = false;
@@ -852,7 +885,15 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
 int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
                         const double *profile, int mem_space, double amplitude, double f0,
                         double t0, double tp) {
+  return fdtd_llg_add_source(s, FDTD_LLG_SRC_SOFT_E, comp, lo, hi, profile, mem_space, amplitude, f0, t0, tp);
+}
+
+int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const int *hi,
+                        const double *profile, int mem_space, double amplitude, double f0,
+                        double t0, double tp) {
   if (!s) return FDTD_LLG_EINVAL;
+  if (kind < FDTD_LLG_SRC_SOFT_E || kind > FDTD_LLG_SRC_HARD_H)
+    return fail(s, FDTD_LLG_EINVAL, "kind must be one of FDTD_LLG_SRC_*");
   if (s->src.count >= MAX_SOURCES) return fail(s, FDTD_LLG_ESTATE, "at most %d sources", MAX_SOURCES);
   if (comp < 0 || comp > 2) return fail(s, FDTD_LLG_EINVAL, "comp must be 0, 1 or 2");
   if (!lo || !hi) return fail(s, FDTD_LLG_EINVAL, "lo / hi is NULL");
@@ -865,6 +906,7 @@ int fdtd_llg_set_source(fdtd_llg *s, int comp, const int *lo, const int *hi,
     nb *= (size_t)(hi[d] - lo[d]);
   }
   SourceP &S = s->src.s[s->src.count];
+  S.kind = kind;
   S.comp = comp;
   for (int d = 0; d < 3; ++d) { S.lo[d] = lo[d]; S.hi[d] = hi[d]; }
   S.amplitude = amplitude; S.f0 = f0; S.t0 = t0; S.tp = tp;

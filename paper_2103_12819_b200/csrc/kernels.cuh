@@ -74,6 +74,7 @@ struct DevState {
 };
 
 struct SourceP {
+  int kind;  // 0 soft E (J of eq. 11), 1 hard E, 2 soft H, 3 hard H (fdtd_llg.h)
   int comp;
   int lo[3], hi[3];
   const double *profile;  // device, box sized, or nullptr
@@ -611,7 +612,7 @@ __device__ __forceinline__ double source_term(const EArgs &a, int i, int j, int 
   double J = 0.0;
   for (int s = 0; s < a.src.count; ++s) {
     const SourceP &S = a.src.s[s];
-    if (S.comp != D) continue;
+    if (S.kind != 0 || S.comp != D) continue;
     if (i < S.lo[0] || i >= S.hi[0] || j < S.lo[1] || j >= S.hi[1] || k < S.lo[2] || k >= S.hi[2])
       continue;
     double p = 1.0;
@@ -659,9 +660,47 @@ __global__ void __launch_bounds__(NTHREADS, 4) k_e_update(const __grid_constant_
 __global__ void k_step_begin(DevState *st, const __grid_constant__ SourcesP src, double dt) {
   const int s = threadIdx.x;
   if (s >= src.count) return;
-  const double t = ((double)st->steps + 0.5) * dt;
+  // the time a source is evaluated at: soft E (n+1/2) dt (eq. 11), soft H n dt (the beginning of
+  // the step), hard E / hard H (n+1) dt (after their updates)          (reading A25)
+  const int kind = src.s[s].kind;
+  const double t = ((double)st->steps + (kind == 0 ? 0.5 : (kind == 2 ? 0.0 : 1.0))) * dt;
   const double uu = (t - src.s[s].t0) / src.s[s].tp;
   st->src_amp[s] = src.s[s].amplitude * exp(-0.5 * uu * uu) * cos(2.0 * kPi * src.s[s].f0 * t);
+}
+
+// Hard E / soft H / hard H source number `idx` applied to field component F on its box
+// (PAPER.md:100): F = amp * profile (hard) or F += dt * amp * profile (soft H).  Wall-tangential E
+// edges and wall faces of H stay 0; periodic ghost images are refreshed.
+struct BoxSrcArgs {
+  GridP g;
+  SourceP S;
+  int idx;
+  double *F;
+  const DevState *st;
+};
+__global__ void k_box_source(const __grid_constant__ BoxSrcArgs a) {
+  const SourceP &S = a.S;
+  const int bx = S.hi[0] - S.lo[0], by = S.hi[1] - S.lo[1], bz = S.hi[2] - S.lo[2];
+  const long long n = (long long)bx * by * bz;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n;
+       q += (long long)gridDim.x * blockDim.x) {
+    const int i = S.lo[0] + (int)(q % bx), j = S.lo[1] + (int)((q / bx) % by),
+              k = S.lo[2] + (int)(q / ((long long)bx * by));
+    const int idx[3] = {i, j, k};
+    bool wall = false;
+    if (S.kind == 1) {  // E edge: tangential to the walls of the two other axes
+      for (int d = 0; d < 3; ++d)
+        if (d != S.comp && !a.g.per[d] && idx[d] == 0) wall = true;
+    } else {            // H face: the wall of its own axis
+      wall = !a.g.per[S.comp] && idx[S.comp] == 0;
+    }
+    if (wall) continue;
+    const double v = a.st->src_amp[a.idx] * (S.profile ? __ldg(S.profile + q) : 1.0);
+    const int c = a.g.org + i + a.g.sy * j + a.g.sz * k;
+    const double out = S.kind == 2 ? a.F[c] + a.g.dt * v : v;
+    a.F[c] = out;
+    store_images_inl(a.F, a.g, i, j, k, c, out);
+  }
 }
 
 // ------------------------------------------------------------------ set-up kernels

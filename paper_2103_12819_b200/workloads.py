@@ -93,6 +93,7 @@ class Source:
     t0: float
     tp: float
     profile: Optional[torch.Tensor] = None
+    kind: int = 0   # 0 soft E (J of eq. 11), 1 hard E, 2 soft H, 3 hard H
 
 
 @dataclass

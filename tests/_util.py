@@ -24,7 +24,7 @@ def oracle_from_workload(w, kind="f64", time_scheme=0) -> Oracle:
     o.set_fields(a["E"], a["H"], a["M_cell"])
     for s in w.sources:
         prof = None if s.profile is None else s.profile.detach().cpu().numpy()
-        o.set_source(s.comp, s.lo, s.hi, prof, s.amplitude, s.f0, s.t0, s.tp)
+        o.set_source(s.comp, s.lo, s.hi, prof, s.amplitude, s.f0, s.t0, s.tp, kind=getattr(s, "kind", 0))
     return o
 
 
