@@ -153,8 +153,8 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": f"cfg{args.config} {full[0]}x{full[1]}x{full[2]} (sampled)",
-                       "sample": sample},
+            "config": {"workload": f"{w.name} {full[0]}x{full[1]}x{full[2]}", "sample": sample,
+                       "time_scheme": "first-order" if args.time_scheme else "second-order"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
