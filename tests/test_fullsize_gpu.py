@@ -185,3 +185,34 @@ def test_config5_full_size_windows_and_invariants():
         for g in ("E", "H", "M"):
             num = max(float(np.max(np.abs(got[nm][core] - ref[nm][core]))) for nm in FIELD_GROUPS[g])
             assert num / sc[g] <= TOL, (lo, g, num / sc[g])
+
+
+def test_config5_full_size_kernel_paths_agree_bitwise():
+    """768^3: the staged sweeps (kernel_path 0, what bench.py times) against the direct-load
+    kernels, bit for bit, through checksums of the bit patterns (two 129 GB workspaces do not fit
+    side by side): wrap-around sum and xor of every result array viewed as int64."""
+    _need_gb(165)
+    import gc
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(5, device="cuda:0")
+    sums = []
+    for path in (1, 0):
+        sim = from_workload(w, kernel_path=path)
+        sim.step(2)
+        cs = {}
+        for nm in ALL:
+            t = sim.read_fields(names=(nm,), device="cuda:0")[nm].view(torch.int64)
+            x = t.flatten()
+            while x.numel() > 1:                      # xor reduction by halving
+                h = x.numel() // 2
+                x = torch.cat([x[:h] ^ x[h:2 * h], x[2 * h:]])
+            cs[nm] = (int(t.sum()), int(x[0]))
+            del t, x
+        assert sim.stats()["iters_total"] == 12
+        sums.append(cs)
+        sim.close()
+        del sim
+        gc.collect()
+        torch.cuda.empty_cache()
+    assert sums[0] == sums[1]
+    assert len({v for v in sums[0].values()}) > 10     # not all the same (not all zero)
