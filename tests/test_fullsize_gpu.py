@@ -29,6 +29,9 @@ ALL = FIELD_GROUPS["E"] + FIELD_GROUPS["H"] + FIELD_GROUPS["M"]
 
 
 def _need_gb(gb):
+    import gc
+    gc.collect()                      # workspaces of earlier tests
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info(0)
     if free < gb * 1e9:
         pytest.skip(f"needs {gb} GB of free device memory, {free / 1e9:.0f} GB available")
