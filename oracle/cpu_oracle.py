@@ -83,7 +83,8 @@ class Oracle:
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, *, eps_r=None, sigma=None, mu_r=None,
                  Ms=None, alpha=None, gamma=None, bc=(0, 0, 0), enable_llg=True,
                  h_bias=(0.0, 0.0, 0.0), ani_hk=0.0, ani_axis=(0.0, 0.0, 1.0),
-                 llg_tol=1e-12, llg_max_iter=20, kind="f64", time_scheme=0):
+                 llg_tol=1e-12, llg_max_iter=20, kind="f64", time_scheme=0, pml=None,
+                 pml_r0=1e-6, pml_order=3):
         self._lib, self._p = _lib(kind)
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
@@ -108,6 +109,16 @@ class Oracle:
             g.argtypes = [C.c_void_p, C.c_int]
             if g(self._h, int(time_scheme)):
                 raise ValueError("oracle_set_scheme rejected the scheme")
+
+        if pml is not None and any(int(v) for v in pml):
+            # open boundary: pml = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi) cells
+            g = self._fn("set_pml")
+            g.restype = C.c_int
+            g.argtypes = [C.c_void_p, _IP, C.c_double, C.c_int]
+            rc = g(self._h, (C.c_int * 6)(*[int(v) for v in pml]), float(pml_r0), int(pml_order))
+            if rc:
+                raise ValueError(f"oracle_set_pml failed ({rc}): PML on a periodic axis, too thick, "
+                                 "or magnetic faces inside the layer")
 
     def _fn(self, name):
         return getattr(self._lib, self._p + name)

@@ -92,6 +92,12 @@ typedef struct {
   REAL hbias[3], hk, axis[3], tol;
   int max_iter;
   int scheme;          /* 0: second order, eqs. 15-21 (default); 1: first order, eqs. 6-9, 12-14 */
+  /* open boundary: split-field PML with multiplicative damping (reading A26) */
+  int has_pml, pml[3][2];          /* PML cells on the low / high side of each axis          */
+  int pml_synced;                  /* split parts hold the present total fields              */
+  REAL *pdE[3], *pdH[3];           /* sqrt of the damping factor of one update along each axis: */
+                                   /* E parts (nodes, step dt), H parts (half positions, dt/2)   */
+  REAL *Esp[3][2], *Hsp[3][2];     /* split parts: [component][0: d/d(d+1) term, 1: d/d(d+2)] */
   size_t ncell;
   REAL *eps_r, *sigma, *mu_r, *Ms, *alpha, *gamma; /* cell centred */
   REAL *E[3], *H[3], *M[3][3];
@@ -305,6 +311,10 @@ void ORC(destroy)(void *h) {
     for (int c = 0; c < 3; ++c) { free(o->M[d][c]); free(o->Mn[d][c]); free(o->Mp[d][c]); }
   }
   for (int s = 0; s < o->nsrc; ++s) free(o->src[s].profile);
+  for (int a = 0; a < 3; ++a) {
+    free(o->pdE[a]); free(o->pdH[a]);
+    for (int q = 0; q < 2; ++q) { free(o->Esp[a][q]); free(o->Hsp[a][q]); }
+  }
   free(o);
 }
 
@@ -357,6 +367,7 @@ int ORC(set_fields)(void *h, const double *Ex, const double *Ey, const double *E
         }
       }
   for (int c = 0; c < 3; ++c) free(Mc[c]);
+  o->pml_synced = 0;
   return rc;
 }
 
@@ -428,6 +439,121 @@ static REAL source_at(const oracle_t *o, int comp, const int c[3], REAL t) {
 /* eq. 11:
  * E^{n+1} = (sigma/2 + eps/dt)^-1 [ curl H^{n+1/2} - (sigma/2 - eps/dt) E^n - J_src^{n+1/2} ]
  * at every edge that is not wall-tangential; eps, sigma = four-cell means. */
+/* ------------------------------------------------------------------ PML (open boundary)
+ * "a perfectly matched layer (PML) first developed by Berenger ... damps out EM
+ * waves using a non-physical conductivity in the guard cells ... field components E and H are
+ * updated using macroscopic Maxwell's equations that account for spatially varying material
+ * properties and then the updated field components are multiplied by the corresponding PML
+ * damping coefficients".  The paper gives no formulas (it points to Shapoval et al. 2019); the
+ * reading taken (A26):
+ *  - the layer is the outermost pml[a][side] cells of the grid along axis a, backed by the PEC wall;
+ *  - there every component is split in two parts, one per term of the curl (Berenger):
+ *      F_d = F_d,0 + F_d,1,  part 0 <- d/d(d+1) term, part 1 <- d/d(d+2) term;
+ *  - each part is advanced by the macroscopic update (eq. 11 for E with the local eps, sigma;
+ *    eq. 21 with M = 0 and the local mu for H) with its own term of the curl, between two
+ *    multiplications by the square root of its damping factor (two-step, time-centred: the
+ *    "2SC" of the name): the factor is exp(-s_a dt) for E (one step) and exp(-s_a dt/2) for H
+ *    (one half-step), a = the axis of the derivative in that term: the same decay RATE s_a for E
+ *    and H, which is the matching condition sigma_a/eps = sigma*_a/mu in any medium;
+ *  - s_a(u) = s_max (u/L)^m at depth u into a layer of thickness L, sampled at the nodes (E parts)
+ *    and half positions (H parts) of axis a; s_max = -(m+1) c ln(R0) / (2 L), the textbook choice
+ *    for a theoretical normal-incidence reflection R0;
+ *  - no magnetic face inside the layer (future work in the paper too). */
+static int in_pml(const oracle_t *o, const int c[3]) {
+  for (int a = 0; a < 3; ++a)
+    if (c[a] < o->pml[a][0] || c[a] >= o->n[a] - o->pml[a][1]) return 1;
+  return 0;
+}
+
+static REAL pml_rate(const oracle_t *o, int a, long double x, long double r0, int order) {
+  long double L, u;
+  const long double len = (long double)o->n[a] * (long double)o->d[a];
+  if (o->pml[a][0] > 0 && x < (L = o->pml[a][0] * (long double)o->d[a])) u = L - x;
+  else if (o->pml[a][1] > 0 && x > len - (L = o->pml[a][1] * (long double)o->d[a])) u = x - (len - L);
+  else return 0;
+  long double smax = -(order + 1) * (long double)C0 * logl(r0) / (2 * L);
+  return (REAL)(smax * powl(u / L, order));
+}
+
+int ORC(set_pml)(void *h, const int *pml, double r0, int order) {
+  oracle_t *o = (oracle_t *)h;
+  if (!(r0 > 0 && r0 < 1) || order < 1 || order > 6) return -1;
+  for (int a = 0; a < 3; ++a)
+    for (int sd = 0; sd < 2; ++sd) {
+      int p = pml[2 * a + sd];
+      if (p < 0 || (p > 0 && o->bc[a])) return -1; /* a PML axis ends on a PEC wall, not periodic */
+      o->pml[a][sd] = p;
+    }
+  for (int a = 0; a < 3; ++a)
+    if (o->pml[a][0] + o->pml[a][1] > o->n[a]) return -1;
+  o->has_pml = 0;
+  for (int a = 0; a < 3; ++a) o->has_pml |= (o->pml[a][0] | o->pml[a][1]) != 0;
+  for (int a = 0; a < 3; ++a) {
+    free(o->pdE[a]);
+    free(o->pdH[a]);
+    o->pdE[a] = (REAL *)malloc(sizeof(REAL) * (size_t)o->n[a]);
+    o->pdH[a] = (REAL *)malloc(sizeof(REAL) * (size_t)o->n[a]);
+    for (int i = 0; i < o->n[a]; ++i) {
+      long double xe = i * (long double)o->d[a], xh = (i + 0.5L) * (long double)o->d[a];
+      /* half of the damping of one update: exp(-s dt/2) for E (step dt), exp(-s dt/4) for H (dt/2) */
+      o->pdE[a][i] = (REAL)expl(-(long double)pml_rate(o, a, xe, r0, order) * (long double)o->dt / 2);
+      o->pdH[a][i] = (REAL)expl(-(long double)pml_rate(o, a, xh, r0, order) * (long double)o->dt / 4);
+    }
+    for (int q = 0; q < 2; ++q) {
+      if (!o->Esp[a][q]) o->Esp[a][q] = alloc_fill(o->ncell, NULL, 0.0);
+      if (!o->Hsp[a][q]) o->Hsp[a][q] = alloc_fill(o->ncell, NULL, 0.0);
+    }
+  }
+  o->pml_synced = 0;
+  /* no magnetic face may belong to a PML cell */
+  for (int k = 0; k < o->n[2]; ++k)
+    for (int j = 0; j < o->n[1]; ++j)
+      for (int i = 0; i < o->n[0]; ++i) {
+        int c[3] = {i, j, k};
+        if (!in_pml(o, c)) continue;
+        for (int d = 0; d < 3; ++d) {
+          REAL Msf;
+          if (magnetic_face(o, d, c, &Msf)) return -2;
+        }
+      }
+  return 0;
+}
+
+/* one E edge of a PML cell: eq. 11 on each part, then the damping factors */
+static REAL pml_e_edge(oracle_t *o, int d, const int c[3], size_t id, REAL J) {
+  const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+  REAL eps = EPS0 * edge_mean(o, o->eps_r, d, c);
+  REAL sig = edge_mean(o, o->sigma, d, c);
+  REAL term0 = (rd(o, o->H[d2], c) - rd_off(o, o->H[d2], c, d1, -1)) / o->d[d1];
+  REAL term1 = -(rd(o, o->H[d1], c) - rd_off(o, o->H[d1], c, d2, -1)) / o->d[d2];
+  REAL den = sig / 2 + eps / o->dt, keep = -(sig / 2 - eps / o->dt);
+  /* two-step, time-centred damping ("PML-2SC"): half of it before the update, half after */
+  const REAL g0 = o->pdE[d1][c[d1]], g1 = o->pdE[d2][c[d2]];
+  REAL p0 = (term0 + keep * (g0 * o->Esp[d][0][id]) - J) / den;
+  REAL p1 = (term1 + keep * (g1 * o->Esp[d][1][id])) / den;
+  p0 *= g0;
+  p1 *= g1;
+  o->Esp[d][0][id] = p0;
+  o->Esp[d][1][id] = p1;
+  return p0 + p1;
+}
+
+/* one H face of a PML cell over half a step: eq. 21 with M = 0 on each part, then the damping */
+static REAL pml_h_face(oracle_t *o, int d, const int c[3], size_t id) {
+  const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+  REAL mu = MU0 * face_mean(o, o->mu_r, d, c);
+  REAL term0 = (rd_off(o, o->E[d2], c, d1, +1) - rd(o, o->E[d2], c)) / o->d[d1];
+  REAL term1 = -(rd_off(o, o->E[d1], c, d2, +1) - rd(o, o->E[d1], c)) / o->d[d2];
+  const REAL g0 = o->pdH[d1][c[d1]], g1 = o->pdH[d2][c[d2]];
+  REAL p0 = g0 * o->Hsp[d][0][id] - (o->dt / 2 / mu) * term0;
+  REAL p1 = g1 * o->Hsp[d][1][id] - (o->dt / 2 / mu) * term1;
+  p0 *= g0;
+  p1 *= g1;
+  o->Hsp[d][0][id] = p0;
+  o->Hsp[d][1][id] = p1;
+  return p0 + p1;
+}
+
 static void e_update(oracle_t *o) {
   REAL t_half = ((REAL)o->steps + (REAL)0.5) * o->dt;
 #pragma omp parallel for schedule(static)
@@ -441,6 +567,10 @@ static void e_update(oracle_t *o) {
           REAL eps = EPS0 * edge_mean(o, o->eps_r, d, c);
           REAL sig = edge_mean(o, o->sigma, d, c);
           REAL J = o->nsrc ? source_at(o, d, c, t_half) : (REAL)0;
+          if (o->has_pml && in_pml(o, c)) {
+            o->E[d][id] = pml_e_edge(o, d, c, id, J);
+            continue;
+          }
           REAL rhs = curl_H(o, o->H, d, c) - (sig / 2 - eps / o->dt) * o->E[d][id] - J;
           o->E[d][id] = rhs / (sig / 2 + eps / o->dt);
         }
@@ -557,8 +687,12 @@ static void hm_half(oracle_t *o) {
           }
           REAL v = 0;
           if (!wall_face(o, d, c)) {
-            REAL mu = MU0 * face_mean(o, o->mu_r, d, c);
-            v = o->Hn[d][id] - (half_dt / mu) * o->C[d][id];
+            if (o->has_pml && in_pml(o, c)) {
+              v = pml_h_face(o, d, c, id);
+            } else {
+              REAL mu = MU0 * face_mean(o, o->mu_r, d, c);
+              v = o->Hn[d][id] - (half_dt / mu) * o->C[d][id];
+            }
           }
           o->H[d][id] = v;
           o->Hc[d][id] = v; /* iterate r >= 1; Hp keeps H^{r=0} = H^n for the r = 1 sweep (A6) */
@@ -630,6 +764,17 @@ static void hm_half(oracle_t *o) {
 }
 
 /* n time steps:  HM half (curl E^n) ; E update ; HM half (curl E^{n+1}) */
+/* fields given from outside (initial condition) enter the layer as part 0 of each component */
+static void pml_sync(oracle_t *o) {
+  if (!o->has_pml || o->pml_synced) return;
+  for (int d = 0; d < 3; ++d)
+    for (size_t i = 0; i < o->ncell; ++i) {
+      o->Esp[d][0][i] = o->E[d][i]; o->Esp[d][1][i] = 0;
+      o->Hsp[d][0][i] = o->H[d][i]; o->Hsp[d][1][i] = 0;
+    }
+  o->pml_synced = 1;
+}
+
 /* sources of one kind applied to E (kinds 1) or H (kinds 2, 3) at time t */
 static void apply_field_sources(oracle_t *o, int kind, REAL t) {
   for (int q = 0; q < o->nsrc; ++q) {
@@ -645,6 +790,7 @@ static void apply_field_sources(oracle_t *o, int kind, REAL t) {
         for (int i = S->lo[0]; i < S->hi[0]; ++i) {
           int c[3] = {i, j, k};
           if (kind == 1 ? wall_edge(o, S->comp, c) : wall_face(o, S->comp, c)) continue;
+          if (o->has_pml && in_pml(o, c)) continue; /* field sources act outside the layer only */
           REAL p = S->profile ? S->profile[(size_t)(i - S->lo[0]) +
                                            bx * ((size_t)(j - S->lo[1]) + by * (size_t)(k - S->lo[2]))]
                               : 1;
@@ -658,6 +804,7 @@ static void apply_field_sources(oracle_t *o, int kind, REAL t) {
 
 int ORC(step)(void *h, int n) {
   oracle_t *o = (oracle_t *)h;
+  pml_sync(o);
   for (int s = 0; s < n; ++s) {
     apply_field_sources(o, 2, (REAL)o->steps * o->dt);        /* soft H, beginning of the step */
     hm_half(o);
@@ -679,6 +826,7 @@ int ORC(set_scheme)(void *h, int scheme) {
 
 /* test hook: ONE (H,M) half-step with the present E (no E update, no step count) */
 int ORC(hm_half_step)(void *h) {
+  pml_sync((oracle_t *)h);
   hm_half((oracle_t *)h);
   return 0;
 }
@@ -712,6 +860,7 @@ int ORC(write_fields)(void *h, const double *const *in) {
       if (in[6 + 3 * d + c])
         for (size_t i = 0; i < o->ncell; ++i) o->M[d][c][i] = (REAL)in[6 + 3 * d + c][i];
   }
+  o->pml_synced = 0;
   return 0;
 }
 
