@@ -81,6 +81,14 @@ typedef struct {
                          1: the first-order scheme: one forward-Euler sweep of
                          eq. 7 / 12 per (H,M) half-step (advancing dt/2), N(M), then eq. 9 / 14;
                          llg_tol and llg_max_iter are not used                                   */
+  int pml[6];         /* open boundary: cells of the PML on the x-low, x-high, y-low,
+                         y-high, z-low, z-high side (0 = none).  The layer is part of the grid (its
+                         outermost cells), the axis must be FDTD_LLG_PEC (the wall behind the layer)
+                         and no magnetic cell may touch it.  Split-field Berenger layer with two-step
+                         time-centred multiplicative damping, decay rate s(u) = s_max (u/L)^order,
+                         s_max = -(order+1) c ln(pml_r0) / (2 L) (A26)                  */
+  double pml_r0;      /* theoretical normal-incidence reflection of the layer (default 1e-6)       */
+  int pml_order;      /* grading order m (default 3)                                               */
 } fdtd_llg_options;
 
 typedef struct {
@@ -121,8 +129,9 @@ void fdtd_llg_default_options(fdtd_llg_options *opt);
 /* Bytes of DEVICE workspace fdtd_llg_create needs for this grid.  `material_mask` = OR of the
  * FDTD_LLG_MAT_* bits of the material arrays that will be passed non-NULL (a uniform array costs
  * nothing once detected, so this is an upper bound).  Returns 0 on invalid arguments.
- * Budget: 6 doubles/cell for E,H; +24/cell when enable_llg (two more H sets for the Jacobi
- * iterates, M and its time-n copy); +1/cell per material array. */
+ * Budget: 12 doubles/cell for E,H (two sets each: every update is out of place); +21/cell when
+ * enable_llg (the Jacobi H buffer, M and its time-n copy); +1/cell per material array; +13/cell
+ * with a PML (12 split parts, the damping tables). */
 size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
                                 unsigned material_mask);
 

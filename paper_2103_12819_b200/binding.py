@@ -30,7 +30,8 @@ class Options(C.Structure):
                 ("ani_hk", C.c_double), ("ani_axis", C.c_double * 3), ("llg_tol", C.c_double),
                 ("llg_max_iter", C.c_int), ("use_graph", C.c_int),
                 ("scalar_material_mask", C.c_uint), ("kernel_path", C.c_int),
-                ("time_scheme", C.c_int)]
+                ("time_scheme", C.c_int), ("pml", C.c_int * 6), ("pml_r0", C.c_double),
+                ("pml_order", C.c_int)]
 
 
 class Stats(C.Structure):
@@ -156,7 +157,7 @@ class FdtdLlg:
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, *, materials=None, bc=(PEC, PEC, PEC),
                  enable_llg=True, h_bias=(0.0, 0.0, 0.0), ani_hk=0.0, ani_axis=(0.0, 0.0, 1.0),
                  llg_tol=1e-6, llg_max_iter=20, use_graph=True, device="cuda:0", stream=None,
-                 kernel_path=0, time_scheme=0):
+                 kernel_path=0, time_scheme=0, pml=None, pml_r0=None, pml_order=None):
         import torch
         self._torch = torch
         self.shape = (nz, ny, nx)
@@ -176,6 +177,13 @@ class FdtdLlg:
         opt.use_graph = int(bool(use_graph))
         opt.kernel_path = int(kernel_path)
         opt.time_scheme = int(time_scheme)
+        if pml is not None:
+            for q in range(6):
+                opt.pml[q] = int(pml[q])
+        if pml_r0 is not None:
+            opt.pml_r0 = float(pml_r0)
+        if pml_order is not None:
+            opt.pml_order = int(pml_order)
         self.options = opt
         materials = {k: v for k, v in (materials or {}).items() if v is not None}
         scalars = {k: C.c_double(float(v)) for k, v in materials.items()
@@ -318,7 +326,8 @@ def from_workload(w, device="cuda:0", use_graph=True, stream=None, fields_device
                   enable_llg=w.enable_llg, h_bias=w.h_bias, ani_hk=w.ani_hk, ani_axis=w.ani_axis,
                   llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, use_graph=use_graph,
                   device=device, stream=stream, kernel_path=kernel_path,
-                  time_scheme=time_scheme)
+                  time_scheme=time_scheme, pml=getattr(w, "pml", None),
+                  pml_r0=getattr(w, "pml_r0", None), pml_order=getattr(w, "pml_order", None))
     sim.set_fields(w.E, w.H, w.M_cell)
     for s in w.sources:
         sim.set_source(s.comp, s.lo, s.hi, s.profile, s.amplitude, s.f0, s.t0, s.tp,

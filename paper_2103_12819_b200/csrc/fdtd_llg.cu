@@ -70,6 +70,12 @@ struct fdtd_llg {
   CUtensorMap mapT{}, mapPM{};
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
+  // open boundary: split parts of E and H, damping tables, the layer's slabs
+  bool has_pml = false;
+  double *Esp[6]{}, *Hsp[6]{};   // [2 * component + part]
+  double *pdE[3]{}, *pdH[3]{};   // sqrt damping factors along x, y, z (device)
+  BoxP box_pml[6]{};
+  int n_pml = 0;
 
   DevState *dstate = nullptr;
   unsigned long long *resid = nullptr;
@@ -190,6 +196,15 @@ bool valid_opts(const fdtd_llg_options *o, const char **why) {
   for (int d = 0; d < 3; ++d)
     if (o->bc[d] != FDTD_LLG_PEC && o->bc[d] != FDTD_LLG_PERIODIC) { *why = "bc must be 0 (PEC) or 1 (periodic)"; return false; }
   if (o->time_scheme != 0 && o->time_scheme != 1) { *why = "time_scheme must be 0 (second order) or 1 (first order)"; return false; }
+  for (int a = 0; a < 3; ++a)
+    for (int sd = 0; sd < 2; ++sd) {
+      if (o->pml[2 * a + sd] < 0) { *why = "pml thickness must be >= 0"; return false; }
+      if (o->pml[2 * a + sd] > 0 && o->bc[a] != FDTD_LLG_PEC) { *why = "a PML axis must be FDTD_LLG_PEC (the wall behind the layer)"; return false; }
+    }
+  if (o->pml[0] | o->pml[1] | o->pml[2] | o->pml[3] | o->pml[4] | o->pml[5]) {
+    if (!(o->pml_r0 > 0 && o->pml_r0 < 1)) { *why = "pml_r0 must be in (0, 1)"; return false; }
+    if (o->pml_order < 1 || o->pml_order > 6) { *why = "pml_order must be in 1..6"; return false; }
+  }
   if (o->enable_llg) {
     if (!(o->llg_tol > 0) || !std::isfinite(o->llg_tol)) { *why = "llg_tol must be > 0"; return false; }
     if (o->llg_max_iter < 1 || o->llg_max_iter > 1000) { *why = "llg_max_iter must be in 1..1000"; return false; }
@@ -448,6 +463,102 @@ int setup_hm_stage_by(fdtd_llg *s) {
   return FDTD_LLG_OK;
 }
 
+// ---- open boundary (A26) ---------------------------------------------
+
+// decay rate s_a(x) of the layer on axis a at position x (host, long double)
+long double pml_rate(const fdtd_llg *s, int a, long double x) {
+  const long double dx = s->d[a], len = s->g.n[a] * dx;
+  const int plo = s->opt.pml[2 * a], phi = s->opt.pml[2 * a + 1];
+  long double L, u;
+  if (plo > 0 && x < (L = plo * dx)) u = L - x;
+  else if (phi > 0 && x > len - (L = phi * dx)) u = x - (len - L);
+  else return 0.0L;
+  const long double smax = -(s->opt.pml_order + 1) * (long double)kC0 * logl((long double)s->opt.pml_r0) / (2 * L);
+  return smax * powl(u / L, s->opt.pml_order);
+}
+
+// split parts, damping tables and the slabs of the layer; *q = next free array of the workspace
+int setup_pml(fdtd_llg *s, double **q) {
+  const int *pm = s->opt.pml;
+  s->has_pml = (pm[0] | pm[1] | pm[2] | pm[3] | pm[4] | pm[5]) != 0;
+  if (!s->has_pml) return FDTD_LLG_OK;
+  for (int a = 0; a < 3; ++a)
+    if (pm[2 * a] + pm[2 * a + 1] > s->g.n[a]) return fail(s, FDTD_LLG_EINVAL, "the PML is thicker than the grid on axis %d", a);
+  if (s->llg)  // the sweep box (magnetic cells + 1) must stay clear of the layer
+    for (int a = 0; a < 3; ++a)
+      if (s->lo[a] < pm[2 * a] || s->hi[a] > s->g.n[a] - pm[2 * a + 1])
+        return fail(s, FDTD_LLG_EINVAL, "magnetic cells touch the PML on axis %d (PAPER.md:189: not supported)", a);
+  const size_t abytes = s->stride * sizeof(double);
+  for (int c = 0; c < 6; ++c) { s->Esp[c] = *q; *q += s->stride; }
+  for (int c = 0; c < 6; ++c) { s->Hsp[c] = *q; *q += s->stride; }
+  CU(s, cudaMemsetAsync(s->Esp[0], 0, 12 * abytes, s->stream));
+  double *tab = *q;
+  *q += s->stride;
+  std::vector<double> host;
+  for (int a = 0; a < 3; ++a) {
+    s->pdE[a] = tab + host.size();
+    for (int i = 0; i < s->g.n[a]; ++i)  // E parts: nodes of axis a, half the damping of one step dt
+      host.push_back((double)expl(-pml_rate(s, a, i * (long double)s->d[a]) * (long double)s->dt / 2));
+    s->pdH[a] = tab + host.size();
+    for (int i = 0; i < s->g.n[a]; ++i)  // H parts: half positions, half the damping of dt/2
+      host.push_back((double)expl(-pml_rate(s, a, (i + 0.5L) * (long double)s->d[a]) * (long double)s->dt / 4));
+  }
+  CU(s, cudaMemcpyAsync(tab, host.data(), host.size() * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+  CU(s, cudaStreamSynchronize(s->stream));
+  // the layer = complement of the interior box, peeled into <= 6 disjoint slabs (z, then y, then x)
+  int lo[3] = {0, 0, 0}, hi[3] = {s->g.n[0], s->g.n[1], s->g.n[2]};
+  s->n_pml = 0;
+  for (int d = 2; d >= 0; --d) {
+    const int il = pm[2 * d], ih = s->g.n[d] - pm[2 * d + 1];
+    if (il > lo[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      h[d] = il;
+      s->box_pml[s->n_pml++] = make_box(s, l, h);
+    }
+    if (ih < hi[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      l[d] = ih;
+      s->box_pml[s->n_pml++] = make_box(s, l, h);
+    }
+    lo[d] = il;
+    hi[d] = ih;
+  }
+  return FDTD_LLG_OK;
+}
+
+// the layer's update of E (after k_e_update) or of H (after the H half-step): In = the other field
+int enqueue_pml(fdtd_llg *s, bool is_e, double *const *In, double *const *Out, int *launches) {
+  if (!s->has_pml) return FDTD_LLG_OK;
+  PmlArgs a{};
+  a.g = s->g;
+  for (int d = 0; d < 3; ++d) {
+    a.In[d] = In[d];
+    a.Out[d] = Out[d];
+    a.d[d] = is_e ? s->pdE[d] : s->pdH[d];
+  }
+  for (int c = 0; c < 6; ++c) a.P[c] = is_e ? s->Esp[c] : s->Hsp[c];
+  a.eps_r = s->eps_r.is_array ? s->eps_r.dev : nullptr;
+  a.sigma = s->sigma.is_array ? s->sigma.dev : nullptr;
+  a.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
+  a.eps_u = kEps0 * s->eps_r.uniform;
+  a.sigma_u = s->sigma.uniform;
+  a.mu_u = kMu0 * s->mu_r.uniform;
+  a.src = s->src;
+  a.st = s->dstate;
+  const dim3 blk(TX, TY, 1);
+  for (int b = 0; b < s->n_pml; ++b) {
+    a.box = s->box_pml[b];
+    if (a.box.items == 0) continue;
+    prof_begin(s, FDTD_LLG_K_OTHER, 0);
+    if (is_e) k_pml<true><<<grid_for(s, a.box, 0), blk, 0, s->stream>>>(a);
+    else k_pml<false><<<grid_for(s, a.box, 0), blk, 0, s->stream>>>(a);
+    prof_end(s);
+    ++*launches;
+  }
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
 // ---- launching one step ----------------------------------------------------------------
 
 template <bool FIRST>
@@ -489,6 +600,10 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     else k_h_update<false><<<grid, blk, 0, s->stream>>>(h);
     prof_end(s);
     ++*launches;
+  }
+  {
+    int rc = enqueue_pml(s, false, E, s->Hset[out], launches);
+    if (rc) return rc;
   }
   if (s->llg) {
     HMArgs a{};
@@ -649,6 +764,8 @@ int enqueue_step(fdtd_llg *s, int par, int *launches) {
   if (rc) return rc;
   rc = enqueue_e(s, Ea, Eb, 1, launches);
   if (rc) return rc;
+  rc = enqueue_pml(s, true, s->Hset[1], Eb, launches);
+  if (rc) return rc;
   rc = enqueue_box_sources(s, FDTD_LLG_SRC_HARD_E, Eb, launches);              // after the E update
   if (rc) return rc;
   rc = enqueue_half(s, Eb, 1, 0, 2, 1, 0, true, launches);
@@ -695,6 +812,8 @@ void fdtd_llg_default_options(fdtd_llg_options *o) {
   o->llg_tol = 1e-6;
   o->llg_max_iter = 20;
   o->use_graph = 1;
+  o->pml_r0 = 1e-6;
+  o->pml_order = 3;
 }
 
 size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
@@ -705,6 +824,8 @@ size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *
   if (opt->enable_llg) arrays += 3 + 18;   // the Jacobi H buffer, two M sets
   for (unsigned b = 0; b < 6; ++b)
     if (material_mask & (1u << b)) ++arrays;
+  if (opt->pml[0] | opt->pml[1] | opt->pml[2] | opt->pml[3] | opt->pml[4] | opt->pml[5])
+    arrays += 13;                          // 12 split parts + one slot for the damping tables
   return arrays * stride * sizeof(double) + small_bytes(opt);
 }
 
@@ -805,6 +926,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   if ((rc = find_sweep_box(s))) return bail(rc);
   make_boxes(s);
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
+  if ((rc = setup_pml(s, &q))) return bail(rc);
   const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
   s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 || opt->kernel_path == 4 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
   s->stage_lean = opt->kernel_path == 4;
@@ -841,6 +963,13 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
     if ((rc = fill_ghosts(s, s->E[d]))) return rc;
     if ((rc = fill_ghosts(s, s->Hset[0][d]))) return rc;
   }
+  if (s->has_pml)  // fields given from outside enter the layer as part 0 of each component
+    for (int d = 0; d < 3; ++d) {
+      CU(s, cudaMemcpyAsync(s->Esp[2 * d], s->E[d], abytes, cudaMemcpyDeviceToDevice, s->stream));
+      CU(s, cudaMemcpyAsync(s->Hsp[2 * d], s->Hset[0][d], abytes, cudaMemcpyDeviceToDevice, s->stream));
+      CU(s, cudaMemsetAsync(s->Esp[2 * d + 1], 0, abytes, s->stream));
+      CU(s, cudaMemsetAsync(s->Hsp[2 * d + 1], 0, abytes, s->stream));
+    }
   // reset run state
   CU(s, cudaMemsetAsync(s->dstate, 0, sizeof(DevState), s->stream));
   CU(s, cudaMemsetAsync(s->resid, 0, (size_t)(s->opt.llg_max_iter + 2) * 8, s->stream));
@@ -905,6 +1034,10 @@ int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const in
       return fail(s, FDTD_LLG_EINVAL, "source box outside the grid or empty on axis %d", d);
     nb *= (size_t)(hi[d] - lo[d]);
   }
+  if (s->has_pml && kind != FDTD_LLG_SRC_SOFT_E)
+    for (int d = 0; d < 3; ++d)
+      if (lo[d] < s->opt.pml[2 * d] || hi[d] > s->g.n[d] - s->opt.pml[2 * d + 1])
+        return fail(s, FDTD_LLG_EINVAL, "hard / soft field sources must lie outside the PML");
   SourceP &S = s->src.s[s->src.count];
   S.kind = kind;
   S.comp = comp;

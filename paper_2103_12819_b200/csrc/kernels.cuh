@@ -703,6 +703,116 @@ __global__ void k_box_source(const __grid_constant__ BoxSrcArgs a) {
   }
 }
 
+// ------------------------------------------------------------------ open boundary (PML)
+// PAPER.md:189 (reading A26): split-field PML with two-step time-centred multiplicative
+// damping.  In the layer (the outermost cells of a PEC-backed axis) every component is the sum of
+// two parts, one per term of the curl; each part is advanced by the macroscopic update (eq. 11
+// with the local eps, sigma; eq. 21 with M = 0 and the local mu) between two multiplications by
+// the square root g of its damping factor, g taken along the axis of the derivative in that term
+// (dE: E parts at the nodes of that axis, one step; dH: H parts at the half positions, one half
+// step).  These kernels run on the layer's slabs AFTER the regular update of the whole grid and
+// overwrite the total fields there (every update is out of place, so they see the same inputs).
+struct PmlArgs {
+  GridP g;
+  BoxP box;             // one slab of the layer
+  const double *In[3];  // the OTHER field: H^{n+1/2} for the E update, E for the H half-step
+  double *Out[3];       // total field of this update's result set
+  double *P[6];         // split parts of the updated field: [2 * component + part]
+  const double *d[3];   // sqrt damping factors along x, y, z (dE or dH), n[a] entries each
+  const double *eps_r, *sigma, *mu_r;  // cell-centred arrays or nullptr (uniform)
+  double eps_u, sigma_u, mu_u;
+  SourcesP src;         // soft E sources (E update only)
+  const DevState *st;
+};
+
+template <int D>
+__device__ __forceinline__ double pml_e_edge(const PmlArgs &a, int c, const int idx[3], bool wall, double J) {
+  constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
+  const int s1 = stride_of<d1>(a.g), s2 = stride_of<d2>(a.g);
+  double eps = a.eps_u, sig = a.sigma_u;
+  if (a.eps_r)
+    eps = kEps0 * (0.25 * ((__ldg(a.eps_r + c) + __ldg(a.eps_r + c - s1)) +
+                           (__ldg(a.eps_r + c - s2) + __ldg(a.eps_r + c - s1 - s2))));
+  if (a.sigma)
+    sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c - s1)) +
+                  (__ldg(a.sigma + c - s2) + __ldg(a.sigma + c - s1 - s2)));
+  const double t0 = (__ldg(a.In[d2] + c) - __ldg(a.In[d2] + c - s1)) * a.g.rd[d1];
+  const double t1 = -(__ldg(a.In[d1] + c) - __ldg(a.In[d1] + c - s2)) * a.g.rd[d2];
+  const double den = 0.5 * sig + eps / a.g.dt, keep = eps / a.g.dt - 0.5 * sig;
+  const double g0 = __ldg(a.d[d1] + idx[d1]), g1 = __ldg(a.d[d2] + idx[d2]);
+  double p0 = (t0 + keep * (g0 * a.P[2 * D][c]) - J) / den * g0;
+  double p1 = (t1 + keep * (g1 * a.P[2 * D + 1][c])) / den * g1;
+  if (wall) p0 = p1 = 0.0;
+  a.P[2 * D][c] = p0;
+  a.P[2 * D + 1][c] = p1;
+  return p0 + p1;
+}
+
+template <int D>
+__device__ __forceinline__ double pml_h_face(const PmlArgs &a, int c, const int idx[3], bool wall) {
+  constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
+  const int s1 = stride_of<d1>(a.g), s2 = stride_of<d2>(a.g);
+  double mu = a.mu_u;
+  if (a.mu_r) mu = kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + c - stride_of<D>(a.g))));
+  const double t0 = (__ldg(a.In[d2] + c + s1) - __ldg(a.In[d2] + c)) * a.g.rd[d1];
+  const double t1 = -(__ldg(a.In[d1] + c + s2) - __ldg(a.In[d1] + c)) * a.g.rd[d2];
+  const double k = 0.5 * a.g.dt / mu;
+  const double g0 = __ldg(a.d[d1] + idx[d1]), g1 = __ldg(a.d[d2] + idx[d2]);
+  double p0 = (g0 * a.P[2 * D][c] - k * t0) * g0;
+  double p1 = (g1 * a.P[2 * D + 1][c] - k * t1) * g1;
+  if (wall) p0 = p1 = 0.0;
+  a.P[2 * D][c] = p0;
+  a.P[2 * D + 1][c] = p1;
+  return p0 + p1;
+}
+
+template <bool IS_E>
+__global__ void __launch_bounds__(NTHREADS) k_pml(const __grid_constant__ PmlArgs a) {
+  for (int it = blockIdx.x; it < a.box.items; it += gridDim.x) {
+    const Item w = decode_item(a.box, it);
+    if (!w.active) continue;
+    const Column col = make_column(a.g, w.i, w.j);
+    int c = a.g.org + w.i + a.g.sy * w.j + a.g.sz * w.k0;
+    for (int k = w.k0; k < w.k1; ++k, c += a.g.sz) {
+      const int idx[3] = {w.i, w.j, k};
+      const bool wk = wall_k(a.g, k);
+      double v0, v1, v2;
+      if (IS_E) {
+        // soft E sources reach the layer through part 0 (source_term reads EArgs-like fields)
+        double J0 = 0.0, J1 = 0.0, J2 = 0.0;
+        for (int q = 0; q < a.src.count; ++q) {
+          const SourceP &S = a.src.s[q];
+          if (S.kind != 0) continue;
+          if (w.i < S.lo[0] || w.i >= S.hi[0] || w.j < S.lo[1] || w.j >= S.hi[1] || k < S.lo[2] || k >= S.hi[2])
+            continue;
+          double pr = 1.0;
+          if (S.profile) {
+            const long long bx = S.hi[0] - S.lo[0], by = S.hi[1] - S.lo[1];
+            pr = __ldg(S.profile + (w.i - S.lo[0]) + bx * ((w.j - S.lo[1]) + by * (long long)(k - S.lo[2])));
+          }
+          const double J = a.st->src_amp[q] * pr;
+          if (S.comp == 0) J0 += J; else if (S.comp == 1) J1 += J; else J2 += J;
+        }
+        v0 = pml_e_edge<0>(a, c, idx, col.wall[1] || wk, J0);
+        v1 = pml_e_edge<1>(a, c, idx, wk || col.wall[0], J1);
+        v2 = pml_e_edge<2>(a, c, idx, col.wall[0] || col.wall[1], J2);
+      } else {
+        v0 = pml_h_face<0>(a, c, idx, col.wall[0]);
+        v1 = pml_h_face<1>(a, c, idx, col.wall[1]);
+        v2 = pml_h_face<2>(a, c, idx, wk);
+      }
+      a.Out[0][c] = v0;
+      a.Out[1][c] = v1;
+      a.Out[2][c] = v2;
+      if (col.edge_ij || edge_k(a.g, k)) {
+        store_images_inl(a.Out[0], a.g, w.i, w.j, k, c, v0);
+        store_images_inl(a.Out[1], a.g, w.i, w.j, k, c, v1);
+        store_images_inl(a.Out[2], a.g, w.i, w.j, k, c, v2);
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------ set-up kernels
 
 __device__ __forceinline__ Cell make_cell(const GridP &g, int i, int j, int k) {

@@ -121,6 +121,9 @@ class Workload:
     H: list = field(default_factory=lambda: [None, None, None])
     M_cell: list = field(default_factory=lambda: [None, None, None])
     sources: list = field(default_factory=list)
+    pml: Optional[tuple] = None     # (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi) cells of the open boundary layer
+    pml_r0: Optional[float] = None
+    pml_order: Optional[int] = None
     seed: int = BASE_SEED
     notes: str = ""
 

@@ -20,7 +20,8 @@ def oracle_from_workload(w, kind="f64", time_scheme=0) -> Oracle:
                Ms=m.get("Ms"), alpha=m.get("alpha"), gamma=m.get("gamma"),
                bc=w.bc, enable_llg=w.enable_llg, h_bias=w.h_bias, ani_hk=w.ani_hk,
                ani_axis=w.ani_axis, llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, kind=kind,
-               time_scheme=time_scheme)
+               time_scheme=time_scheme, pml=getattr(w, "pml", None),
+               **{k: getattr(w, k) for k in ("pml_r0", "pml_order") if getattr(w, k, None) is not None})
     o.set_fields(a["E"], a["H"], a["M_cell"])
     for s in w.sources:
         prof = None if s.profile is None else s.profile.detach().cpu().numpy()

@@ -39,7 +39,7 @@ def test_header_structs_match_binding(B):
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
     for cname, mirror in (("fdtd_llg_options", B.Options), ("fdtd_llg_stats", B.Stats)):
         body = re.search(r"typedef struct \{([^{}]*)\} %s;" % cname, txt).group(1)
-        fields = re.findall(r"\b([a-z_]+)(?:\[\d\])?\s*;", body)
+        fields = re.findall(r"\b([a-z_][a-z_0-9]*)(?:\[\d\])?\s*;", body)
         assert fields == [f for f, _ in mirror._fields_], cname
 
 
