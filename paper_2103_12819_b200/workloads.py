@@ -339,6 +339,28 @@ def paper_convergence_test(n: int, steps: int, device="cpu") -> Workload:
     return w
 
 
+def paper_air_waveguide(nx=512, ny=4, nz=512, npml=16, device="cpu") -> Workload:
+    """The paper's first validation device (Fig. 4a): air-filled X-band
+    rectangular waveguide, W = 14.95 mm (x), h = 10.16 mm (y), 500 mm long (z) on 512 x 4 x 512
+    cells, CFL 0.8; PEC side walls and PEC at z = +L/2 where a surface current "directly added on
+    top of the H field" launches the TE10 mode towards -z (eq. 31: f0 = 10.5 GHz, T_p one period,
+    centred at 3 T_p).  Readings: the excitation is a HARD source on the tangential Hx faces next to
+    the wall, H_x = I(t) cos(pi x / W) with x measured from the guide axis (the TE10 profile; the
+    printed shape function cos(2 pi x / (W/2)) is not that mode: taken as garbled); the far end is
+    closed by the open boundary (npml cells)."""
+    W, h, L = 14.95e-3, 10.16e-3, 500e-3
+    dx, dy, dz = W / nx, h / ny, L / nz
+    w = Workload("paper_air_waveguide", nx, ny, nz, dx, dy, dz, courant_dt(0.8, dx, dy, dz),
+                 (PEC, PEC, PEC), 80000, enable_llg=False)
+    w.pml = (0, 0, 0, 0, npml, 0)
+    f0 = 10.5e9
+    tp = 1.0 / f0
+    x = -W / 2 + torch.arange(nx, device=device, dtype=torch.float64) * dx     # Hx faces sit at x_i
+    prof = torch.cos(math.pi * x / W).view(1, 1, nx).expand(1, ny, nx).contiguous()
+    w.sources = [Source(0, (0, 0, nz - 1), (nx, ny, nz), 1.0, f0, 3.0 * tp, tp, prof, 3)]
+    return w
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 # shapes the oracle finishes in seconds: several tiles of the kernels plus a ragged tail
