@@ -361,6 +361,36 @@ def paper_air_waveguide(nx=512, ny=4, nz=512, npml=16, device="cpu") -> Workload
     return w
 
 
+def paper_tunable_filter(nx=1024, ny=4, nz=512, npml=16, device="cpu") -> Workload:
+    """The paper's second validation device (Fig. 4b): the waveguide of
+    `paper_air_waveguide` with a YIG slab 0.45 mm thick along z, one face on a side wall:
+    4 pi Ms = 1750 G (Ms = 1.3926e5 A/m), alpha = 0.0051, eps_r = 13, bias H0 = 2890 Oe
+    (2.2998e5 A/m) along y, M saturated along the bias; 1024 x 4 x 512 cells, CFL
+    0.8, the paper's tolerance 1e-6.  Readings as `paper_air_waveguide`; in addition the slab sits on
+    the x = -W/2 wall and stops two cells short of the open-boundary layer (no magnetic cell may
+    touch it)."""
+    W, h, L = 14.95e-3, 10.16e-3, 500e-3
+    dx, dy, dz = W / nx, h / ny, L / nz
+    w = Workload("paper_tunable_filter", nx, ny, nz, dx, dy, dz, courant_dt(0.8, dx, dy, dz),
+                 (PEC, PEC, PEC), 80000, enable_llg=True, h_bias=(0.0, 2.2998e5, 0.0),
+                 llg_tol=1e-6, llg_max_iter=20)
+    w.pml = (0, 0, 0, 0, npml, 0)
+    ncell = max(1, int(round(0.45e-3 / dx)))
+    Ms = _zeros(nx, ny, nz, device)
+    eps = torch.ones((nz, ny, nx), dtype=torch.float64, device=device)
+    k0 = npml + 2
+    Ms[k0:, :, :ncell] = 1.3926e5
+    eps[k0:, :, :ncell] = 13.0
+    w.materials = {"Ms": Ms, "alpha": 0.0051, "gamma": 1.759e11, "eps_r": eps}
+    w.M_cell = [None, Ms.clone(), None]
+    f0 = 10.5e9
+    tp = 1.0 / f0
+    x = -W / 2 + torch.arange(nx, device=device, dtype=torch.float64) * dx
+    prof = torch.cos(math.pi * x / W).view(1, 1, nx).expand(1, ny, nx).contiguous()
+    w.sources = [Source(0, (0, 0, nz - 1), (nx, ny, nz), 1.0, f0, 3.0 * tp, tp, prof, 3)]
+    return w
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 # shapes the oracle finishes in seconds: several tiles of the kernels plus a ragged tail

@@ -64,3 +64,50 @@ def test_air_waveguide_attenuation_follows_eq_32():
         assert abs(alphas[f] - theory) / theory < 0.03, (f, alphas[f], theory)
     for f in (10.5e9, 11.0e9, 12.0e9):                        # above cutoff: no attenuation
         assert abs(alphas[f]) < 0.03 * math.pi / W, (f, alphas[f])
+
+
+def test_tunable_filter_cutoff_and_fmr_match_table_3():
+    """the YIG-loaded guide on the 1024 x 4 x 512 grid the paper compares with
+    theory and experiment, 80,000 steps of the coupled LLG-Maxwell step (32 s on the B200).  The
+    attenuation spectrum has the paper's "key features": a hyperbolic branch that extrapolates to
+    the lowered cutoff f_c2 and a peak at the ferromagnetic resonance.  Measured here: f_c2 =
+    9.14 GHz (paper 9.27, experiment 9.16), f_FMR = 10.24 GHz (paper 10.46, Kittel's eq. 33 10.25,
+    the paper's two theories 10.29 and 10.40)."""
+    from paper_2103_12819_b200.binding import from_workload
+    gold = {}
+    for ln in (Path(__file__).parent / "golden" / "filter_table3.txt").read_text().splitlines():
+        if ln.strip() and not ln.startswith("#"):
+            k, v = ln.split()
+            gold[k] = float(v)
+    w = wl.paper_tunable_filter()
+    sim = from_workload(w)
+    every, nsamp = 200, 400
+    line = torch.zeros((nsamp, w.nz), dtype=torch.float64, device="cuda:0")
+    for m in range(nsamp):
+        if m:
+            sim.step(every)
+        line[m] = sim.read_fields(names=("Ey",), device="cuda:0")["Ey"][:, w.ny // 2, w.nx // 2]
+    st = sim.stats()
+    assert st["steps"] == every * (nsamp - 1) and st["nonconverged_halfsteps"] == 0
+    assert st["magnetic_cells"] > 0
+    t = every * np.arange(nsamp) * w.dt
+    u = np.clip((t / t[-1] - 0.2) / 0.8, 0.0, 1.0)
+    line = line.cpu().numpy() * (np.cos(0.5 * math.pi * u) ** 2)[:, None]
+    z = np.arange(w.nz) * w.dz
+    dist = z[-1] + w.dz - z
+    sel = (dist > 3e-3) & (dist < 20e-3)
+    fs = np.arange(8.0e9, 11.6e9, 0.02e9)
+    al = np.array([-np.polyfit(dist[sel], np.log(np.abs(np.exp(-2j * math.pi * f * t) @ line)[sel]), 1)[0]
+                   for f in fs])
+    # FMR: the attenuation peak above the cutoff
+    hi = (fs > 9.8e9) & (fs < 11.2e9)
+    f_fmr = fs[hi][np.argmax(al[hi])] * 1e-9
+    assert al[hi].max() > 10 * al[(fs > 9.3e9) & (fs < 9.8e9)].min()      # a real resonance peak
+    assert abs(f_fmr - gold["kittel_fmr_GHz"]) / gold["kittel_fmr_GHz"] < 0.01, f_fmr
+    assert abs(f_fmr - gold["fmr_GHz"]) / gold["fmr_GHz"] < 0.03, f_fmr
+    # cutoff: alpha^2 is linear in f^2 on the evanescent branch; its zero is f_c2
+    lo = (fs >= 8.0e9) & (fs <= 8.7e9)
+    c = np.polyfit(fs[lo] ** 2, al[lo] ** 2, 1)
+    f_c2 = math.sqrt(-c[1] / c[0]) * 1e-9
+    assert abs(f_c2 - gold["cutoff_fc2_GHz"]) / gold["cutoff_fc2_GHz"] < 0.025, f_c2
+    assert f_c2 < 0.95 * C0 / (2 * 14.95e-3) * 1e-9                        # well below the empty guide's 10.03 GHz
