@@ -259,8 +259,7 @@ def run_ours(args):
              "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
              "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
     extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
-    uniform_agm = not any(mask & MAT_BITS[m] for m in ("alpha", "gamma", "mu_r"))   # the staged sweeps' condition
-    words = WORDS_LEAN if (args.kernel_path == 4 and st["magnetic_cells"] and uniform_agm) else WORDS
+    words = WORDS_LEAN if (args.kernel_path == 4 and st["staged_sweeps"]) else WORDS
     if words is WORDS and "hm_second" in prof:   # r = 2 and r >= 3 are the same kernel: one class
         prof = dict(prof)
         a2, b2 = prof.pop("hm_second"), prof["hm_iter"]
@@ -285,7 +284,7 @@ def run_ours(args):
     timed = [c for c in per_class if "alg_GBps" in per_class[c]]
     dom = max(timed, key=lambda c: per_class[c]["ms_total"])
     lean = words is WORDS_LEAN
-    staged = args.kernel_path in (0, 3, 4) and st["magnetic_cells"] and uniform_agm
+    staged = bool(st["staged_sweeps"])
     dom_kernel = {"h_update": "k_h_update",
                   "hm_first": "k_hm_stage<FIRST_H>" if lean else "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
                   "hm_second": "k_hm_stage<ITER_RE>" if lean else "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",

@@ -73,10 +73,12 @@ typedef struct {
                          in HOST memory, the uniform value (no nx*ny*nz array needed)            */
   int kernel_path;    /* which LLG sweep kernel runs (same arithmetic in all: bitwise-equal results).
                          0 (default): staged sweep, tile 32x16 (TMA-fed shared-memory ring for the
-                         neighbour operands) wherever it applies (alpha, gamma, mu_r uniform);
-                         1: direct-load kernels everywhere; 3: staged sweep, tile 32x7, two blocks
-                         per SM; 4: staged sweep that never writes M^1 (r = 1 stores H^1 only, r = 2
-                         recomputes M^1: 18 words/cell less traffic, one more LLG evaluation)     */
+                         neighbour operands) where it applies (alpha, gamma, mu_r uniform) and the
+                         sweep box gives every SM a work item, else the direct-load kernels;
+                         1: direct-load kernels everywhere; 5: staged 32x16 whatever the box size;
+                         3: staged sweep, tile 32x7, two blocks per SM; 4: staged sweep that never
+                         writes M^1 (r = 1 stores H^1 only, r = 2 recomputes M^1: 18 words/cell less
+                         traffic, one more LLG evaluation; equal to rounding).  1, 3-5: A/B checks  */
   int time_scheme;    /* 0 (default): the second-order scheme, iterated trapezoidal LLG;
                          1: the first-order scheme: one forward-Euler sweep of
                          eq. 7 / 12 per (H,M) half-step (advancing dt/2), N(M), then eq. 9 / 14;
@@ -108,6 +110,9 @@ typedef struct {
                                        cells + 1 halo cell), what one k_hm_sweep launch covers  */
   unsigned material_array_mask;     /* FDTD_LLG_MAT_* bits of the materials kept as device arrays
                                        (a uniform map is folded into a scalar)                  */
+  int staged_sweeps;                /* 1: the LLG iterates r <= 3 run the staged kernel (hm_stage.cuh);
+                                       0: the direct-load kernel (general materials, kernel_path 1,
+                                       or a sweep box too small to give every SM a work item)   */
 } fdtd_llg_stats;
 
 /* kernel classes of fdtd_llg_step_timed */

@@ -412,7 +412,8 @@ int array_index(const fdtd_llg *s, const double *p) { return (int)((p - s->E[0])
 
 // SW x by columns marched over kz planes; a persistent grid of `grid` blocks draws the items
 // dynamically.  kz: as long as possible (every item loads one extra stage) while leaving >= 24
-// items per block, so that the last items of the sweep are a small fraction of it; >= 32 planes.
+// items per block, so that the last items of the sweep are a small fraction of it; >= 32 planes
+// (>= 16 on boxes too small to give every block two items).
 StBox make_stbox(const int lo[3], const int hi[3], int by, int grid) {
   StBox b{};
   for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
@@ -422,6 +423,7 @@ StBox make_stbox(const int lo[3], const int hi[3], int by, int grid) {
   const long long cols = (long long)b.ntx * b.nty;
   int nc = 1;
   while (cols * nc < 24LL * grid && (ez + nc) / (nc + 1) >= 32) ++nc;
+  while (cols * nc < 2LL * grid && (ez + nc) / (nc + 1) >= 16) ++nc;  // small boxes: shorter items
   b.kz = (ez + nc - 1) / nc;
   b.items = (int)(cols * ((ez + b.kz - 1) / b.kz));
   return b;
@@ -460,6 +462,10 @@ int setup_hm_stage_by(fdtd_llg *s) {
   if ((rc = make_map(s, &s->mapT, SROW, BY + 1, 1))) return rc;
   if ((rc = make_map(s, &s->mapPM, SW, BY, 9))) return rc;
   s->st_box = make_stbox(s->lo, s->hi, BY, s->num_sms * StLayout<BY, true, true>::BPS);
+  // A sweep box that cannot give every SM an item (a thin slab, a small grid) is latency bound:
+  // the direct-load kernels with their 32 x 8 x 16 blocks fill the GPU better there (32^3: 9 us
+  // against 79 us per sweep; the bits are the same).
+  if (s->opt.kernel_path == 0 && s->st_box.items < s->num_sms) s->stage_by = 0;
   return FDTD_LLG_OK;
 }
 
@@ -928,7 +934,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
   if ((rc = setup_pml(s, &q))) return bail(rc);
   const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
-  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 || opt->kernel_path == 4 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
+  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 || opt->kernel_path == 4 || opt->kernel_path == 5 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
   s->stage_lean = opt->kernel_path == 4;
   if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
   if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
@@ -1173,6 +1179,7 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   out->material_array_mask = (s->eps_r.is_array ? 1u : 0) | (s->sigma.is_array ? 2u : 0) |
                              (s->mu_r.is_array ? 4u : 0) | (s->Ms.is_array ? 8u : 0) |
                              (s->alpha.is_array ? 16u : 0) | (s->gamma.is_array ? 32u : 0);
+  out->staged_sweeps = s->stage_by != 0;
   out->sweep_cells = 0;
   if (s->llg) {
     out->sweep_cells = 1;

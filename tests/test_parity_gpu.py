@@ -52,8 +52,17 @@ def _assert_parity(got, ref, llg, tol=TOL):
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
 def test_parity_100_steps_all_configs(cfg):
+    """On these shapes the default kernel_path picks the direct-load sweeps (the box is too small
+    to give every SM an item); the staged sweeps are forced with kernel_path 5 below and run by
+    default at the sizes of test_fullsize_gpu.py and of the every-SM-busy test."""
     w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
     got, ref, gs, os_ = _run_both(w, 100)
+    if w.enable_llg:
+        from paper_2103_12819_b200.binding import from_workload
+        sim = from_workload(w, kernel_path=5)
+        assert sim.stats()["staged_sweeps"] == 1 and gs["staged_sweeps"] == 0
+        sim.step(100)
+        _assert_parity(_gpu_fields(sim), ref, True)
     _assert_parity(got, ref, w.enable_llg)
     assert gs["steps"] == 100
     if w.enable_llg:
@@ -121,7 +130,7 @@ def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
 @pytest.mark.parametrize("cfg,shape", [(1, (32, 32, 32)), (4, (44, 36, 40)), (5, (40, 44, 36)),
                                        (5, (70, 19, 23)), (4, (33, 8, 50))])
 def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
-    """kernel_path 0 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell) and 1 (direct
+    """kernel_path 5 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell) and 1 (direct
     global loads) share the arithmetic (hm_face_core); 4 (staged, M^1 recomputed at r = 2 instead
     of stored) agrees to rounding:
     every field and the iteration counts agree bit for bit, on shapes with ragged tiles in x and
@@ -129,12 +138,13 @@ def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(cfg, shape=shape)
     outs, stats = [], []
-    for path in (1, 0, 3, 4):
+    for path in (1, 5, 3, 4):
         sim = from_workload(w, kernel_path=path)
+        assert sim.stats()["staged_sweeps"] == (path != 1)
         sim.step(25)
         outs.append(_gpu_fields(sim))
         stats.append(sim.stats())
-    for path, other, st in zip((0, 3, 4), outs[1:], stats[1:]):
+    for path, other, st in zip((5, 3, 4), outs[1:], stats[1:]):
         if path == 4:
             _assert_close_to_rounding(other, outs[0])
         else:
@@ -178,7 +188,7 @@ def test_early_stop_after_one_or_two_iterates_on_every_kernel_path(tol, iters):
     ref = o.read_fields()
     assert int(o.stats()["iters_total"]) == 40 * iters
     outs = []
-    for path in (1, 0, 3, 4):
+    for path in (1, 5, 3, 4):
         sim = from_workload(w, kernel_path=path)
         sim.step(20)
         outs.append(_gpu_fields(sim))
@@ -201,7 +211,7 @@ def test_first_order_scheme_parity_100_steps(cfg):
     o.step(100)
     ref = o.read_fields()
     outs = []
-    for path in (0, 1, 3):
+    for path in (5, 1, 3):
         sim = from_workload(w, kernel_path=path, time_scheme=1)
         sim.step(100)
         outs.append(_gpu_fields(sim))
