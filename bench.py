@@ -56,7 +56,8 @@ def _parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5 (6: the paper's weak-scaling base case, "
+                         "the tunable filter on 1024x4x512 cells)")
     ap.add_argument("--shape", default=None, help="nx,ny,nz (default: the config's full size)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -583,7 +583,7 @@ __device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, doubl
     sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c - s1)) +
                   (__ldg(a.sigma + c - s2) + __ldg(a.sigma + c - s1 - s2)));
   const double curl = (h2 - h2m) * a.g.rd[d1] - (h1 - h1m) * a.g.rd[d2];
-  const double edt = eps / a.g.dt, hs = 0.5 * sig;
+  const double edt = eps * (1.0 / a.g.dt), hs = 0.5 * sig;  // 1/dt is loop invariant: one division per edge
   const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
   return wall ? 0.0 : e1;
 }

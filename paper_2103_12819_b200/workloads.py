@@ -391,7 +391,15 @@ def paper_tunable_filter(nx=1024, ny=4, nz=512, npml=16, device="cpu") -> Worklo
     return w
 
 
-CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+def config6(shape=(1024, 4, 512), device="cpu", steps=80000) -> Workload:
+    """Not a BASELINE.json config: the paper's own weak-scaling base case (the
+    tunable filter on 1024 x 4 x 512 cells per GPU), for `bench.py --config 6`."""
+    w = paper_tunable_filter(shape[0], shape[1], shape[2], device=device)
+    w.steps = steps
+    return w
+
+
+CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5, 6: config6}
 
 # shapes the oracle finishes in seconds: several tiles of the kernels plus a ragged tail
 SMALL_SHAPES = {1: (32, 32, 32), 2: (40, 36, 28), 3: (72, 40, 36), 4: (44, 36, 40),
