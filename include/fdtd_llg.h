@@ -105,7 +105,8 @@ typedef struct {
   double courant;                   /* dt / vacuum Courant limit (>1 is allowed, not an error) */
   long long kernel_launches;        /* kernels this handle has launched in fdtd_llg_step       */
   long long magnetic_cells;         /* cells with Ms > 0 (0 when LLG is disabled)              */
-  int launches_per_step;            /* kernel nodes in one captured step                       */
+  int launches_per_step;            /* kernel nodes one captured step launches (the LLG iterates
+                                       r >= 4 sit in a conditional node and are not counted)   */
   long long sweep_cells;            /* cells of the LLG sweep box (bounding box of the magnetic
                                        cells + 1 halo cell), what one k_hm_sweep launch covers  */
   unsigned material_array_mask;     /* FDTD_LLG_MAT_* bits of the materials kept as device arrays

@@ -92,6 +92,8 @@ struct fdtd_llg {
   int *r_hist = nullptr;  // device: iteration count R of half-step h at [h % R_HIST]
 
   cudaGraphExec_t graph[2] = {nullptr, nullptr};  // one captured step per E parity
+  bool capturing = false;        // inside build_graph: the rarely needed iterates go into an IF node
+  cudaStream_t aux = nullptr;    // captures the body of that node
   bool graph_valid[2] = {false, false};
   int launches_per_step = 0;
   long long kernel_launches = 0;
@@ -587,10 +589,48 @@ int launch_sweep(fdtd_llg *s, const HMArgs &a, int grid) {
   return FDTD_LLG_OK;
 }
 
+// The launches from here to end_cond_tail are captured into the body of an IF node of the step's
+// graph; k_set_cond arms it when iterate r_next - 1 ran and missed the tolerance.
+int begin_cond_tail(fdtd_llg *s, int r_next, cudaStream_t *outer) {
+  cudaStreamCaptureStatus st;
+  cudaGraph_t g = nullptr;
+  const cudaGraphNode_t *deps = nullptr;
+  size_t nd = 0;
+  CU(s, cudaStreamGetCaptureInfo_v2(s->stream, &st, nullptr, &g, &deps, &nd));
+  if (st != cudaStreamCaptureStatusActive || !g) return fail(s, FDTD_LLG_ESTATE, "begin_cond_tail outside a capture");
+  cudaGraphConditionalHandle h;
+  CU(s, cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault));
+  k_set_cond<<<1, 1, 0, s->stream>>>(h, s->resid, s->opt.llg_tol, r_next);
+  CU(s, cudaGetLastError());
+  CU(s, cudaStreamGetCaptureInfo_v2(s->stream, &st, nullptr, &g, &deps, &nd));
+  cudaGraphNodeParams np{};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = h;
+  np.conditional.type = cudaGraphCondTypeIf;
+  np.conditional.size = 1;
+  cudaGraphNode_t node;
+  CU(s, cudaGraphAddNode(&node, g, deps, nd, &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  CU(s, cudaStreamUpdateCaptureDependencies(s->stream, &node, 1, cudaStreamSetCaptureDependencies));
+  CU(s, cudaStreamBeginCaptureToGraph(s->aux, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+  *outer = s->stream;
+  s->stream = s->aux;
+  return FDTD_LLG_OK;
+}
+
+int end_cond_tail(fdtd_llg *s, cudaStream_t outer) {
+  cudaGraph_t body = nullptr;
+  cudaError_t e = cudaStreamEndCapture(s->aux, &body);
+  s->stream = outer;
+  if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaStreamEndCapture (IF body): %s", cudaGetErrorString(e));
+  return FDTD_LLG_OK;
+}
+
 // (H,M) half-step: time-n set `in`, result in set `out`, `tmp` is the other Jacobi buffer.
 // M: time-n set `min`, result in set `mout`.
 int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int min, int mout, bool last,
                  int *launches) {
+  int *const launches_outer = launches;
   const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
@@ -631,7 +671,18 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     a.euler = s->opt.time_scheme == 1;
     a.resid = s->resid;
     a.pipe_error = &s->dstate->pipe_error;
+    cudaStream_t outer = nullptr;  // set while the launches go into the body of the IF node
+    int body_launches = 0;
     for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
+      // Iterates r >= 4 almost never run.  In the captured step they sit in ONE conditional (IF)
+      // node armed on the device by k_set_cond, so the usual step does not even launch them.
+      // (The node itself costs about as much as ten empty launches: only worth it for a long tail.)
+      if (r == 4 && s->capturing && s->aux && s->opt.llg_max_iter >= 12) {
+        int rc = begin_cond_tail(s, r, &outer);
+        if (rc) return rc;
+        ++*launches;  // k_set_cond
+        launches = &body_launches;
+      }
       // r <= 3 normally run: one block per item.  Later iterates almost never run: a small
       // persistent grid keeps their early exit at launch-latency cost.
       const int grid = grid_for(s, a.box, r <= 3 ? 0 : s->sweep_blocks_per_sm);
@@ -679,6 +730,11 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
       prof_end(s);
       if (rc) return rc;
       ++*launches;
+    }
+    if (outer) {
+      launches = launches_outer;
+      int rc = end_cond_tail(s, outer);
+      if (rc) return rc;
     }
   }
   prof_begin(s, FDTD_LLG_K_OTHER, 0);
@@ -784,7 +840,9 @@ int build_graph(fdtd_llg *s, int par) {
   cudaGraph_t g = nullptr;
   CU(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
   int launches = 0;
+  s->capturing = true;
   int rc = enqueue_step(s, par, &launches);
+  s->capturing = false;
   cudaError_t e = cudaStreamEndCapture(s->stream, &g);
   if (rc) { if (g) cudaGraphDestroy(g); return rc; }
   if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
@@ -883,6 +941,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   if (!opt->enable_llg) { s->opt.llg_max_iter = 1; s->opt.llg_tol = 1.0; }
   if (opt->time_scheme == 1) s->opt.llg_max_iter = 1;  // explicit: one sweep per half-step, no iteration
   s->stream = static_cast<cudaStream_t>(cuda_stream);
+  if (cuda_stream && cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking) != cudaSuccess) s->aux = nullptr;
   if (!cuda_stream) s->opt.use_graph = 0;  // the legacy default stream cannot be captured
   s->ws = static_cast<char *>(dev_workspace);
   s->ws_bytes = workspace_bytes;
@@ -1196,6 +1255,7 @@ void fdtd_llg_destroy(fdtd_llg *s) {
   if (!s) return;
   for (int p = 0; p < 2; ++p)
     if (s->graph[p]) cudaGraphExecDestroy(s->graph[p]);
+  if (s->aux) cudaStreamDestroy(s->aux);
   delete s;
 }
 

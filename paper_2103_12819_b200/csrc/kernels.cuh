@@ -500,6 +500,14 @@ __global__ void __launch_bounds__(NTHREADS) k_hm_sweep(const __grid_constant__ H
   }
 }
 
+// 1 thread: arm the conditional graph node that holds the iterates r >= r_next: they are needed
+// only if iterate r_next - 1 ran and missed the tolerance
+__global__ void k_set_cond(cudaGraphConditionalHandle h, const unsigned long long *resid, double tol,
+                           int r_next) {
+  const double res = __longlong_as_double((long long)resid[r_next - 1]);
+  cudaGraphSetConditional(h, res < tol ? 0u : 1u);
+}
+
 // 1 thread: close an (H,M) half-step
 __global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, int *r_hist, int max_iter,
                            double tol, int any_magnetic, int last_of_step) {
