@@ -66,6 +66,9 @@ def _parse():
     ap.add_argument("--kernel-path", type=int, default=0,
                     help="fdtd_llg_options.kernel_path: 0 = staged sweeps (default), 1 = direct-load kernels, "
                          "3 = staged 32x7 tiles, 4 = staged + M^1 recomputed (fewer bytes, more flops)")
+    ap.add_argument("--plain-graph", action="store_true",
+                    help="capture the step without the conditional node (use_graph = 2), so that ncu lists "
+                         "the kernels of the replayed steps too")
     ap.add_argument("--time-scheme", type=int, default=0,
                     help="0 = second-order scheme (the BASELINE metric), 1 = first-order scheme (PAPER.md:102-150)")
     return ap.parse_args()
@@ -213,7 +216,8 @@ def run_ours(args):
     w = wl.make_config(args.config, shape=_shape(args), device=dev)
     cells = w.cells
     name = _workload_name(w)
-    sim = from_workload(w, device=dev, kernel_path=args.kernel_path, time_scheme=args.time_scheme)
+    sim = from_workload(w, device=dev, kernel_path=args.kernel_path, time_scheme=args.time_scheme,
+                        use_graph=2 if args.plain_graph else True)
     stream = sim.stream
 
     # host copies of the initial state for the end-to-end leg (pinned), before the device inputs go

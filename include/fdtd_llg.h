@@ -68,7 +68,9 @@ typedef struct {
   double ani_axis[3]; /* unit vector u                                                            */
   double llg_tol;     /* stop when max |M^r - M^{r-1}|/Ms < tol (paper uses 1e-6)   */
   int llg_max_iter;   /* iteration cap (the paper has none); at the cap the iterate is accepted   */
-  int use_graph;      /* 1 (default): the step is captured once in a CUDA Graph and replayed      */
+  int use_graph;      /* 1 (default): the step is captured once in a CUDA Graph and replayed, the LLG
+                         iterates r >= 4 in a conditional node; 2: the same graph with plain kernel
+                         nodes only (profilers do not look into conditional graphs); 0: no graph  */
   unsigned scalar_material_mask; /* FDTD_LLG_MAT_* bits: that material pointer addresses ONE double
                          in HOST memory, the uniform value (no nx*ny*nz array needed)            */
   int kernel_path;    /* which LLG sweep kernel runs (same arithmetic in all: bitwise-equal results).

@@ -174,7 +174,7 @@ class FdtdLlg:
         opt.ani_hk = float(ani_hk)
         opt.llg_tol = float(llg_tol)
         opt.llg_max_iter = int(llg_max_iter)
-        opt.use_graph = int(bool(use_graph))
+        opt.use_graph = 2 if use_graph == 2 else int(bool(use_graph))   # 2: graph without the conditional node
         opt.kernel_path = int(kernel_path)
         opt.time_scheme = int(time_scheme)
         if pml is not None:

@@ -677,7 +677,7 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
       // Iterates r >= 4 almost never run.  In the captured step they sit in ONE conditional (IF)
       // node armed on the device by k_set_cond, so the usual step does not even launch them.
       // (The node itself costs about as much as ten empty launches: only worth it for a long tail.)
-      if (r == 4 && s->capturing && s->aux && s->opt.llg_max_iter >= 12) {
+      if (r == 4 && s->capturing && s->aux && s->opt.use_graph == 1 && s->opt.llg_max_iter >= 12) {
         int rc = begin_cond_tail(s, r, &outer);
         if (rc) return rc;
         ++*launches;  // k_set_cond
