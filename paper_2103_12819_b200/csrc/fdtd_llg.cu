@@ -66,7 +66,7 @@ struct fdtd_llg {
   // staged sweeps (hm_stage.cuh): kernel_path 0, 4 (tile rows 16) and 3 (tile rows 7)
   int stage_by = 0;  // 0 = not used
   bool stage_lean = false;  // kernel_path 4: M^1 recomputed at r = 2 instead of stored at r = 1
-  StBox st_box{};
+  StBox st_box{}, st_box_first{};  // work items of the iterates r >= 2 / of the r = 1 sweep
   CUtensorMap mapT{}, mapPM{};
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
@@ -412,22 +412,20 @@ int array_index(const fdtd_llg *s, const double *p) { return (int)((p - s->E[0])
 
 // ---- staged sweeps (hm_stage.cuh) ----------------------------------------------------------
 
-// SW x by columns marched over kz planes; a persistent grid of `grid` blocks draws the items
-// dynamically.  kz: as long as possible (every item loads one extra stage) while leaving >= 24
-// items per block, so that the last items of the sweep are a small fraction of it; >= 32 planes
-// (>= 16 on boxes too small to give every block two items).
-StBox make_stbox(const int lo[3], const int hi[3], int by, int grid) {
+// SW x by columns marched over ~kz_target planes; a persistent grid draws the items dynamically in
+// the order x, y, z.  Short items keep the blocks that run at the same time on the same few planes
+// (neighbouring tiles: their rims hit in L2, DRAM pages are shared) and balance the SMs; every
+// item costs one extra stage.  Measured at 768^3: the iterates r >= 2 are fastest at 8-16 planes
+// (14.1 ms at 97, 12.3 ms at 8), the r = 1 sweep at about 32.
+StBox make_stbox(const int lo[3], const int hi[3], int by, int kz_target) {
   StBox b{};
   for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
   b.ntx = (hi[0] - lo[0] + SW - 1) / SW;
   b.nty = (hi[1] - lo[1] + by - 1) / by;
   const int ez = std::max(1, hi[2] - lo[2]);
-  const long long cols = (long long)b.ntx * b.nty;
-  int nc = 1;
-  while (cols * nc < 24LL * grid && (ez + nc) / (nc + 1) >= 32) ++nc;
-  while (cols * nc < 2LL * grid && (ez + nc) / (nc + 1) >= 16) ++nc;  // small boxes: shorter items
+  const int nc = std::max(1, (ez + kz_target / 2) / kz_target);   // chunks of about kz_target planes
   b.kz = (ez + nc - 1) / nc;
-  b.items = (int)(cols * ((ez + b.kz - 1) / b.kz));
+  b.items = (int)((long long)b.ntx * b.nty * ((ez + b.kz - 1) / b.kz));
   return b;
 }
 
@@ -463,7 +461,8 @@ int setup_hm_stage_by(fdtd_llg *s) {
   int rc;
   if ((rc = make_map(s, &s->mapT, SROW, BY + 1, 1))) return rc;
   if ((rc = make_map(s, &s->mapPM, SW, BY, 9))) return rc;
-  s->st_box = make_stbox(s->lo, s->hi, BY, s->num_sms * StLayout<BY, true, true>::BPS);
+  s->st_box_first = make_stbox(s->lo, s->hi, BY, 32);
+  s->st_box = make_stbox(s->lo, s->hi, BY, 8);
   // A sweep box that cannot give every SM an item (a thin slab, a small grid) is latency bound:
   // the direct-load kernels with their 32 x 8 x 16 blocks fill the GPU better there (32^3: 9 us
   // against 79 us per sweep; the bits are the same).
@@ -696,7 +695,7 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
       if (s->stage_by) {
         HMSArgs p{};
         p.a = a;
-        p.tb = s->st_box;
+        p.tb = r == 1 ? s->st_box_first : s->st_box;
         p.mapT = s->mapT; p.mapM = s->mapPM;
         p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
         p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
