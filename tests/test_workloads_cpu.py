@@ -92,10 +92,11 @@ def test_small_configs_have_the_structure_of_the_full_ones(cfg):
 def test_full_size_configs_are_the_baseline_json_ones():
     import inspect
     shapes = {n: inspect.signature(f).parameters["shape"].default for n, f in wl.CONFIGS.items()}
+    # 1-5: BASELINE.json; 6: the paper's own weak-scaling base case, bench only
     assert shapes == {1: (32, 32, 32), 2: (256, 256, 256), 3: (512, 128, 128),
-                      4: (384, 384, 384), 5: (768, 768, 768)}
+                      4: (384, 384, 384), 5: (768, 768, 768), 6: (1024, 4, 512)}
     steps = {n: inspect.signature(f).parameters["steps"].default for n, f in wl.CONFIGS.items()}
-    assert steps == {1: 100, 2: 1000, 3: 2000, 4: 2000, 5: 200}
+    assert steps == {1: 100, 2: 1000, 3: 2000, 4: 2000, 5: 200, 6: 80000}
 
 
 def test_paper_convergence_workload_samples_eqs_22_to_28():
