@@ -10,6 +10,8 @@
  *                                       (H,M)^{n+1/2} -> (H,M)^{n+1} with curl E^{n+1} [Step 3]
  *   each (H,M) half-step is the iterated trapezoidal LLG solve of eqs. 18-21
  *   with |M| = Ms renormalisation and the global stopping test of PAPER.md:154.
+ *   Options add the first-order scheme, hard / soft sources of E and H
+ *    and the open boundary (PML).
  *
  * Plain C types only: pointers (each argument says HOST or DEVICE), sizes, PODs.  No torch types.
  * Every step of the path runs in the library's own CUDA kernels; there is no CPU fallback.
@@ -20,7 +22,8 @@
  *     Hx (i,j+1/2,k+1/2)  Hy (i+1/2,j,k+1/2)  Hz (i+1/2,j+1/2,k)  normal H on faces
  *     M on the x-, y-, z-faces: all three components at every face (9 arrays)
  *     materials eps_r, sigma, mu_r, Ms, alpha, gamma at cell centres
- *   Boundaries per axis: FDTD_LLG_PEC or FDTD_LLG_PERIODIC.  On a PEC axis index 0
+ *   Boundaries per axis: FDTD_LLG_PEC or FDTD_LLG_PERIODIC; a PEC axis can carry
+ *   an absorbing layer in front of its walls (options.pml).  On a PEC axis index 0
  *   is the lower wall, index n (not stored) the upper wall; wall-tangential E, wall-normal H and M on
  *   wall faces are identically 0.
  *
