@@ -658,6 +658,8 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
     a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
     a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
+    a.cf_u = kMu0 * a.gamma_u * s->dt * 0.25;   // the device expression, evaluated once
+    a.kh = s->dt / (2.0 * kMu0);
     a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
     if (s->stage_by && s->Ms.is_array) {  // the most common face value and its reciprocal
       a.Ms_u = s->Ms.maxv;

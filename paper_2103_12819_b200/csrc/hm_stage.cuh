@@ -182,7 +182,7 @@ __device__ __forceinline__ FaceOut s_face(const HMArgs &a, const double *A, cons
   Vec3 he = hn;
   if (!FIRST) he = s_hem<L, L::HP, D>(A, B, t);
   const double C = s_curl<L, D>(a.g, A, B, t);
-  return hm_face_core<D, FIRST, ANISO, RECOMP>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.gamma_u,
+  return hm_face_core<D, FIRST, ANISO, RECOMP>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.cf_u,
                                                a.ch_uniform, wall);
 }
 

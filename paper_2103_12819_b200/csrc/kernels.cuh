@@ -236,6 +236,8 @@ struct HMArgs {
   double *Mr[9];        // M^{r-1} in, M^r out (same thread); FIRST: out only
   const double *Ms, *alpha, *gamma, *mu_r;  // cell-centred arrays or nullptr (uniform)
   double Ms_u, rMs_u, alpha_u, gamma_u, ch_uniform;
+  double cf_u;  // mu0 |gamma_u| dt / 4, the coefficient of eqs. 19-20 when gamma is uniform
+  double kh;    // dt / (2 mu0), the coefficient of curl E in eq. 21
   double hb[3], hk, u[3];
   double tol;
   int euler;  // 1: first-order scheme: the r = 1 sweep is a forward-Euler step
@@ -342,20 +344,19 @@ struct FaceOut {
 // the end.  (A non-magnetic face runs the LLG arithmetic on rMs = 0 and discards it.)
 //   mn = M^n, mp = M^{r-1}, hn / he = H_EM^n / H_EM^{r-1} (own normal component + the two
 //   four-point averages), C = (curl E)_D, Msf / rMs = face Ms and its reciprocal (0 if Msf = 0),
-//   alf, gam = face alpha, |gamma|, ch = dt / (2 mu) of a non-magnetic face.
+//   alf = face alpha, cf = mu0 |gamma_face| dt / 4, ch = dt / (2 mu) of a non-magnetic face.
 // The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces).
 // RECOMP (an iterate r = 2 only): M^1 is not read but recomputed from M^n and H_eff^n -- the very
 // expression the r = 1 sweep evaluated, so the value is the one it would have stored.
 template <int D, bool FIRST, bool ANISO, bool RECOMP = false>
 __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn, const Vec3 &mp_in,
                                                 Vec3 hn, Vec3 he, double C, double Msf, double rMs,
-                                                double alf, double gam, double ch, bool wall) {
+                                                double alf, double cf, double ch, bool wall) {
   Vec3 mp = FIRST ? mn : mp_in;
   const double hn_own = comp<D>(hn), hp_own = comp<D>(he);
 
   // ---- magnetic face: eqs. 18-21
   const bool magnetic = !wall && Msf > 0.0;
-  const double cf = kMu0 * gam * a.g.dt * 0.25;  // mu0 |gamma| dt / 4
   const Vec3 hb = {a.hb[0], a.hb[1], a.hb[2]};
   const Vec3 u = {a.u[0], a.u[1], a.u[2]};
   // H_eff^n = H_EM^n + H_bias + H_k (M^n.u / Ms) u            (A19)
@@ -385,7 +386,7 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
     dM = llg_increment<FIRST>(mn, hn, he, cf, alf * rMs, rMs);
   const Vec3 mr = {mn.x + dM.x, mn.y + dM.y, mn.z + dM.z};
   // eq. 21, normal component:  H^r = H^n + M^n - M^r - (dt / 2 mu0) curl E
-  const double h_mag = hn_own - comp<D>(dM) - (a.g.dt / (2.0 * kMu0)) * C;
+  const double h_mag = hn_own - comp<D>(dM) - a.kh * C;
   // stopping test of PAPER.md:154, per face; reduced by the caller
   const double e = fmax(fmax(fabs(mr.x - mp.x), fabs(mr.y - mp.y)), fabs(mr.z - mp.z));
 
@@ -419,16 +420,17 @@ __device__ __forceinline__ FaceOut hm_face(const HMArgs &a, int c, bool wall, do
   Vec3 he = hn;
   if (!FIRST) he = h_em<D>(a.g, c, a.Hp);
   const double C = curl_e<D>(a.g, c, a.E);
-  double alf = a.alpha_u, gam = a.gamma_u, ch = a.ch_uniform;
+  double alf = a.alpha_u, cf = a.cf_u, ch = a.ch_uniform;
   if (AG_ARR) {
     alf = 0.5 * (__ldg(a.alpha + c) + __ldg(a.alpha + cm));
-    gam = 0.5 * (fabs(__ldg(a.gamma + c)) + fabs(__ldg(a.gamma + cm)));  // |gamma| (eqs. 19-20)
+    const double gam = 0.5 * (fabs(__ldg(a.gamma + c)) + fabs(__ldg(a.gamma + cm)));  // |gamma| (eqs. 19-20)
+    cf = kMu0 * gam * a.g.dt * 0.25;                                                // mu0 |gamma| dt / 4
   }
   if (MU_ARR) ch = a.g.dt / (2.0 * kMu0 * (0.5 * (__ldg(a.mu_r + c) + __ldg(a.mu_r + cm))));
   const double Msf = 0.5 * (Ms_c + Ms_m);
   double rMs = rMs_c;
   if (MS_ARR && Ms_m != Ms_c) rMs = Msf > 0.0 ? 1.0 / Msf : 0.0;
-  return hm_face_core<D, FIRST, ANISO>(a, mn, mp, hn, he, C, Msf, rMs, alf, gam, ch, wall);
+  return hm_face_core<D, FIRST, ANISO>(a, mn, mp, hn, he, C, Msf, rMs, alf, cf, ch, wall);
 }
 
 template <int D>
