@@ -142,8 +142,12 @@ int fail(fdtd_llg *s, int code, const char *fmt, ...) {
 BoxP make_box(const fdtd_llg *s, const int lo[3], const int hi[3]) {
   BoxP b{};
   for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.hi[d] = hi[d]; }
-  b.ntx = (hi[0] - lo[0] + TX - 1) / TX;
-  b.nty = (hi[1] - lo[1] + TY - 1) / TY;
+  // a box with fewer than TY rows (the paper's ny = 4 guides): tiles of 1, 2 or 4 rows, wider in x
+  b.tyr = TY;
+  while (b.tyr > 1 && b.tyr / 2 >= hi[1] - lo[1]) b.tyr /= 2;
+  const int tw = TX * (TY / b.tyr);
+  b.ntx = (hi[0] - lo[0] + tw - 1) / tw;
+  b.nty = (hi[1] - lo[1] + b.tyr - 1) / b.tyr;
   const int ez = std::max(0, hi[2] - lo[2]);
   int kz = std::min(KZ_MAX, std::max(1, ez));
   while (kz > 1 && (long long)b.ntx * b.nty * ((ez + kz - 1) / kz) < 8LL * s->num_sms) kz = (kz + 1) / 2;

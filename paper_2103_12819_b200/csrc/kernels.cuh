@@ -55,7 +55,9 @@ struct GridP {
 struct BoxP {
   int lo[3], hi[3];  // hi exclusive
   int ntx, nty, items;
-  int kz;  // planes marched per work item
+  int kz;   // planes marched per work item
+  int tyr;  // rows of a tile: TY, or a smaller power of two on a box with fewer rows (the block's
+            // other thread rows then take further 32-column strips: the tile is TX*TY/tyr wide)
 };
 
 // device-resident run state (one per handle)
@@ -165,9 +167,10 @@ struct Item {
 __device__ __forceinline__ Item decode_item(const BoxP &b, int it) {
   const int tx = it % b.ntx, r = it / b.ntx;
   const int ty = r % b.nty, tz = r / b.nty;
+  const int strip = (int)threadIdx.y / b.tyr, row = (int)threadIdx.y % b.tyr;
   Item w;
-  w.i = b.lo[0] + tx * TX + (int)threadIdx.x;
-  w.j = b.lo[1] + ty * TY + (int)threadIdx.y;
+  w.i = b.lo[0] + (tx * (TY / b.tyr) + strip) * TX + (int)threadIdx.x;
+  w.j = b.lo[1] + ty * b.tyr + row;
   w.k0 = b.lo[2] + tz * b.kz;
   w.k1 = min(w.k0 + b.kz, b.hi[2]);
   w.active = w.i < b.hi[0] && w.j < b.hi[1];
