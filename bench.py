@@ -130,7 +130,7 @@ def _oracle_rate(cfg, shape, steps, warmup=0, time_scheme=0):
     from oracle import Oracle  # noqa: F401  (the one place bench.py may execute oracle/)
     from oracle.cpu_oracle import omp_threads
     from paper_2103_12819_b200 import workloads as wl
-    from tests._util import oracle_from_workload
+    from oracle import oracle_from_workload
     w = wl.make_config(cfg, shape=shape)
     o = oracle_from_workload(w, time_scheme=time_scheme)
     if warmup:

@@ -11,7 +11,9 @@
  *   each (H,M) half-step is the iterated trapezoidal LLG solve of eqs. 18-21
  *   with |M| = Ms renormalisation and the global stopping test of PAPER.md:154.
  *   Options add the first-order scheme, hard / soft sources of E and H
- *    and the open boundary (PML).
+ *   (PAPER.md:100), the open boundary (PML) and the decomposition of the grid into
+ *   z-slabs, one per GPU, with the halo exchange done by peer stores inside the update kernels
+ *   (domain decomposition is the paper's parallelism; "Z-SLABS" below).
  *
  * Plain C types only: pointers (each argument says HOST or DEVICE), sizes, PODs.  No torch types.
  * Every step of the path runs in the library's own CUDA kernels; there is no CPU fallback.
@@ -80,10 +82,8 @@ typedef struct {
                          0 (default): staged sweep, tile 32x16 (TMA-fed shared-memory ring for the
                          neighbour operands) where it applies (alpha, gamma, mu_r uniform) and the
                          sweep box gives every SM a work item, else the direct-load kernels;
-                         1: direct-load kernels everywhere; 5: staged 32x16 whatever the box size;
-                         3: staged sweep, tile 32x7, two blocks per SM; 4: staged sweep that never
-                         writes M^1 (r = 1 stores H^1 only, r = 2 recomputes M^1: 18 words/cell less
-                         traffic, one more LLG evaluation; equal to rounding).  1, 3-5: A/B checks  */
+                         1: direct-load kernels everywhere; 5: staged sweep whatever the box size
+                         (1, 5: A/B checks of the two implementations)                           */
   int time_scheme;    /* 0 (default): the second-order scheme, iterated trapezoidal LLG;
                          1: the first-order scheme: one forward-Euler sweep of
                          eq. 7 / 12 per (H,M) half-step (advancing dt/2), N(M), then eq. 9 / 14;
@@ -96,6 +96,16 @@ typedef struct {
                          s_max = -(order+1) c ln(pml_r0) / (2 L) (A26)                  */
   double pml_r0;      /* theoretical normal-incidence reflection of the layer (default 1e-6)       */
   int pml_order;      /* grading order m (default 3)                                               */
+  int merge_h;        /* 1 (default): a face that no magnetic face reads (outside the LLG sweep box: the
+                         whole grid of a Maxwell-only run) takes the second H half-step of step n and
+                         the first of step n+1 -- the same curl E^{n+1}, PAPER.md:94 -- as ONE update:
+                         H is kept at half-integer time there and the integer-time value (the mean
+                         the paper's scheme holds) is formed when fields are read.  A third less
+                         traffic; equal to the two half-steps up to rounding.  Not applied with a PML
+                         or with H sources.  0: two half-steps everywhere                        */
+  int slab_ext[2];    /* z-low / z-high side of this grid is an INTERFACE to a neighbouring z-slab
+                         (see Z-SLABS), neither wall nor periodic wrap; bc[2] must be FDTD_LLG_PEC
+                         (it then describes the sides that are not interfaces)                    */
 } fdtd_llg_options;
 
 typedef struct {
@@ -119,6 +129,8 @@ typedef struct {
   int staged_sweeps;                /* 1: the LLG iterates r <= 3 run the staged kernel (hm_stage.cuh);
                                        0: the direct-load kernel (general materials, kernel_path 1,
                                        or a sweep box too small to give every SM a work item)   */
+  int merged_h;                     /* 1: the H half-steps outside the sweep box are merged
+                                       (options.merge_h and no PML, no H source)                */
 } fdtd_llg_stats;
 
 /* kernel classes of fdtd_llg_step_timed */
@@ -129,12 +141,12 @@ enum {
   FDTD_LLG_K_HM_SKIPPED = 3, /* LLG iterate launched after convergence (exits on the flag)      */
   FDTD_LLG_K_E_UPDATE = 4,   /* eq. 11                                                          */
   FDTD_LLG_K_OTHER = 5,      /* source amplitudes, half-step bookkeeping, canonical-buffer copy */
-  FDTD_LLG_K_HM_SECOND = 6,  /* LLG iterate r = 2 that ran (the staged sweep recomputes M^1 there) */
+  FDTD_LLG_K_HM_SECOND = 6,  /* LLG iterate r = 2 that ran                                       */
   FDTD_LLG_K_NCLASS = 7
 };
 
 /* Fill *opt with the defaults: PEC x3, LLG on, no bias, no anisotropy (axis z), tol 1e-6
- * (PAPER.md:154), max 20 iterations, graph on. */
+ * (PAPER.md:154), max 20 iterations, graph on, merge_h on, no slab interfaces. */
 void fdtd_llg_default_options(fdtd_llg_options *opt);
 
 /* Bytes of DEVICE workspace fdtd_llg_create needs for this grid.  `material_mask` = OR of the
@@ -142,7 +154,8 @@ void fdtd_llg_default_options(fdtd_llg_options *opt);
  * nothing once detected, so this is an upper bound).  Returns 0 on invalid arguments.
  * Budget: 12 doubles/cell for E,H (two sets each: every update is out of place); +21/cell when
  * enable_llg (the Jacobi H buffer, M and its time-n copy); +1/cell per material array; +13/cell
- * with a PML (12 split parts, the damping tables). */
+ * with a PML (12 split parts, the damping tables).  The same for a slab (its ghost planes exist
+ * in every layout). */
 size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
                                 unsigned material_mask);
 
@@ -225,6 +238,81 @@ const char *fdtd_llg_last_error(const fdtd_llg *s);
 
 /* Release the handle (host memory, graph).  The workspace stays the caller's.  NULL is a no-op. */
 void fdtd_llg_destroy(fdtd_llg *s);
+
+/* ------------------------------------------------------------------------------------ Z-SLABS
+ * Domain decomposition (one grid per rank, ghost cells exchanged "after each
+ * variable advancement routine"; in the paper that exchange went through the MPI hosts and was 60 %
+ * of the GPU run time).  Here the global grid is cut into slabs along z, one
+ * handle (one GPU) each, every slab nx x ny x nz with the SAME nx, ny, nz.  A handle created with
+ * options.slab_ext[side] = 1 treats that z side as an interface:
+ *   - every array passed to fdtd_llg_create and fdtd_llg_set_fields then carries the neighbour's
+ *     adjacent plane on that side: planes k = -1 (if slab_ext[0]) .. nz (if slab_ext[1]), i.e.
+ *     nx*ny*(nz + slab_ext[0] + slab_ext[1]) doubles, lowest plane first (the caller cuts them out
+ *     of the global arrays; for a globally periodic z axis the planes wrap around).  A material
+ *     given as one scalar (scalar_material_mask) stays one scalar.  fdtd_llg_read_fields returns
+ *     the slab's own nz planes; source boxes are in slab coordinates (0 <= index < nz).
+ *   - after fdtd_llg_slab_connect, the kernel that writes a value of the slab's first / last plane
+ *     also stores it into the neighbour's ghost plane (E_x, E_y, H_z of plane 0 go down, H_x, H_y
+ *     of plane nz-1 go up: what the curls and the four-point averages read across the cut), with
+ *     plain stores to the neighbour's workspace, which must be mapped in this process (same
+ *     process, or fdtd_llg_ipc_open + peer access over NVLink).  No separate exchange step exists.
+ * The caller drives the step with fdtd_llg_substep and orders the slabs:
+ *   RULE: a sub-step may be enqueued on a slab only after BOTH neighbours have completed the
+ *   previous sub-step (it reads ghost planes they wrote and overwrites ghost planes they read), and
+ *   the residual word of LLG iterate r (fdtd_llg_residual_word) must hold the MAXIMUM over all
+ *   slabs before iterate r+1 or the closing sub-step is enqueued anywhere (the
+ *   stopping test is over the entire domain).  A max-allreduce of that one word on the slabs'
+ *   streams (NCCL) is both the merge and the barrier; one host thread driving several handles on one
+ *   stream gets the order for free.  Nothing here needs a host synchronisation.
+ * The slabs then hold, bit for bit, what a single handle on the global grid holds (every update
+ * is a Jacobi sweep: independent of the order in which faces are visited). */
+typedef struct {
+  unsigned long long fields_offset; /* bytes from the workspace start to the first field array */
+  unsigned long long array_stride;  /* doubles between consecutive arrays                        */
+  int nx;
+  int ny;
+  int nz;
+  int n_arrays;                     /* field arrays at that stride (E, H, M sets)                */
+} fdtd_llg_slab_info;
+
+/* Layout facts a neighbour needs (HOST struct out). */
+int fdtd_llg_get_slab_info(fdtd_llg *s, fdtd_llg_slab_info *out);
+
+/* Connect the interfaces.  lo / hi: the lower / upper neighbour's info (NULL on a side that is not
+ * an interface), lo_workspace / hi_workspace: DEVICE address of that neighbour's workspace as seen
+ * from this process and this GPU.  EINVAL if the shapes differ.  Invalidates the captured step. */
+int fdtd_llg_slab_connect(fdtd_llg *s, const fdtd_llg_slab_info *lo, void *lo_workspace,
+                          const fdtd_llg_slab_info *hi, void *hi_workspace);
+
+/* The sub-steps of one time step, in the order they must be enqueued: */
+enum {
+  FDTD_LLG_SUB_BEGIN = 0,   /* source amplitudes, soft H sources                      */
+  FDTD_LLG_SUB_HM1 = 1,     /* first (H,M) half-step, LLG iterate r (argument): r = 1 also advances
+                               the faces outside the sweep box; r >= 2 exits on the device if iterate
+                               r-1 met the tolerance                                               */
+  FDTD_LLG_SUB_HM1_END = 2, /* closes the half-step: iteration count, canonical H set              */
+  FDTD_LLG_SUB_E = 3,       /* eq. 11, then the hard E sources                                     */
+  FDTD_LLG_SUB_HM2 = 4,     /* second (H,M) half-step, iterate r (r = 1: also the merged H update
+                               of the faces outside the sweep box, see merge_h)                    */
+  FDTD_LLG_SUB_HM2_END = 5  /* closes it; hard H sources; the step counter advances                */
+};
+/* Enqueue one sub-step (asynchronous, plain launches).  r is used by the two HM phases only
+ * (1 <= r <= llg_max_iter; without magnetic cells only r = 1 does anything).  ESTATE when called out
+ * of order.  Works on any handle (a handle without interfaces: the same result as fdtd_llg_step). */
+int fdtd_llg_substep(fdtd_llg *s, int phase, int r);
+
+/* DEVICE address of the 8-byte residual word of LLG iterate r (1..llg_max_iter): the bit pattern
+ * of the double max |M^r - M^{r-1}|/Ms over this slab's magnetic faces, >= 0, re-armed to 0 by the
+ * closing sub-step.  r = 0: a scratch word the library never reads (for barriers). */
+int fdtd_llg_residual_word(fdtd_llg *s, int r, void **dev_ptr);
+
+/* Sharing a workspace between processes (one process per GPU): export gives the CUDA IPC handle
+ * (64 bytes, HOST) of the allocation that holds this handle's workspace and the workspace's offset
+ * in it; open maps it in another process (peer access is enabled as needed) and returns the
+ * workspace's DEVICE address there; close unmaps (pass what open returned and the same offset). */
+int fdtd_llg_ipc_export(fdtd_llg *s, unsigned char *handle64, unsigned long long *offset);
+int fdtd_llg_ipc_open(const unsigned char *handle64, unsigned long long offset, void **dev_ptr);
+int fdtd_llg_ipc_close(void *dev_ptr, unsigned long long offset);
 
 #ifdef __cplusplus
 }

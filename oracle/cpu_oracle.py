@@ -197,6 +197,26 @@ class Oracle:
             pass
 
 
+def oracle_from_workload(w, kind="f64", time_scheme=0) -> Oracle:
+    """An Oracle loaded with a workload description (any object with the attributes of
+    ``workloads.Workload``: grid, materials, initial fields, sources, boundary options; its
+    ``numpy()`` gives host arrays).  Duck-typed: the oracle imports nothing of the CUDA package."""
+    a = w.numpy()
+    m = a["materials"]
+    o = Oracle(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt,
+               eps_r=m.get("eps_r"), sigma=m.get("sigma"), mu_r=m.get("mu_r"),
+               Ms=m.get("Ms"), alpha=m.get("alpha"), gamma=m.get("gamma"),
+               bc=w.bc, enable_llg=w.enable_llg, h_bias=w.h_bias, ani_hk=w.ani_hk,
+               ani_axis=w.ani_axis, llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, kind=kind,
+               time_scheme=time_scheme, pml=getattr(w, "pml", None),
+               **{k: getattr(w, k) for k in ("pml_r0", "pml_order") if getattr(w, k, None) is not None})
+    o.set_fields(a["E"], a["H"], a["M_cell"])
+    for s in w.sources:
+        prof = None if s.profile is None else s.profile.detach().cpu().numpy()
+        o.set_source(s.comp, s.lo, s.hi, prof, s.amplitude, s.f0, s.t0, s.tp, kind=getattr(s, "kind", 0))
+    return o
+
+
 def omp_threads() -> int:
     """Threads the oracle's OpenMP loops will use (for bench.py's ``cores``)."""
     v = os.environ.get("OMP_NUM_THREADS")

@@ -31,7 +31,7 @@ class Options(C.Structure):
                 ("llg_max_iter", C.c_int), ("use_graph", C.c_int),
                 ("scalar_material_mask", C.c_uint), ("kernel_path", C.c_int),
                 ("time_scheme", C.c_int), ("pml", C.c_int * 6), ("pml_r0", C.c_double),
-                ("pml_order", C.c_int)]
+                ("pml_order", C.c_int), ("merge_h", C.c_int), ("slab_ext", C.c_int * 2)]
 
 
 class Stats(C.Structure):
@@ -41,16 +41,34 @@ class Stats(C.Structure):
                 ("halfsteps", C.c_longlong), ("courant", C.c_double),
                 ("kernel_launches", C.c_longlong), ("magnetic_cells", C.c_longlong),
                 ("launches_per_step", C.c_int), ("sweep_cells", C.c_longlong),
-                ("material_array_mask", C.c_uint), ("staged_sweeps", C.c_int)]
+                ("material_array_mask", C.c_uint), ("staged_sweeps", C.c_int),
+                ("merged_h", C.c_int)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
+class SlabInfo(C.Structure):
+    _fields_ = [("fields_offset", C.c_ulonglong), ("array_stride", C.c_ulonglong),
+                ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("n_arrays", C.c_int)]
+
+    def as_tuple(self):
+        return tuple(getattr(self, k) for k, _ in self._fields_)
+
+    @classmethod
+    def from_tuple(cls, t):
+        return cls(*t)
+
+
 EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_create",
            "fdtd_llg_set_fields", "fdtd_llg_set_source", "fdtd_llg_add_source", "fdtd_llg_step", "fdtd_llg_step_timed",
            "fdtd_llg_read_fields",
-           "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy")
+           "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy",
+           "fdtd_llg_get_slab_info", "fdtd_llg_slab_connect", "fdtd_llg_substep",
+           "fdtd_llg_residual_word", "fdtd_llg_ipc_export", "fdtd_llg_ipc_open", "fdtd_llg_ipc_close")
+
+# sub-steps of one time step (fdtd_llg.h FDTD_LLG_SUB_*)
+SUB_BEGIN, SUB_HM1, SUB_HM1_END, SUB_E, SUB_HM2, SUB_HM2_END = range(6)
 
 KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other", "hm_second")
 
@@ -102,6 +120,20 @@ def lib() -> C.CDLL:
         L.fdtd_llg_last_error.restype = C.c_char_p
         L.fdtd_llg_destroy.argtypes = [_VP]
         L.fdtd_llg_destroy.restype = None
+        L.fdtd_llg_get_slab_info.argtypes = [_VP, C.POINTER(SlabInfo)]
+        L.fdtd_llg_get_slab_info.restype = C.c_int
+        L.fdtd_llg_slab_connect.argtypes = [_VP, C.POINTER(SlabInfo), _VP, C.POINTER(SlabInfo), _VP]
+        L.fdtd_llg_slab_connect.restype = C.c_int
+        L.fdtd_llg_substep.argtypes = [_VP, C.c_int, C.c_int]
+        L.fdtd_llg_substep.restype = C.c_int
+        L.fdtd_llg_residual_word.argtypes = [_VP, C.c_int, C.POINTER(_VP)]
+        L.fdtd_llg_residual_word.restype = C.c_int
+        L.fdtd_llg_ipc_export.argtypes = [_VP, C.POINTER(C.c_ubyte), C.POINTER(C.c_ulonglong)]
+        L.fdtd_llg_ipc_export.restype = C.c_int
+        L.fdtd_llg_ipc_open.argtypes = [C.POINTER(C.c_ubyte), C.c_ulonglong, C.POINTER(_VP)]
+        L.fdtd_llg_ipc_open.restype = C.c_int
+        L.fdtd_llg_ipc_close.argtypes = [_VP, C.c_ulonglong]
+        L.fdtd_llg_ipc_close.restype = C.c_int
         _lib = L
     return _lib
 
@@ -157,11 +189,15 @@ class FdtdLlg:
     def __init__(self, nx, ny, nz, dx, dy, dz, dt, *, materials=None, bc=(PEC, PEC, PEC),
                  enable_llg=True, h_bias=(0.0, 0.0, 0.0), ani_hk=0.0, ani_axis=(0.0, 0.0, 1.0),
                  llg_tol=1e-6, llg_max_iter=20, use_graph=True, device="cuda:0", stream=None,
-                 kernel_path=0, time_scheme=0, pml=None, pml_r0=None, pml_order=None):
+                 kernel_path=0, time_scheme=0, pml=None, pml_r0=None, pml_order=None,
+                 merge_h=True, slab_ext=(0, 0)):
         import torch
         self._torch = torch
         self.shape = (nz, ny, nx)
         self.n = nx * ny * nz
+        # a slab's input arrays carry the neighbours' adjacent planes (fdtd_llg.h "Z-SLABS")
+        self.slab_ext = (int(bool(slab_ext[0])), int(bool(slab_ext[1])))
+        self.n_in = nx * ny * (nz + sum(self.slab_ext))
         self.device = torch.device(device)
         self._h = None
         L = lib()
@@ -184,6 +220,8 @@ class FdtdLlg:
             opt.pml_r0 = float(pml_r0)
         if pml_order is not None:
             opt.pml_order = int(pml_order)
+        opt.merge_h = int(bool(merge_h))
+        opt.slab_ext[0], opt.slab_ext[1] = self.slab_ext
         self.options = opt
         materials = {k: v for k, v in (materials or {}).items() if v is not None}
         scalars = {k: C.c_double(float(v)) for k, v in materials.items()
@@ -219,8 +257,8 @@ class FdtdLlg:
         else:
             import numpy as np
             t = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64))
-        if t.numel() != self.n:
-            raise ValueError(f"array has {t.numel()} entries, expected {self.n}")
+        if t.numel() != self.n_in:
+            raise ValueError(f"array has {t.numel()} entries, expected {self.n_in}")
         return t
 
     @staticmethod
@@ -297,6 +335,38 @@ class FdtdLlg:
         _check(rc, self._h)
         return out
 
+    # -- z-slabs (fdtd_llg.h "Z-SLABS") -------------------------------------------------------
+    def slab_info(self) -> SlabInfo:
+        info = SlabInfo()
+        _check(lib().fdtd_llg_get_slab_info(self._h, C.byref(info)), self._h)
+        return info
+
+    def connect(self, lo=None, hi=None):
+        """lo / hi: (SlabInfo, device address of that neighbour's workspace in this process) or None."""
+        a = [(C.byref(x[0]), C.c_void_p(x[1])) if x is not None else (None, None) for x in (lo, hi)]
+        with self._torch.cuda.device(self.device):
+            rc = lib().fdtd_llg_slab_connect(self._h, a[0][0], a[0][1], a[1][0], a[1][1])
+        _check(rc, self._h)
+
+    def substep(self, phase, r=0):
+        with self._torch.cuda.device(self.device):
+            rc = lib().fdtd_llg_substep(self._h, int(phase), int(r))
+        _check(rc, self._h)
+
+    def residual_word(self, r):
+        """Zero-copy view (1 float64) of the residual word of LLG iterate r inside the workspace."""
+        p = C.c_void_p()
+        _check(lib().fdtd_llg_residual_word(self._h, int(r), C.byref(p)), self._h)
+        off = p.value - self.workspace.data_ptr()
+        return self.workspace[off:off + 8].view(self._torch.float64)
+
+    def ipc_export(self):
+        """(64-byte CUDA IPC handle, offset) of the workspace, for fdtd_llg_ipc_open in another process."""
+        h = (C.c_ubyte * 64)()
+        off = C.c_ulonglong()
+        _check(lib().fdtd_llg_ipc_export(self._h, h, C.byref(off)), self._h)
+        return bytes(h), int(off.value)
+
     def stats(self) -> dict:
         st = Stats()
         with self._torch.cuda.device(self.device):
@@ -318,8 +388,24 @@ class FdtdLlg:
             pass
 
 
+def fdtd_llg_ipc_open(handle: bytes, offset: int) -> int:
+    """Map another process's workspace; returns its device address here."""
+    h = (C.c_ubyte * 64).from_buffer_copy(handle)
+    p = C.c_void_p()
+    rc = lib().fdtd_llg_ipc_open(h, C.c_ulonglong(offset), C.byref(p))
+    if rc != OK:
+        raise FdtdLlgError(rc, fdtd_llg_last_error(None))
+    return p.value
+
+
+def fdtd_llg_ipc_close(ptr: int, offset: int) -> None:
+    rc = lib().fdtd_llg_ipc_close(C.c_void_p(ptr), C.c_ulonglong(offset))
+    if rc != OK:
+        raise FdtdLlgError(rc, fdtd_llg_last_error(None))
+
+
 def from_workload(w, device="cuda:0", use_graph=True, stream=None, fields_device=None,
-                  kernel_path=0, time_scheme=0) -> FdtdLlg:
+                  kernel_path=0, time_scheme=0, merge_h=True, slab_ext=None) -> FdtdLlg:
     """Create a simulation from a :class:`workloads.Workload` and load its initial state.
     Arrays are passed in whatever memory space the workload's tensors live in."""
     sim = FdtdLlg(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.dt, materials=w.materials, bc=w.bc,
@@ -327,7 +413,9 @@ def from_workload(w, device="cuda:0", use_graph=True, stream=None, fields_device
                   llg_tol=w.llg_tol, llg_max_iter=w.llg_max_iter, use_graph=use_graph,
                   device=device, stream=stream, kernel_path=kernel_path,
                   time_scheme=time_scheme, pml=getattr(w, "pml", None),
-                  pml_r0=getattr(w, "pml_r0", None), pml_order=getattr(w, "pml_order", None))
+                  pml_r0=getattr(w, "pml_r0", None), pml_order=getattr(w, "pml_order", None),
+                  merge_h=merge_h,
+                  slab_ext=slab_ext if slab_ext is not None else getattr(w, "slab_ext", (0, 0)))
     sim.set_fields(w.E, w.H, w.M_cell)
     for s in w.sources:
         sim.set_source(s.comp, s.lo, s.hi, s.profile, s.amplitude, s.f0, s.t0, s.tp,

@@ -46,8 +46,8 @@ struct fdtd_llg {
   GridP g{};
   double d[3]{}, dt = 0;
   size_t ncell = 0, stride = 0;  // stride = array_stride(): doubles between consecutive arrays
+  size_t ncell_user = 0;         // entries of a user array passed IN: ncell + the interface planes
   int num_sms = 148;
-  int sweep_blocks_per_sm = 4;
   fdtd_llg_options opt{};
   cudaStream_t stream = nullptr;
   char *ws = nullptr;
@@ -61,11 +61,10 @@ struct fdtd_llg {
   bool llg = false;  // LLG enabled AND at least one magnetic cell
   long long magnetic_cells = 0;
   int lo[3]{}, hi[3]{};  // sweep box (index triples), hi exclusive
+  int lo0_unrounded = 0; // lo[0] before it was rounded down to an even index (kept odd next to a PML)
   BoxP box_llg{}, box_all{};
   int n_arrays = 0;  // arrays in the workspace tensor (4th TMA coordinate)
-  // staged sweeps (hm_stage.cuh): kernel_path 0, 4 (tile rows 16) and 3 (tile rows 7)
-  int stage_by = 0;  // 0 = not used
-  bool stage_lean = false;  // kernel_path 4: M^1 recomputed at r = 2 instead of stored at r = 1
+  bool staged = false;  // the LLG iterates run the staged sweep (hm_stage.cuh)
   StBox st_box{}, st_box_first{};  // work items of the iterates r >= 2 / of the r = 1 sweep
   CUtensorMap mapT{}, mapPM{};
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
@@ -98,6 +97,15 @@ struct fdtd_llg {
   int launches_per_step = 0;
   long long kernel_launches = 0;
   long long host_steps = 0;
+  // merged H half-steps (options.merge_h): outside the sweep box H lives at half-integer time
+  bool merge = false;        // active for this handle (no PML, no H sources)
+  bool primed = false;       // the outside faces have been advanced to t = dt/2 (first step taken)
+  long long prime_at = 0;    // host_steps when that happened
+  bool recon_valid = false;  // the integer-time H of the present state has been formed for reading
+  // z-slab decomposition
+  bool is_slab = false;      // any slab_ext side set
+  int sub_next = 0;          // the sub-step fdtd_llg_substep expects next (FDTD_LLG_SUB_*)
+  int sub_r = 0;             // last LLG iterate enqueued in the current half-step
   std::string err = "";
 };
 
@@ -168,12 +176,13 @@ int grid_1d(const fdtd_llg *s, long long n) {
 }
 
 // strided copies between a user's compact array and the ghosted device layout
+// (a slab's user arrays carry the neighbours' adjacent planes: k = -ext[0] .. nz - 1 + ext[1])
 int copy_in(fdtd_llg *s, double *dev, const double *user, int mem_space) {
   cudaMemcpy3DParms p{};
   p.srcPtr = make_cudaPitchedPtr(const_cast<double *>(user), (size_t)s->g.n[0] * 8, (size_t)s->g.n[0] * 8, (size_t)s->g.n[1]);
   p.dstPtr = make_cudaPitchedPtr(dev, (size_t)s->g.sy * 8, (size_t)s->g.sy * 8, (size_t)s->g.n[1] + 2);
-  p.dstPos = make_cudaPos((size_t)PADL * 8, 1, 1);
-  p.extent = make_cudaExtent((size_t)s->g.n[0] * 8, (size_t)s->g.n[1], (size_t)s->g.n[2]);
+  p.dstPos = make_cudaPos((size_t)PADL * 8, 1, (size_t)(1 - s->g.ext[0]));
+  p.extent = make_cudaExtent((size_t)s->g.n[0] * 8, (size_t)s->g.n[1], (size_t)(s->g.n[2] + s->g.ext[0] + s->g.ext[1]));
   p.kind = mem_space == FDTD_LLG_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
   cudaError_t e = cudaMemcpy3DAsync(&p, s->stream);
   if (e != cudaSuccess) { s->err = std::string("cudaMemcpy3DAsync (in): ") + cudaGetErrorString(e); return FDTD_LLG_ECUDA; }
@@ -211,9 +220,15 @@ bool valid_opts(const fdtd_llg_options *o, const char **why) {
     if (!(o->pml_r0 > 0 && o->pml_r0 < 1)) { *why = "pml_r0 must be in (0, 1)"; return false; }
     if (o->pml_order < 1 || o->pml_order > 6) { *why = "pml_order must be in 1..6"; return false; }
   }
+  if (o->llg_max_iter < 1 || o->llg_max_iter > 1000) { *why = "llg_max_iter must be in 1..1000"; return false; }
+  if (o->kernel_path != 0 && o->kernel_path != 1 && o->kernel_path != 5) { *why = "kernel_path must be 0, 1 or 5"; return false; }
+  for (int sd = 0; sd < 2; ++sd) {
+    if (o->slab_ext[sd] != 0 && o->slab_ext[sd] != 1) { *why = "slab_ext must be 0 or 1"; return false; }
+    if (o->slab_ext[sd] && o->bc[2] != FDTD_LLG_PEC) { *why = "a slab interface needs bc[2] = FDTD_LLG_PEC (a periodic z axis is closed by connecting the end slabs)"; return false; }
+    if (o->slab_ext[sd] && o->pml[4 + sd] > 0) { *why = "no PML on a slab interface"; return false; }
+  }
   if (o->enable_llg) {
     if (!(o->llg_tol > 0) || !std::isfinite(o->llg_tol)) { *why = "llg_tol must be > 0"; return false; }
-    if (o->llg_max_iter < 1 || o->llg_max_iter > 1000) { *why = "llg_max_iter must be in 1..1000"; return false; }
     if (o->ani_hk != 0.0) {
       double n2 = 0;
       for (int d = 0; d < 3; ++d) n2 += o->ani_axis[d] * o->ani_axis[d];
@@ -237,7 +252,7 @@ size_t small_bytes(const fdtd_llg_options *o) {
 
 // min/max of a user array (host or device)
 int array_minmax(fdtd_llg *s, const double *a, int mem_space, double *lo, double *hi) {
-  const size_t n = s->ncell;
+  const size_t n = s->ncell_user;
   if (mem_space == FDTD_LLG_HOST) {
     double l = INFINITY, h = -INFINITY;
     bool nan = false;
@@ -312,36 +327,46 @@ int find_sweep_box(fdtd_llg *s) {
   if (!s->Ms.is_array) {
     if (!(s->Ms.uniform > 0.0)) return FDTD_LLG_OK;
     for (int d = 0; d < 3; ++d) { clo[d] = 0; chi[d] = s->g.n[d] - 1; }
+    clo[2] -= s->g.ext[0];   // a uniform map includes the neighbours' planes
+    chi[2] += s->g.ext[1];
     s->magnetic_cells = (long long)s->ncell;
   } else {
     int *box = reinterpret_cast<int *>(s->scratch + 2 * 1024);
     unsigned long long *cnt = reinterpret_cast<unsigned long long *>(s->scratch + 2 * 1024 + 8);
-    int init[6] = {INT_MAX, INT_MAX, INT_MAX, -1, -1, -1};
+    int init[6] = {INT_MAX, INT_MAX, INT_MAX, INT_MIN, INT_MIN, INT_MIN};
     unsigned long long zero = 0;
     CU(s, cudaMemcpyAsync(box, init, sizeof init, cudaMemcpyHostToDevice, s->stream));
     CU(s, cudaMemcpyAsync(cnt, &zero, sizeof zero, cudaMemcpyHostToDevice, s->stream));
-    k_mag_box<<<grid_1d(s, (long long)s->ncell), 256, 0, s->stream>>>(s->Ms.dev, s->g, box, cnt);
+    k_mag_box<<<grid_1d(s, (long long)s->ncell_user), 256, 0, s->stream>>>(s->Ms.dev, s->g, box, cnt);
     CU(s, cudaGetLastError());
     int out[6];
     unsigned long long c = 0;
     CU(s, cudaMemcpyAsync(out, box, sizeof out, cudaMemcpyDeviceToHost, s->stream));
     CU(s, cudaMemcpyAsync(&c, cnt, sizeof c, cudaMemcpyDeviceToHost, s->stream));
     CU(s, cudaStreamSynchronize(s->stream));
-    if (c == 0) return FDTD_LLG_OK;
+    if (out[3] == INT_MIN) return FDTD_LLG_OK;   // no magnetic cell, not even in a neighbour's plane
     for (int d = 0; d < 3; ++d) { clo[d] = out[d]; chi[d] = out[3 + d]; }
     s->magnetic_cells = (long long)c;
   }
-  // index triples owning a magnetic face: cells clo..chi+1; plus one triple of halo each side,
-  // because the four-point averages of a magnetic face read its neighbours' H from the Jacobi
-  // buffers.  A box touching a periodic end wraps: take the full axis there.
+  // A D-face at index p is magnetic iff cell p-1 or p is: p in clo..chi+1.  It reads its own H, and
+  // through the four-point averages H at p-1, p along D and at t, t+1 along the
+  // transverse axis (t in clo..chi): every H a magnetic face reads from the Jacobi buffers has its
+  // index in clo-1..chi+1 on every axis.  That is the sweep box.  A box touching a periodic end
+  // wraps: take the full axis there.
   for (int d = 0; d < 3; ++d) {
-    int l = clo[d] - 1, h = chi[d] + 3;  // exclusive upper bound
+    int l = clo[d] - 1, h = chi[d] + 2;  // exclusive upper bound
     const int n = s->g.n[d];
     if (s->g.per[d] && (l < 0 || h > n)) { l = 0; h = n; }
     s->lo[d] = l < 0 ? 0 : l;
     s->hi[d] = h > n ? n : h;
-    if (d == 0) s->lo[d] &= ~1;  // even start in x: TMA box rows begin on 16-byte boundaries
+    if (d == 0) {
+      // even start in x for the staged sweeps (their TMA boxes then begin on 16-byte boundaries);
+      // not when the extra column would lie in a PML (the layer has its own update there)
+      s->lo0_unrounded = s->lo[d];
+      if ((s->lo[d] & ~1) >= s->opt.pml[0]) s->lo[d] &= ~1;
+    }
   }
+  if (s->lo[2] >= s->hi[2]) return FDTD_LLG_OK;  // (cannot happen: a neighbour's magnetic plane reaches into the slab)
   s->llg = true;
   return FDTD_LLG_OK;
 }
@@ -433,44 +458,39 @@ StBox make_stbox(const int lo[3], const int hi[3], int by, int kz_target) {
   return b;
 }
 
-template <int BY, int MODE>
-int launch_hm_stage_by(fdtd_llg *s, const HMSArgs &p) {
+template <bool FIRST>
+int launch_hm_stage(fdtd_llg *s, const HMSArgs &p) {
   const bool ms = s->Ms.is_array, an = s->opt.ani_hk != 0.0;
-  const int grid = std::max(1, std::min(p.tb.items, s->num_sms * StLayout<BY, st_first(MODE), true>::BPS));
+  const int grid = std::max(1, std::min(p.tb.items, s->num_sms));   // one persistent block per SM
 #define SK(MS, AN)                                                                          \
   if (ms == MS && an == AN) {                                                               \
-    using L = StLayout<BY, st_first(MODE), MS>;                                             \
-    k_hm_stage<BY, MODE, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);       \
+    using L = StLayout<FIRST, MS>;                                                          \
+    k_hm_stage<FIRST, MS, AN><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);          \
     return FDTD_LLG_OK;                                                                     \
   }
   SK(false, false) SK(false, true) SK(true, false) SK(true, true)
 #undef SK
   return FDTD_LLG_OK;
 }
-template <int MODE>
-int launch_hm_stage(fdtd_llg *s, const HMSArgs &p) {
-  return s->stage_by == 16 ? launch_hm_stage_by<16, MODE>(s, p) : launch_hm_stage_by<7, MODE>(s, p);
-}
 
-template <int BY>
-int setup_hm_stage_by(fdtd_llg *s) {
-#define SA(MODE, MS, AN)                                                                    \
-  CU(s, cudaFuncSetAttribute(k_hm_stage<BY, MODE, MS, AN>,                                  \
+int setup_hm_stage(fdtd_llg *s) {
+#define SA(FIRST, MS, AN)                                                                   \
+  CU(s, cudaFuncSetAttribute(k_hm_stage<FIRST, MS, AN>,                                     \
                              cudaFuncAttributeMaxDynamicSharedMemorySize,                   \
-                             (int)StLayout<BY, st_first(MODE), MS>::SMEM_BYTES));
-#define SA4(MODE) SA(MODE, false, false) SA(MODE, false, true) SA(MODE, true, false) SA(MODE, true, true)
-  SA4(ST_FIRST) SA4(ST_ITER) SA4(ST_FIRST_H) SA4(ST_ITER_RE)
+                             (int)StLayout<FIRST, MS>::SMEM_BYTES));
+#define SA4(FIRST) SA(FIRST, false, false) SA(FIRST, false, true) SA(FIRST, true, false) SA(FIRST, true, true)
+  SA4(true) SA4(false)
 #undef SA4
 #undef SA
   int rc;
-  if ((rc = make_map(s, &s->mapT, SROW, BY + 1, 1))) return rc;
-  if ((rc = make_map(s, &s->mapPM, SW, BY, 9))) return rc;
-  s->st_box_first = make_stbox(s->lo, s->hi, BY, 32);
-  s->st_box = make_stbox(s->lo, s->hi, BY, 8);
+  if ((rc = make_map(s, &s->mapT, SROW, SBY + 1, 1))) return rc;
+  if ((rc = make_map(s, &s->mapPM, SW, SBY, 9))) return rc;
+  s->st_box_first = make_stbox(s->lo, s->hi, SBY, 32);
+  s->st_box = make_stbox(s->lo, s->hi, SBY, 8);
   // A sweep box that cannot give every SM an item (a thin slab, a small grid) is latency bound:
   // the direct-load kernels with their 32 x 8 x 16 blocks fill the GPU better there (32^3: 9 us
   // against 79 us per sweep; the bits are the same).
-  if (s->opt.kernel_path == 0 && s->st_box.items < s->num_sms) s->stage_by = 0;
+  if (s->opt.kernel_path == 0 && s->st_box.items < s->num_sms) s->staged = false;
   return FDTD_LLG_OK;
 }
 
@@ -629,17 +649,39 @@ int end_cond_tail(fdtd_llg *s, cudaStream_t outer) {
   return FDTD_LLG_OK;
 }
 
-// (H,M) half-step: time-n set `in`, result in set `out`, `tmp` is the other Jacobi buffer.
-// M: time-n set `min`, result in set `mout`.
-int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int min, int mout, bool last,
-                 int *launches) {
-  int *const launches_outer = launches;
+// ---- which H set holds what ------------------------------------
+// Two half-steps everywhere (merge off): H^n in set 0, H^{n+1/2} in set 1, Jacobi buffer set 2.
+// Merged H half-steps: the faces OUTSIDE the sweep box live at half-integer time and ping-pong
+// between two sets, one read by the E update of even steps, the other by that of odd steps
+// (every update stays out of place); the box uses the same set for its H^{n+1/2} and the other
+// one as Jacobi buffer (disjoint regions).  With LLG storage these are sets 1 and 2 and the box's
+// H^n stays in set 0; a Maxwell-only handle has two sets, 1 and 0.
+int set_half(const fdtd_llg *s, int par) {
+  if (!s->merge) return 1;
+  return s->opt.enable_llg ? (par ? 2 : 1) : (par ? 0 : 1);
+}
+int set_tmp(const fdtd_llg *s, int par) {
+  if (!s->merge) return 2;
+  return s->opt.enable_llg ? (par ? 1 : 2) : 2;   // Maxwell-only: no sweep ever uses it
+}
+bool merge_allowed(const fdtd_llg *s) {
+  if (!s->opt.merge_h || s->has_pml) return false;
+  for (int q = 0; q < s->src.count; ++q)
+    if (s->src.s[q].kind == FDTD_LLG_SRC_SOFT_H || s->src.s[q].kind == FDTD_LLG_SRC_HARD_H) return false;
+  return true;
+}
+
+// Maxwell update of the faces outside the sweep box (eq. 21 with M = 0):
+// set `out` = set `in` - cmul (dt / 2 mu) curl E; cmul = 1: half a step, 2: two half-steps at once
+int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul, bool exports, int *launches) {
   const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
+  if (!exports) h.g.dlo = h.g.dhi = 0;
   for (int d = 0; d < 3; ++d) { h.E[d] = E[d]; h.Hn[d] = s->Hset[in][d]; h.Hc[d] = s->Hset[out][d]; }
   h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
   h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
+  h.cmul = cmul;
   for (int b = 0; b < s->n_out; ++b) {
     h.box = s->box_out[b];
     if (h.box.items == 0) continue;
@@ -650,103 +692,88 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
     prof_end(s);
     ++*launches;
   }
-  {
-    int rc = enqueue_pml(s, false, E, s->Hset[out], launches);
-    if (rc) return rc;
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
+// (H,M) half-step, part 1: the faces outside the sweep box and the open-boundary layer.
+// Merged H half-steps: nothing in the first half-step; in the second one (merged_to >= 0) the
+// second half of this step and the first half of the next are taken at once, both with curl E^{n+1}
+// (PAPER.md:94), from the set the E update read into the set the next E update will read.
+int enqueue_half_pre(fdtd_llg *s, double *const *E, int in, int out, int merged_to, int *launches) {
+  int rc = FDTD_LLG_OK;
+  if (!s->merge) rc = enqueue_outside(s, E, in, out, 1.0, true, launches);
+  else if (merged_to >= 0) rc = enqueue_outside(s, E, in, merged_to, 2.0, true, launches);
+  if (rc) return rc;
+  return enqueue_pml(s, false, E, s->Hset[out], launches);
+}
+
+// (H,M) half-step, part 2: LLG iterate r on the sweep box.  Time-n set `in`, result in set `out`,
+// `tmp` is the other Jacobi buffer (odd r writes `out`, even r `tmp`); M: time-n set `min`, iterate
+// in set `mout`.
+int enqueue_sweep(fdtd_llg *s, double *const *E, int in, int out, int tmp, int min, int mout, int r,
+                  int *launches) {
+  HMArgs a{};
+  a.g = s->g;
+  a.box = s->box_llg;
+  for (int d = 0; d < 3; ++d) { a.E[d] = E[d]; a.Hn[d] = s->Hset[in][d]; }
+  for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
+  a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
+  a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
+  a.cf_u = kMu0 * a.gamma_u * s->dt * 0.25;   // the device expression, evaluated once
+  a.kh = s->dt / (2.0 * kMu0);
+  a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
+  if (s->staged && s->Ms.is_array) {  // the most common face value and its reciprocal
+    a.Ms_u = s->Ms.maxv;
+    a.rMs_u = 1.0 / s->Ms.maxv;
   }
-  if (s->llg) {
-    HMArgs a{};
-    a.g = s->g;
-    a.box = s->box_llg;
-    for (int d = 0; d < 3; ++d) { a.E[d] = E[d]; a.Hn[d] = s->Hset[in][d]; }
-    for (int q = 0; q < 9; ++q) { a.Mn[q] = s->Mset[min][q]; a.Mr[q] = s->Mset[mout][q]; }
-    a.Ms = s->Ms.dev; a.alpha = s->alpha.dev; a.gamma = s->gamma.dev; a.mu_r = s->mu_r.dev;
-    a.Ms_u = s->Ms.uniform; a.alpha_u = s->alpha.uniform; a.gamma_u = std::fabs(s->gamma.uniform);
-    a.cf_u = kMu0 * a.gamma_u * s->dt * 0.25;   // the device expression, evaluated once
-    a.kh = s->dt / (2.0 * kMu0);
-    a.rMs_u = s->Ms.uniform > 0.0 ? 1.0 / s->Ms.uniform : 0.0;
-    if (s->stage_by && s->Ms.is_array) {  // the most common face value and its reciprocal
-      a.Ms_u = s->Ms.maxv;
-      a.rMs_u = 1.0 / s->Ms.maxv;
-    }
-    a.ch_uniform = h.ch_uniform;
-    for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
-    a.hk = s->opt.ani_hk;
-    a.tol = s->opt.llg_tol;
-    a.euler = s->opt.time_scheme == 1;
-    a.resid = s->resid;
-    a.pipe_error = &s->dstate->pipe_error;
-    cudaStream_t outer = nullptr;  // set while the launches go into the body of the IF node
-    int body_launches = 0;
-    for (int r = 1; r <= s->opt.llg_max_iter; ++r) {
-      // Iterates r >= 4 almost never run.  In the captured step they sit in ONE conditional (IF)
-      // node armed on the device by k_set_cond, so the usual step does not even launch them.
-      // (The node itself costs about as much as ten empty launches: only worth it for a long tail.)
-      if (r == 4 && s->capturing && s->aux && s->opt.use_graph == 1 && s->opt.llg_max_iter >= 12) {
-        int rc = begin_cond_tail(s, r, &outer);
-        if (rc) return rc;
-        ++*launches;  // k_set_cond
-        launches = &body_launches;
-      }
-      // r <= 3 normally run: one block per item.  Later iterates almost never run: a small
-      // persistent grid keeps their early exit at launch-latency cost.
-      const int grid = grid_for(s, a.box, r <= 3 ? 0 : s->sweep_blocks_per_sm);
-      // iterate r reads H^{r-1} and writes H^r: odd r -> `out`, even r -> `tmp`
-      const int from = (r == 1) ? in : ((r & 1) ? tmp : out);
-      const int to = (r & 1) ? out : tmp;
-      for (int d = 0; d < 3; ++d) { a.Hp[d] = s->Hset[from][d]; a.Hc[d] = s->Hset[to][d]; }
-      a.r = r;
-      prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
-      int rc;
-      if (s->stage_by) {
-        HMSArgs p{};
-        p.a = a;
-        p.tb = r == 1 ? s->st_box_first : s->st_box;
-        p.mapT = s->mapT; p.mapM = s->mapPM;
-        p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
-        p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
-        p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
-        p.work = s->work + r;
-        p.cond = r > 1;
-        // kernel_path 4: M^1 never goes to memory: r = 1 stores H^1 only and r = 2
-        // recomputes M^1 from the operands it reads anyway (18 words/cell less traffic).  Should
-        // iterate 1 already pass the stopping test, M^1 IS the result: the full r = 1 sweep then
-        // runs after all (cond 2; otherwise it exits on its first flag read).
-        const bool lean = s->stage_lean && s->opt.llg_max_iter >= 2;
-        if (r == 1 && lean) {
-          rc = launch_hm_stage<ST_FIRST_H>(s, p);
-          prof_end(s);
-          if (rc) return rc;
-          ++*launches;
-          prof_begin(s, FDTD_LLG_K_HM_ITER, s->opt.llg_max_iter + 1);  // counted as skipped unless it ran
-          p.work = s->work;
-          p.cond = 2;
-          rc = launch_hm_stage<ST_FIRST>(s, p);
-        } else if (r == 1) {
-          rc = launch_hm_stage<ST_FIRST>(s, p);
-        } else if (r == 2 && lean) {
-          rc = launch_hm_stage<ST_ITER_RE>(s, p);
-        } else {
-          rc = launch_hm_stage<ST_ITER>(s, p);
-        }
-      } else {
-        rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
-      }
-      prof_end(s);
-      if (rc) return rc;
-      ++*launches;
-    }
-    if (outer) {
-      launches = launches_outer;
-      int rc = end_cond_tail(s, outer);
-      if (rc) return rc;
-    }
+  a.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
+  for (int d = 0; d < 3; ++d) { a.hb[d] = s->opt.h_bias[d]; a.u[d] = s->opt.ani_axis[d]; }
+  a.hk = s->opt.ani_hk;
+  a.tol = s->opt.llg_tol;
+  a.euler = s->opt.time_scheme == 1;
+  a.resid = s->resid;
+  a.pipe_error = &s->dstate->pipe_error;
+  // r <= 3 normally run: one block per item.  Later iterates almost never run: a small
+  // persistent grid keeps their early exit at launch-latency cost.
+  const int grid = grid_for(s, a.box, r <= 3 ? 0 : 4);
+  // iterate r reads H^{r-1} and writes H^r: odd r -> `out`, even r -> `tmp`
+  const int from = (r == 1) ? in : ((r & 1) ? tmp : out);
+  const int to = (r & 1) ? out : tmp;
+  for (int d = 0; d < 3; ++d) { a.Hp[d] = s->Hset[from][d]; a.Hc[d] = s->Hset[to][d]; }
+  a.r = r;
+  prof_begin(s, r == 1 ? FDTD_LLG_K_HM_FIRST : FDTD_LLG_K_HM_ITER, r);
+  int rc;
+  if (s->staged) {
+    HMSArgs p{};
+    p.a = a;
+    p.tb = r == 1 ? s->st_box_first : s->st_box;
+    p.mapT = s->mapT; p.mapM = s->mapPM;
+    p.aE = array_index(s, a.E[0]); p.aHn = array_index(s, a.Hn[0]); p.aHp = array_index(s, a.Hp[0]);
+    p.aMn = array_index(s, a.Mn[0]); p.aMp = array_index(s, a.Mr[0]);
+    p.aMs = a.Ms ? array_index(s, a.Ms) : 0;
+    p.work = s->work + r;
+    p.cond = r > 1;
+    rc = (r == 1) ? launch_hm_stage<true>(s, p) : launch_hm_stage<false>(s, p);
+  } else {
+    rc = (r == 1) ? launch_sweep<true>(s, a, grid) : launch_sweep<false>(s, a, grid);
   }
+  prof_end(s);
+  if (rc) return rc;
+  ++*launches;
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
+// (H,M) half-step, part 3: iteration count and statistics from the residual words of the r_max
+// iterates that were enqueued, the canonical H set
+int enqueue_half_end(fdtd_llg *s, int out, int tmp, int r_max, bool last, int *launches) {
+  const dim3 blk(TX, TY, 1);
   prof_begin(s, FDTD_LLG_K_OTHER, 0);
-  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->r_hist, s->opt.llg_max_iter,
+  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->r_hist, r_max, s->opt.llg_max_iter,
                                      s->opt.llg_tol, s->llg ? 1 : 0, last ? 1 : 0);
   ++*launches;
-  if (s->llg && s->opt.llg_max_iter >= 2) {
+  if (s->llg && r_max >= 2) {
     CanonArgs c{};
     c.g = s->g;
     c.box = s->box_llg;
@@ -759,6 +786,36 @@ int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int mi
   if (s->prof) s->prof_half++;
   CU(s, cudaGetLastError());
   return FDTD_LLG_OK;
+}
+
+// the whole half-step as fdtd_llg_step enqueues it
+int enqueue_half(fdtd_llg *s, double *const *E, int in, int out, int tmp, int min, int mout, bool last,
+                 int merged_to, int *launches) {
+  int rc = enqueue_half_pre(s, E, in, out, merged_to, launches);
+  if (rc) return rc;
+  if (s->llg) {
+    cudaStream_t outer = nullptr;  // set while the launches go into the body of the IF node
+    int body_launches = 0;
+    int *cnt = launches;
+    for (int r = 1; r <= s->opt.llg_max_iter && !rc; ++r) {
+      // Iterates r >= 4 almost never run.  In the captured step they sit in ONE conditional (IF)
+      // node armed on the device by k_set_cond, so the usual step does not even launch them.
+      // (The node itself costs about as much as ten empty launches: only worth it for a long tail.)
+      if (r == 4 && s->capturing && s->aux && s->opt.use_graph == 1 && s->opt.llg_max_iter >= 12) {
+        rc = begin_cond_tail(s, r, &outer);
+        if (rc) break;
+        ++*launches;  // k_set_cond
+        cnt = &body_launches;
+      }
+      rc = enqueue_sweep(s, E, in, out, tmp, min, mout, r, cnt);
+    }
+    if (outer) {  // on every exit: close the body capture, give the handle its stream back
+      const int rc2 = end_cond_tail(s, outer);
+      if (!rc) rc = rc2;
+    }
+    if (rc) return rc;
+  }
+  return enqueue_half_end(s, out, tmp, s->opt.llg_max_iter, last, launches);
 }
 
 int count_sources(const fdtd_llg *s, int kind) {
@@ -791,8 +848,6 @@ int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, in
   return FDTD_LLG_OK;
 }
 
-// one full time step: HM half (curl E^n), E update, HM half (curl E^{n+1}).
-// H sets: state in 0 -> half 1 result in 1 -> half 2 result back in 0.  M sets: 0 -> 1 -> 0.
 // hard E / soft H / hard H sources of one kind: a small kernel per source on its box
 int enqueue_box_sources(fdtd_llg *s, int kind, double *const *F, int *launches) {
   for (int q = 0; q < s->src.count; ++q) {
@@ -815,30 +870,55 @@ int enqueue_box_sources(fdtd_llg *s, int kind, double *const *F, int *launches) 
   return FDTD_LLG_OK;
 }
 
-// one time step; par = parity of the step: E^n is in E set `par`, E^{n+1} goes to the other set
-int enqueue_step(fdtd_llg *s, int par, int *launches) {
-  *launches = 0;
-  double *const *Ea = par ? s->E2 : s->E, *const *Eb = par ? s->E : s->E2;
+// ---- the phases of one time step: HM half (curl E^n), E update, HM half
+// (curl E^{n+1}).  par = parity of the step: E^n is in E set `par`, E^{n+1} goes to the other set.
+// H sets: state in 0 -> half 1 result in set_half(par) -> half 2 result back in 0.  M: 0 -> 1 -> 0.
+double *const *e_set(fdtd_llg *s, int par) { return par ? s->E2 : s->E; }
+
+// merged H half-steps: the first step after set_fields takes the outside faces from t = 0 to dt/2
+int enqueue_prime(fdtd_llg *s, int par, int *launches) {
+  if (!s->merge || s->primed) return FDTD_LLG_OK;
+  int rc = enqueue_outside(s, e_set(s, par), 0, set_half(s, par), 1.0, true, launches);
+  if (rc) return rc;
+  s->primed = true;
+  s->prime_at = s->host_steps;
+  return FDTD_LLG_OK;
+}
+
+int enqueue_begin(fdtd_llg *s, int *launches) {
   if (s->src.count > 0) {
     prof_begin(s, FDTD_LLG_K_OTHER, 0);
     k_step_begin<<<1, 32, 0, s->stream>>>(s->dstate, s->src, s->dt);
     prof_end(s);
     ++*launches;
   }
-  int rc = enqueue_box_sources(s, FDTD_LLG_SRC_SOFT_H, s->Hset[0], launches);  // beginning of the step
+  return enqueue_box_sources(s, FDTD_LLG_SRC_SOFT_H, s->Hset[0], launches);  // beginning of the step
+}
+
+int enqueue_e_phase(fdtd_llg *s, int par, int *launches) {
+  double *const *Ea = e_set(s, par), *const *Eb = e_set(s, par ^ 1);
+  const int h1 = set_half(s, par);
+  int rc = enqueue_e(s, Ea, Eb, h1, launches);
   if (rc) return rc;
-  rc = enqueue_half(s, Ea, 0, 1, 2, 0, 1, false, launches);
+  rc = enqueue_pml(s, true, s->Hset[h1], Eb, launches);
   if (rc) return rc;
-  rc = enqueue_e(s, Ea, Eb, 1, launches);
+  return enqueue_box_sources(s, FDTD_LLG_SRC_HARD_E, Eb, launches);            // after the E update
+}
+
+int enqueue_step(fdtd_llg *s, int par, int *launches) {
+  *launches = 0;
+  const int h1 = set_half(s, par), tmp = set_tmp(s, par);
+  int rc = enqueue_begin(s, launches);
   if (rc) return rc;
-  rc = enqueue_pml(s, true, s->Hset[1], Eb, launches);
+  rc = enqueue_half(s, e_set(s, par), 0, h1, tmp, 0, 1, false, -1, launches);
   if (rc) return rc;
-  rc = enqueue_box_sources(s, FDTD_LLG_SRC_HARD_E, Eb, launches);              // after the E update
+  rc = enqueue_e_phase(s, par, launches);
   if (rc) return rc;
-  rc = enqueue_half(s, Eb, 1, 0, 2, 1, 0, true, launches);
+  rc = enqueue_half(s, e_set(s, par ^ 1), h1, 0, tmp, 1, 0, true, set_half(s, par ^ 1), launches);
   if (rc) return rc;
   return enqueue_box_sources(s, FDTD_LLG_SRC_HARD_H, s->Hset[0], launches);    // after the H update
 }
+
 int build_graph(fdtd_llg *s, int par) {
   if (s->graph[par]) { cudaGraphExecDestroy(s->graph[par]); s->graph[par] = nullptr; }
   s->graph_valid[par] = false;
@@ -856,6 +936,52 @@ int build_graph(fdtd_llg *s, int par) {
   if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
   s->launches_per_step = launches;
   s->graph_valid[par] = true;
+  return FDTD_LLG_OK;
+}
+
+// Merged H half-steps: form the integer-time H of the present state (time N) where it is kept at
+// half-integer time: H^N = H^{N-1/2} - (dt / 2 mu) curl E^N, the half-step the paper's scheme takes
+// (PAPER.md:94), from the set the last step read.  Returns the H set to read.
+int reconstruct_h(fdtd_llg *s, int *read_set) {
+  *read_set = 0;
+  if (!s->merge || !s->primed) return FDTD_LLG_OK;
+  const int par = (int)(s->host_steps & 1);       // parity of the NEXT step
+  const int dead = set_half(s, par ^ 1);          // H^{N-1/2} outside the box, no longer needed
+  const int target = s->opt.enable_llg ? 0 : dead;  // LLG storage: set 0 holds the box's H^N already
+  *read_set = target;
+  if (s->host_steps == s->prime_at) { *read_set = 0; return FDTD_LLG_OK; }  // set 0 still holds H^N
+  if (s->recon_valid) return FDTD_LLG_OK;
+  int launches = 0;
+  int rc = enqueue_outside(s, e_set(s, par), dead, target, 1.0, false, &launches);
+  if (rc) return rc;
+  s->recon_valid = true;
+  return FDTD_LLG_OK;
+}
+
+// leave the merged mode (an H source was added, which needs H at integer time): the state goes
+// back to set 0 at integer time
+int unmerge(fdtd_llg *s) {
+  if (!s->merge) return FDTD_LLG_OK;
+  int rs = 0;
+  int rc = reconstruct_h(s, &rs);
+  if (rc) return rc;
+  if (rs != 0)
+    for (int d = 0; d < 3; ++d)
+      CU(s, cudaMemcpyAsync(s->Hset[0][d], s->Hset[rs][d], s->stride * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+  s->merge = false;
+  s->primed = false;
+  s->recon_valid = false;
+  s->graph_valid[0] = s->graph_valid[1] = false;
+  return FDTD_LLG_OK;
+}
+
+// synchronise the stream and turn a pipeline time-out of a staged sweep into an error: the
+// fields are only partly updated then
+int check_pipe(fdtd_llg *s) {
+  int pe = 0;
+  CU(s, cudaMemcpyAsync(&pe, &s->dstate->pipe_error, sizeof pe, cudaMemcpyDeviceToHost, s->stream));
+  CU(s, cudaStreamSynchronize(s->stream));
+  if (pe) return fail(s, FDTD_LLG_ESTATE, "a TMA pipeline wait timed out (wait tag %d): results are invalid", pe);
   return FDTD_LLG_OK;
 }
 
@@ -883,11 +1009,13 @@ void fdtd_llg_default_options(fdtd_llg_options *o) {
   o->use_graph = 1;
   o->pml_r0 = 1e-6;
   o->pml_order = 3;
+  o->merge_h = 1;
 }
 
 size_t fdtd_llg_workspace_bytes(int nx, int ny, int nz, const fdtd_llg_options *opt,
                                 unsigned material_mask) {
   if (nx < 1 || ny < 1 || nz < 1 || !opt) return 0;
+  if (opt->llg_max_iter < 1 || opt->llg_max_iter > 1000) return 0;
   const size_t stride = array_stride(nx, ny, nz);
   size_t arrays = 12;                      // two E sets, two H sets (every update is out of place)
   if (opt->enable_llg) arrays += 3 + 18;   // the Jacobi H buffer, two M sets
@@ -931,10 +1059,21 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->g.sz = s->g.sy * (ny + 2);
   s->g.org = PADL + s->g.sy + s->g.sz;
   s->d[0] = dx; s->d[1] = dy; s->d[2] = dz;
-  for (int d = 0; d < 3; ++d) { s->g.per[d] = opt->bc[d] == FDTD_LLG_PERIODIC; s->g.rd[d] = 1.0 / s->d[d]; }
+  for (int d = 0; d < 3; ++d) {
+    s->g.per[d] = opt->bc[d] == FDTD_LLG_PERIODIC;
+    s->g.wall[d] = opt->bc[d] == FDTD_LLG_PEC;
+    s->g.rd[d] = 1.0 / s->d[d];
+  }
+  // a slab interface is neither wall nor wrap; with one interface the other z side keeps its wall
+  // (index 0 stays a wall face only if the LOW side is a real wall)
+  s->g.ext[0] = opt->slab_ext[0];
+  s->g.ext[1] = opt->slab_ext[1];
+  if (s->g.ext[0]) s->g.wall[2] = 0;
+  s->is_slab = s->g.ext[0] || s->g.ext[1];
   s->g.dt = dt;
   s->dt = dt;
   s->ncell = (size_t)nx * ny * nz;
+  s->ncell_user = (size_t)nx * ny * (size_t)(nz + s->g.ext[0] + s->g.ext[1]);
   s->stride = array_stride(nx, ny, nz);
   {
     int dev = 0, sms = 0;
@@ -997,11 +1136,12 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   make_boxes(s);
   s->n_arrays = (int)((q - s->E[0]) / (ptrdiff_t)s->stride);
   if ((rc = setup_pml(s, &q))) return bail(rc);
-  const bool smem_ok = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array;
-  s->stage_by = !smem_ok ? 0 : (opt->kernel_path == 0 || opt->kernel_path == 4 || opt->kernel_path == 5 ? 16 : (opt->kernel_path == 3 ? 7 : 0));
-  s->stage_lean = opt->kernel_path == 4;
-  if (s->stage_by == 16 && (rc = setup_hm_stage_by<16>(s))) return bail(rc);
-  if (s->stage_by == 7 && (rc = setup_hm_stage_by<7>(s))) return bail(rc);
+  // the staged sweeps need uniform alpha, gamma, mu_r and an even first column (TMA boxes on 16-byte
+  // boundaries); the direct-load kernels are the general path
+  s->staged = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array &&
+              (s->lo[0] & 1) == 0 && opt->kernel_path != 1;
+  if (s->staged && (rc = setup_hm_stage(s))) return bail(rc);
+  s->merge = merge_allowed(s);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
   *out = s;
@@ -1027,7 +1167,7 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
   FieldsP f{};
   f.g = s->g;
   for (int d = 0; d < 3; ++d) { f.E[d] = s->E[d]; f.H[d] = s->Hset[0][d]; }
-  k_enforce_walls<<<grid_1d(s, (long long)s->ncell), 256, 0, s->stream>>>(f);
+  k_enforce_walls<<<grid_1d(s, (long long)s->ncell_user), 256, 0, s->stream>>>(f);
   CU(s, cudaGetLastError());
   for (int d = 0; d < 3; ++d) {
     if ((rc = fill_ghosts(s, s->E[d]))) return rc;
@@ -1078,6 +1218,9 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
   CU(s, cudaStreamSynchronize(s->stream));
   s->host_steps = 0;
   s->kernel_launches = 0;
+  s->primed = false;
+  s->recon_valid = false;
+  s->sub_next = FDTD_LLG_SUB_BEGIN;
   return FDTD_LLG_OK;
 }
 
@@ -1108,6 +1251,11 @@ int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const in
     for (int d = 0; d < 3; ++d)
       if (lo[d] < s->opt.pml[2 * d] || hi[d] > s->g.n[d] - s->opt.pml[2 * d + 1])
         return fail(s, FDTD_LLG_EINVAL, "hard / soft field sources must lie outside the PML");
+  if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
+  if (kind == FDTD_LLG_SRC_SOFT_H || kind == FDTD_LLG_SRC_HARD_H) {  // these act on H at integer time
+    int rc = unmerge(s);
+    if (rc) return rc;
+  }
   SourceP &S = s->src.s[s->src.count];
   S.kind = kind;
   S.comp = comp;
@@ -1134,45 +1282,55 @@ int fdtd_llg_step(fdtd_llg *s, int n) {
   if (!s) return FDTD_LLG_EINVAL;
   if (n < 0) return fail(s, FDTD_LLG_EINVAL, "n must be >= 0");
   if (n == 0) return FDTD_LLG_OK;
-  if (s->opt.use_graph) {
-    for (int t = 0; t < n; ++t) {
-      const int par = (int)((s->host_steps + t) & 1);
-      if (!s->graph_valid[par]) {
-        int rc = build_graph(s, par);
-        if (rc) return rc;
-      }
-      CU(s, cudaGraphLaunch(s->graph[par], s->stream));
-    }
-  } else {
-    for (int t = 0; t < n; ++t) {
+  if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
+  if (s->g.dlo != 0 || s->g.dhi != 0)
+    return fail(s, FDTD_LLG_ESTATE, "a connected slab is advanced with fdtd_llg_substep (the caller orders the slabs)");
+  int rc = FDTD_LLG_OK, done = 0, extra = 0;
+  rc = enqueue_prime(s, (int)(s->host_steps & 1), &extra);
+  for (int t = 0; t < n && !rc; ++t) {
+    const int par = (int)((s->host_steps + t) & 1);
+    if (s->opt.use_graph) {
+      if (!s->graph_valid[par]) rc = build_graph(s, par);
+      if (!rc && cudaGraphLaunch(s->graph[par], s->stream) != cudaSuccess)
+        rc = fail(s, FDTD_LLG_ECUDA, "cudaGraphLaunch: %s", cudaGetErrorString(cudaGetLastError()));
+    } else {
       int launches = 0;
-      int rc = enqueue_step(s, (int)((s->host_steps + t) & 1), &launches);
-      if (rc) return rc;
-      s->launches_per_step = launches;
+      rc = enqueue_step(s, par, &launches);
+      if (!rc) s->launches_per_step = launches;
     }
+    if (!rc) ++done;
   }
-  s->host_steps += n;
-  s->kernel_launches += (long long)n * s->launches_per_step;
-  return FDTD_LLG_OK;
+  // the steps that were enqueued count, also when a later one failed: the E-set parity and
+  // fdtd_llg_read_fields follow the device
+  s->host_steps += done;
+  s->kernel_launches += (long long)done * s->launches_per_step + extra;
+  if (done) s->recon_valid = false;
+  return rc;
 }
 
 int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *launches_by_class) {
   if (!s) return FDTD_LLG_EINVAL;
   if (n < 1 || n > R_HIST / 2) return fail(s, FDTD_LLG_EINVAL, "n must be in 1..%d", R_HIST / 2);
   if (!ms_by_class || !launches_by_class) return fail(s, FDTD_LLG_EINVAL, "output array is NULL");
+  if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
+  if (s->g.dlo != 0 || s->g.dhi != 0) return fail(s, FDTD_LLG_ESTATE, "a connected slab is advanced with fdtd_llg_substep");
   std::vector<fdtd_llg::ProfRec> recs;
   DevState h0{};
   CU(s, cudaMemcpyAsync(&h0, s->dstate, sizeof h0, cudaMemcpyDeviceToHost, s->stream));
   CU(s, cudaStreamSynchronize(s->stream));
+  int rc = FDTD_LLG_OK, done = 0, extra = 0;
+  rc = enqueue_prime(s, (int)(s->host_steps & 1), &extra);
   s->prof = &recs;
   s->prof_half = 0;
-  int rc = FDTD_LLG_OK;
   for (int t = 0; t < n && !rc; ++t) {
     int launches = 0;
     rc = enqueue_step(s, (int)((s->host_steps + t) & 1), &launches);
-    s->launches_per_step = launches;
+    if (!rc) { s->launches_per_step = launches; ++done; }
   }
   s->prof = nullptr;
+  s->host_steps += done;
+  s->kernel_launches += (long long)done * s->launches_per_step + extra;
+  if (done) s->recon_valid = false;
   cudaError_t e = cudaStreamSynchronize(s->stream);
   std::vector<int> hist(R_HIST);
   if (e == cudaSuccess)
@@ -1192,9 +1350,7 @@ int fdtd_llg_step_timed(fdtd_llg *s, int n, double *ms_by_class, long long *laun
   }
   if (rc) return rc;
   if (e != cudaSuccess) return fail(s, FDTD_LLG_ECUDA, "step_timed: %s", cudaGetErrorString(e));
-  s->host_steps += n;
-  s->kernel_launches += (long long)n * s->launches_per_step;
-  return FDTD_LLG_OK;
+  return check_pipe(s);
 }
 
 int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double *const *M,
@@ -1202,11 +1358,13 @@ int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double
   if (!s) return FDTD_LLG_EINVAL;
   if (mem_space != FDTD_LLG_HOST && mem_space != FDTD_LLG_DEVICE)
     return fail(s, FDTD_LLG_EINVAL, "mem_space must be FDTD_LLG_HOST or FDTD_LLG_DEVICE");
+  if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
   const size_t bytes = s->ncell * sizeof(double);
-  int rc;
+  int rc, hset = 0;
+  if (H && (H[0] || H[1] || H[2]) && (rc = reconstruct_h(s, &hset))) return rc;
   for (int d = 0; d < 3; ++d) {
     if (E && E[d] && (rc = copy_out(s, E[d], ((s->host_steps & 1) ? s->E2 : s->E)[d], mem_space))) return rc;
-    if (H && H[d] && (rc = copy_out(s, H[d], s->Hset[0][d], mem_space))) return rc;
+    if (H && H[d] && (rc = copy_out(s, H[d], s->Hset[hset][d], mem_space))) return rc;
   }
   if (M)
     for (int c = 0; c < 9; ++c)
@@ -1215,8 +1373,7 @@ int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double
         else if (mem_space == FDTD_LLG_HOST) std::memset(M[c], 0, bytes);
         else CU(s, cudaMemsetAsync(M[c], 0, bytes, s->stream));
       }
-  CU(s, cudaStreamSynchronize(s->stream));
-  return FDTD_LLG_OK;
+  return check_pipe(s);
 }
 
 int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
@@ -1227,6 +1384,7 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   if (h.pipe_error)
     return fail(s, FDTD_LLG_ESTATE, "a TMA pipeline wait timed out (wait tag %d): results are invalid", h.pipe_error);
   std::memset(out, 0, sizeof *out);
+  out->merged_h = s->merge ? 1 : 0;
   out->steps = h.steps;
   out->time = (double)h.steps * s->dt;
   out->iters_last = h.iters_last;
@@ -1243,7 +1401,7 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   out->material_array_mask = (s->eps_r.is_array ? 1u : 0) | (s->sigma.is_array ? 2u : 0) |
                              (s->mu_r.is_array ? 4u : 0) | (s->Ms.is_array ? 8u : 0) |
                              (s->alpha.is_array ? 16u : 0) | (s->gamma.is_array ? 32u : 0);
-  out->staged_sweeps = s->stage_by != 0;
+  out->staged_sweeps = s->staged ? 1 : 0;
   out->sweep_cells = 0;
   if (s->llg) {
     out->sweep_cells = 1;
@@ -1262,6 +1420,145 @@ void fdtd_llg_destroy(fdtd_llg *s) {
     if (s->graph[p]) cudaGraphExecDestroy(s->graph[p]);
   if (s->aux) cudaStreamDestroy(s->aux);
   delete s;
+}
+
+// ------------------------------------------------------------------------------- z-slabs
+
+int fdtd_llg_get_slab_info(fdtd_llg *s, fdtd_llg_slab_info *out) {
+  if (!s || !out) return FDTD_LLG_EINVAL;
+  out->fields_offset = (unsigned long long)(reinterpret_cast<char *>(s->E[0]) - s->ws);
+  out->array_stride = (unsigned long long)s->stride;
+  out->nx = s->g.n[0]; out->ny = s->g.n[1]; out->nz = s->g.n[2];
+  out->n_arrays = 6 + 3 * (s->opt.enable_llg ? 3 : 2) + (s->opt.enable_llg ? 18 : 0);
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_slab_connect(fdtd_llg *s, const fdtd_llg_slab_info *lo, void *lo_workspace,
+                          const fdtd_llg_slab_info *hi, void *hi_workspace) {
+  if (!s) return FDTD_LLG_EINVAL;
+  if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
+  fdtd_llg_slab_info me;
+  fdtd_llg_get_slab_info(s, &me);
+  const fdtd_llg_slab_info *nb[2] = {lo, hi};
+  void *ws[2] = {lo_workspace, hi_workspace};
+  long long delta[2] = {0, 0};
+  for (int sd = 0; sd < 2; ++sd) {
+    if (!nb[sd]) continue;
+    if (!s->g.ext[sd]) return fail(s, FDTD_LLG_EINVAL, "side %d is not a slab interface (options.slab_ext)", sd);
+    if (!ws[sd]) return fail(s, FDTD_LLG_EINVAL, "neighbour workspace is NULL");
+    if (nb[sd]->nx != me.nx || nb[sd]->ny != me.ny || nb[sd]->nz != me.nz ||
+        nb[sd]->array_stride != me.array_stride || nb[sd]->n_arrays != me.n_arrays)
+      return fail(s, FDTD_LLG_EINVAL, "slabs must have the same nx, ny, nz and field storage (neighbour: %d x %d x %d, %d arrays)",
+                  nb[sd]->nx, nb[sd]->ny, nb[sd]->nz, nb[sd]->n_arrays);
+    const char *theirs = static_cast<const char *>(ws[sd]) + nb[sd]->fields_offset;
+    const long long base = (long long)(theirs - reinterpret_cast<const char *>(s->E[0]));
+    const long long plane = 8LL * s->g.sz * s->g.n[2];
+    // my (i,j,0) is their (i,j,nz); my (i,j,nz-1) is their (i,j,-1)
+    delta[sd] = sd == 0 ? base + plane : base - plane;
+    if (delta[sd] == 0) return fail(s, FDTD_LLG_EINVAL, "neighbour workspace overlaps this one");
+  }
+  s->g.dlo = delta[0];
+  s->g.dhi = delta[1];
+  s->graph_valid[0] = s->graph_valid[1] = false;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_substep(fdtd_llg *s, int phase, int r) {
+  if (!s) return FDTD_LLG_EINVAL;
+  const bool hm = phase == FDTD_LLG_SUB_HM1 || phase == FDTD_LLG_SUB_HM2;
+  // order: BEGIN, HM1 r = 1, 2, ..., HM1_END, E, HM2 r = 1, 2, ..., HM2_END
+  const bool in_order = hm ? ((phase == s->sub_next && r == 1) || (phase + 1 == s->sub_next && r == s->sub_r + 1))
+                           : phase == s->sub_next && (phase == FDTD_LLG_SUB_BEGIN || phase == FDTD_LLG_SUB_E || s->sub_r >= 1);
+  if (phase < FDTD_LLG_SUB_BEGIN || phase > FDTD_LLG_SUB_HM2_END || !in_order)
+    return fail(s, FDTD_LLG_ESTATE, "sub-step %d (r = %d) out of order: expected phase %d", phase, r, s->sub_next);
+  if (hm && (r < 1 || r > s->opt.llg_max_iter)) return fail(s, FDTD_LLG_EINVAL, "r must be in 1..llg_max_iter");
+  const int par = (int)(s->host_steps & 1);
+  const int h1 = set_half(s, par), tmp = set_tmp(s, par);
+  int launches = 0, rc = FDTD_LLG_OK;
+  switch (phase) {
+    case FDTD_LLG_SUB_BEGIN:
+      rc = enqueue_prime(s, par, &launches);
+      if (!rc) rc = enqueue_begin(s, &launches);
+      s->sub_next = FDTD_LLG_SUB_HM1;
+      s->sub_r = 0;
+      break;
+    case FDTD_LLG_SUB_HM1:
+      if (r == 1) rc = enqueue_half_pre(s, e_set(s, par), 0, h1, -1, &launches);
+      if (!rc && s->llg) rc = enqueue_sweep(s, e_set(s, par), 0, h1, tmp, 0, 1, r, &launches);
+      s->sub_next = FDTD_LLG_SUB_HM1_END;
+      s->sub_r = r;
+      break;
+    case FDTD_LLG_SUB_HM1_END:
+      rc = enqueue_half_end(s, h1, tmp, s->sub_r, false, &launches);
+      s->sub_next = FDTD_LLG_SUB_E;
+      break;
+    case FDTD_LLG_SUB_E:
+      rc = enqueue_e_phase(s, par, &launches);
+      s->sub_next = FDTD_LLG_SUB_HM2;
+      s->sub_r = 0;
+      break;
+    case FDTD_LLG_SUB_HM2:
+      if (r == 1) rc = enqueue_half_pre(s, e_set(s, par ^ 1), h1, 0, set_half(s, par ^ 1), &launches);
+      if (!rc && s->llg) rc = enqueue_sweep(s, e_set(s, par ^ 1), h1, 0, tmp, 1, 0, r, &launches);
+      s->sub_next = FDTD_LLG_SUB_HM2_END;
+      s->sub_r = r;
+      break;
+    default:  // FDTD_LLG_SUB_HM2_END
+      rc = enqueue_half_end(s, 0, tmp, s->sub_r, true, &launches);
+      if (!rc) rc = enqueue_box_sources(s, FDTD_LLG_SRC_HARD_H, s->Hset[0], &launches);
+      s->sub_next = FDTD_LLG_SUB_BEGIN;
+      s->host_steps += 1;
+      s->recon_valid = false;
+      break;
+  }
+  s->kernel_launches += launches;
+  return rc;
+}
+
+int fdtd_llg_residual_word(fdtd_llg *s, int r, void **dev_ptr) {
+  if (!s || !dev_ptr) return FDTD_LLG_EINVAL;
+  if (r < 0 || r > s->opt.llg_max_iter) return fail(s, FDTD_LLG_EINVAL, "r must be in 0..llg_max_iter");
+  *dev_ptr = s->resid + r;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_ipc_export(fdtd_llg *s, unsigned char *handle64, unsigned long long *offset) {
+  if (!s || !handle64 || !offset) return FDTD_LLG_EINVAL;
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+  // the handle names the whole allocation the workspace was cut from (a caching allocator's block)
+  typedef CUresult (*RangeFn)(CUdeviceptr *, size_t *, CUdeviceptr);
+  void *fp = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fp, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess || !fp)
+    return fail(s, FDTD_LLG_ECUDA, "cuMemGetAddressRange is not available");
+  CUdeviceptr base = 0;
+  size_t size = 0;
+  if (reinterpret_cast<RangeFn>(fp)(&base, &size, (CUdeviceptr)(uintptr_t)s->ws) != CUDA_SUCCESS)
+    return fail(s, FDTD_LLG_ECUDA, "cuMemGetAddressRange failed on the workspace");
+  cudaIpcMemHandle_t h;
+  CU(s, cudaIpcGetMemHandle(&h, reinterpret_cast<void *>((uintptr_t)base)));
+  std::memcpy(handle64, &h, sizeof h);
+  *offset = (unsigned long long)((uintptr_t)s->ws - (uintptr_t)base);
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_ipc_open(const unsigned char *handle64, unsigned long long offset, void **dev_ptr) {
+  if (!handle64 || !dev_ptr) return fail(nullptr, FDTD_LLG_EINVAL, "NULL argument");
+  cudaIpcMemHandle_t h;
+  std::memcpy(&h, handle64, sizeof h);
+  void *base = nullptr;
+  cudaError_t e = cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess);
+  if (e != cudaSuccess) return fail(nullptr, FDTD_LLG_ECUDA, "cudaIpcOpenMemHandle: %s", cudaGetErrorString(e));
+  *dev_ptr = static_cast<char *>(base) + offset;
+  return FDTD_LLG_OK;
+}
+
+int fdtd_llg_ipc_close(void *dev_ptr, unsigned long long offset) {
+  if (!dev_ptr) return FDTD_LLG_OK;
+  cudaError_t e = cudaIpcCloseMemHandle(static_cast<char *>(dev_ptr) - offset);
+  if (e != cudaSuccess) return fail(nullptr, FDTD_LLG_ECUDA, "cudaIpcCloseMemHandle: %s", cudaGetErrorString(e));
+  return FDTD_LLG_OK;
 }
 
 }  // extern "C"

@@ -33,17 +33,12 @@ struct StBox {
   int ntx, nty, kz, items;
 };
 
-// what one launch of the staged sweep does
-enum StMode {
-  ST_FIRST = 0,    // r = 1, stores M^1 and H^1
-  ST_ITER = 1,     // r >= 2, reads M^{r-1}, H^{r-1}, stores M^r, H^r
-  ST_FIRST_H = 2,  // r = 1, stores H^1 only: the r = 2 sweep recomputes M^1 (9 words less written)
-  ST_ITER_RE = 3   // r = 2 after ST_FIRST_H: M^1 recomputed from M^n, H^n (9 words less read)
-};
-__host__ __device__ constexpr bool st_first(int mode) { return mode == ST_FIRST || mode == ST_FIRST_H; }
+constexpr int SBY = 16;        // tile rows: one compute warp each
 
-template <int BY, bool FIRST, bool MS_ARR>
+// FIRST: the r = 1 sweep (no H^{r-1} set staged, M^{r-1} = M^n); otherwise an iterate r >= 2
+template <bool FIRST, bool MS_ARR>
 struct StLayout {
+  static constexpr int BY = SBY;
   static constexpr int ROWS = BY + 1;
   static constexpr int SLOT = round16(ROWS * SROW);  // doubles per staged array
   static constexpr int HN = 0;                       // H^n x, y, z
@@ -53,9 +48,8 @@ struct StLayout {
   static constexpr int NSLOT = (FIRST ? 6 : 9) + (MS_ARR ? 1 : 0);
   static constexpr int STAGE = NSLOT * SLOT;
   static constexpr unsigned BYTES = 8u * NSLOT * ROWS * SROW;  // bytes the TMA writes per stage
-  // ring depth: two live stages + as many in flight as fit (one block per SM for BY >= 12, two below)
-  static constexpr int BPS = BY >= 12 ? 1 : 2;  // blocks per SM
-  static constexpr int BUDGET = (BPS == 1 ? 220 : 108) * 1024;
+  // ring depth: two live stages + as many in flight as fit; one block per SM
+  static constexpr int BUDGET = 220 * 1024;
   static constexpr int NS_FIT = BUDGET / (8 * STAGE);
   static constexpr int NS = NS_FIT > 8 ? 8 : NS_FIT;
   static constexpr int NCW = BY;  // compute warps
@@ -65,7 +59,7 @@ struct StLayout {
 };
 
 // registers are granted in steps that allow 512 threads per SM at 128 and 640 at 96
-constexpr int st_maxreg(int by) { return (by + 1) * 32 * (by >= 12 ? 1 : 2) <= 512 ? 128 : 96; }
+constexpr int ST_MAXREG = (SBY + 1) * 32 <= 512 ? 128 : 96;
 
 struct HMSArgs {
   HMArgs a;  // scalars, M / H pointers, residual words
@@ -74,8 +68,7 @@ struct HMSArgs {
   CUtensorMap mapM;  // box (SW, BY, 1, 9): L2 prefetch of an M set's plane
   int aE, aHn, aHp, aMn, aMp, aMs;  // array indices (4th tensor coordinate)
   unsigned *work;  // item counter of this launch (zero at launch; k_half_end re-arms it)
-  int cond;        // 0: always run; 1: run iff iterate r-1 was not converged; 2: run iff iterate 1
-                   // WAS converged (the full r = 1 sweep after ST_FIRST_H, when M^1 is the result)
+  int cond;        // 0: always run; 1: run iff iterate r-1 was not converged
 };
 
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int c0, int c1, int c2, int c3) {
@@ -168,7 +161,7 @@ __device__ __forceinline__ double s_curl(const GridP &g, const double *A, const 
 }
 
 // One Jacobi iterate on the D-face of this thread's cell, neighbour operands from the ring
-template <class L, int D, bool FIRST, bool MS_ARR, bool ANISO, bool RECOMP>
+template <class L, int D, bool FIRST, bool MS_ARR, bool ANISO>
 __device__ __forceinline__ FaceOut s_face(const HMArgs &a, const double *A, const double *B, int t,
                                           const Vec3 &mn, const Vec3 &mp, bool wall) {
   double Msf = a.Ms_u, rMs = a.rMs_u;
@@ -182,8 +175,8 @@ __device__ __forceinline__ FaceOut s_face(const HMArgs &a, const double *A, cons
   Vec3 he = hn;
   if (!FIRST) he = s_hem<L, L::HP, D>(A, B, t);
   const double C = s_curl<L, D>(a.g, A, B, t);
-  return hm_face_core<D, FIRST, ANISO, RECOMP>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.cf_u,
-                                               a.ch_uniform, wall);
+  return hm_face_core<D, FIRST, ANISO>(a, mn, mp, hn, he, C, Msf, rMs, a.alpha_u, a.cf_u,
+                                       a.ch_uniform, wall);
 }
 
 template <int D, bool LOAD_MP>
@@ -218,11 +211,11 @@ __device__ __forceinline__ void s_issue_stage(const HMSArgs &p, double *dst, uin
 struct StItem {
   int x0, y0, k0, k1;
 };
-__device__ __forceinline__ StItem st_decode(const StBox &T, int it, int by) {
+__device__ __forceinline__ StItem st_decode(const StBox &T, int it) {
   const int tx = it % T.ntx, q = it / T.ntx, ty = q % T.nty, tz = q / T.nty;
   StItem w;
   w.x0 = T.lo[0] + tx * SW;
-  w.y0 = T.lo[1] + ty * by;
+  w.y0 = T.lo[1] + ty * SBY;
   w.k0 = T.lo[2] + tz * T.kz;
   w.k1 = min(w.k0 + T.kz, T.hi[2]);
   return w;
@@ -231,18 +224,14 @@ __device__ __forceinline__ StItem st_decode(const StBox &T, int it, int by) {
 // Work items are handed out dynamically (one atomic per item on p.work): SMs do not all stream at
 // the same rate, and a static split leaves the fast ones idle at the end.  The producer publishes
 // the item of every stage in meta[slot] before arming the stage's barrier; item < 0 ends the march.
-template <int BY, int MODE, bool MS_ARR, bool ANISO>
-__global__ void __maxnreg__(st_maxreg(BY))
+template <bool FIRST, bool MS_ARR, bool ANISO>
+__global__ void __maxnreg__(ST_MAXREG)
 k_hm_stage(const __grid_constant__ HMSArgs p) {
-  constexpr bool FIRST = st_first(MODE);        // no H^{r-1} set, H_eff^{r-1} = H_eff^n
-  constexpr bool LOAD_MP = MODE == ST_ITER;     // M^{r-1} read from memory
-  constexpr bool RECOMP = MODE == ST_ITER_RE;   // M^1 recomputed
-  constexpr bool STORE_M = MODE != ST_FIRST_H;
-  using L = StLayout<BY, FIRST, MS_ARR>;
+  constexpr bool LOAD_MP = !FIRST;              // M^{r-1} read from memory
+  using L = StLayout<FIRST, MS_ARR>;
   const HMArgs &a = p.a;
   // the whole grid takes the same decision (the stopping test is global)
   if (p.cond == 1 && __longlong_as_double((long long)a.resid[a.r - 1]) < a.tol) return;
-  if (p.cond == 2 && !(__longlong_as_double((long long)a.resid[1]) < a.tol)) return;
   // dynamic shared memory starts on a 1 KB boundary of the CTA's window (no static shared memory in
   // this kernel); keeping the pointer a plain offset of the __shared__ array lets the compiler
   // address the ring with LDS instead of generic loads
@@ -258,6 +247,7 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
     for (int s = 0; s < L::NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, L::NCW); }
     mbar_fence_init();
   }
+  if (threadIdx.x < L::NCW) wmax[threadIdx.x] = 0.0;   // a warp that leaves on a pipeline error adds nothing
   __syncthreads();
 
   const StBox &T = p.tb;
@@ -271,7 +261,7 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
       for (;;) {
         const int it = (int)atomicAdd(p.work, 1u);
         const bool end = it >= T.items;
-        const StItem w = st_decode(T, end ? 0 : it, BY);
+        const StItem w = st_decode(T, end ? 0 : it);
         if (!end) {  // the first M plane of a fresh column, towards L2
           tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMn);
           if (LOAD_MP) tma_prefetch_4d(&p.mapM, PADL + w.x0, w.y0 + 1, w.k0 + 1, p.aMp);
@@ -304,7 +294,7 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
       if (!mbar_wait(full + n % L::NS, (n / L::NS) & 1, a.pipe_error, 2)) goto done;
       const int it = *(volatile int *)(meta + n % L::NS);
       if (it < 0) break;
-      const StItem w = st_decode(T, it, BY);
+      const StItem w = st_decode(T, it);
       const int i = w.x0 + lane, j = w.y0 + warp;
       const bool valid = i < T.hi[0] && j < T.hi[1];
       const Column col = make_column(a.g, i, j);
@@ -325,26 +315,23 @@ k_hm_stage(const __grid_constant__ HMSArgs p) {
           const bool edge = col.edge_ij || edge_k(a.g, k);
           const bool more = k + 1 < w.k1;
           {
-            const FaceOut o = s_face<L, 0, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn0, LOAD_MP ? mp0 : mn0, col.wall[0]);
+            const FaceOut o = s_face<L, 0, FIRST, MS_ARR, ANISO>(a, A, B, t, mn0, LOAD_MP ? mp0 : mn0, col.wall[0]);
             if (more) s_load_m<0, LOAD_MP>(a, c + a.g.sz, mn0, mp0);
-            if (STORE_M) store_face<0>(a, c, o);
-            else a.Hc[0][c] = o.h;
+            store_face<0>(a, c, o);
             if (edge) store_face_images<0>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }
           {
-            const FaceOut o = s_face<L, 1, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn1, LOAD_MP ? mp1 : mn1, col.wall[1]);
+            const FaceOut o = s_face<L, 1, FIRST, MS_ARR, ANISO>(a, A, B, t, mn1, LOAD_MP ? mp1 : mn1, col.wall[1]);
             if (more) s_load_m<1, LOAD_MP>(a, c + a.g.sz, mn1, mp1);
-            if (STORE_M) store_face<1>(a, c, o);
-            else a.Hc[1][c] = o.h;
+            store_face<1>(a, c, o);
             if (edge) store_face_images<1>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }
           {
-            const FaceOut o = s_face<L, 2, FIRST, MS_ARR, ANISO, RECOMP>(a, A, B, t, mn2, LOAD_MP ? mp2 : mn2, wall_k(a.g, k));
+            const FaceOut o = s_face<L, 2, FIRST, MS_ARR, ANISO>(a, A, B, t, mn2, LOAD_MP ? mp2 : mn2, wall_k(a.g, k));
             if (more) s_load_m<2, LOAD_MP>(a, c + a.g.sz, mn2, mp2);
-            if (STORE_M) store_face<2>(a, c, o);
-            else a.Hc[2][c] = o.h;
+            store_face<2>(a, c, o);
             if (edge) store_face_images<2>(a, i, j, k, c, o);
             res = fmax(res, o.res);
           }

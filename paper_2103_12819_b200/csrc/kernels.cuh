@@ -11,6 +11,10 @@
 //   interior plane and are refreshed IN-KERNEL by the thread that writes the
 //   boundary cell.  Hence every stencil neighbour is a constant offset from the centre: no index
 //   arithmetic, no predicates in the inner loops.
+//   A z side that is an INTERFACE to a neighbouring slab (multi-GPU z-slab decomposition, PAPER.md:195,
+//   217) is no wall: its ghost plane holds the neighbour's adjacent plane, and the thread that
+//   writes a value of the slab's first / last plane also stores it into the neighbour's ghost plane
+//   through peer-mapped memory (store_images_inl), so the halo exchange is part of the update.
 //
 // THREADING.  A block is TX x TY columns (x fastest, coalesced 256-byte rows) and marches KZ planes
 // in z, so the k-1 / k+1 neighbours of consecutive planes are served by L1.  Grids are persistent
@@ -44,9 +48,14 @@ constexpr double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
 
 struct GridP {
   int n[3];    // nx, ny, nz
-  int per[3];  // 1 = periodic, 0 = PEC
+  int per[3];  // 1 = periodic (the ghost layer mirrors the opposite interior plane)
+  int wall[3]; // 1 = PEC wall at index 0 and at index n
+  int ext[2];  // z-low / z-high side is an interface to a neighbouring slab (neither of the above)
   int sy, sz;  // element strides of j and k (the stride of i is 1)
   int org;     // offset of cell (0,0,0)
+  // BYTE offsets from an element of this slab's first (dlo) / last (dhi) plane to its image in the
+  // lower / upper neighbour's ghost plane (same array, the neighbour's workspace); 0 = not connected
+  long long dlo, dhi;
   double rd[3];  // 1/dx, 1/dy, 1/dz
   double dt;
 };
@@ -96,7 +105,6 @@ template <int D> __device__ __forceinline__ int stride_of(const GridP &g) {
 struct Cell {
   int i, j, k;
   int c;      // element offset of (i,j,k)
-  bool edge;  // on the first / last plane of a periodic axis: its stores have ghost images
 };
 
 // per-column (i,j) part of the predicates, hoisted out of the z march
@@ -109,18 +117,28 @@ __device__ __forceinline__ Column make_column(const GridP &g, int i, int j) {
   Column q;
   q.i = i; q.j = j;
   q.edge_ij = (g.per[0] && (i == 0 || i == g.n[0] - 1)) || (g.per[1] && (j == 0 || j == g.n[1] - 1));
-  q.wall[0] = !g.per[0] && i == 0;
-  q.wall[1] = !g.per[1] && j == 0;
+  q.wall[0] = g.wall[0] && i == 0;
+  q.wall[1] = g.wall[1] && j == 0;
   return q;
 }
+// a value of plane k has images: periodic ghosts, or the ghost plane of a connected neighbour slab
 __device__ __forceinline__ bool edge_k(const GridP &g, int k) {
-  return g.per[2] && (k == 0 || k == g.n[2] - 1);
+  return ((g.per[2] || g.dlo != 0) && k == 0) || ((g.per[2] || g.dhi != 0) && k == g.n[2] - 1);
 }
-__device__ __forceinline__ bool wall_k(const GridP &g, int k) { return !g.per[2] && k == 0; }
+__device__ __forceinline__ bool wall_k(const GridP &g, int k) { return g.wall[2] && k == 0; }
 
-// slow path of a store: the periodic ghost images of an interior value, inlined
-// (no call: a call would wait for every load
-// the caller has in flight).  Up to two shifts per axis (both when the axis is one cell long).
+// What a slab hands to its z neighbours: the curl of E and the four-point averages
+// of an x- or y-face reach one plane UP (E_x, E_y, H_z of the upper neighbour's first plane), the curl
+// of H and the averages of a z-face one plane DOWN (H_x, H_y of the lower neighbour's last plane).
+enum { EXP_NONE = 0, EXP_LO = 1, EXP_HI = 2 };
+template <int D> __host__ __device__ constexpr int exp_of_h() { return D == 2 ? EXP_LO : EXP_HI; }
+template <int D> __host__ __device__ constexpr int exp_of_e() { return D == 2 ? EXP_NONE : EXP_LO; }
+
+// slow path of a store: the periodic ghost images of an interior value and, for a
+// component the neighbouring slab reads (EXP), its image in that slab's ghost plane.  Inlined (no
+// call: a call would wait for every load the caller has in flight).  Up to two shifts per axis
+// (both when the axis is one cell long).
+template <int EXP>
 __device__ __forceinline__ void store_images_inl(double *a, const GridP &g, int i, int j, int k,
                                                  int c, double v) {
   const int sx[3] = {0, (g.per[0] && i == 0) ? g.n[0] : 0, (g.per[0] && i == g.n[0] - 1) ? -g.n[0] : 0};
@@ -128,16 +146,24 @@ __device__ __forceinline__ void store_images_inl(double *a, const GridP &g, int 
                      (g.per[1] && j == g.n[1] - 1) ? -g.n[1] * g.sy : 0};
   const int sz[3] = {0, (g.per[2] && k == 0) ? g.n[2] * g.sz : 0,
                      (g.per[2] && k == g.n[2] - 1) ? -g.n[2] * g.sz : 0};
+  const bool rlo = (EXP & EXP_LO) && g.dlo != 0 && k == 0;
+  const bool rhi = (EXP & EXP_HI) && g.dhi != 0 && k == g.n[2] - 1;
 #pragma unroll
   for (int x = 0; x < 3; ++x)
 #pragma unroll
-    for (int y = 0; y < 3; ++y)
+    for (int y = 0; y < 3; ++y) {
+      if ((x && !sx[x]) || (y && !sy[y])) continue;
+      const int cxy = c + sx[x] + sy[y];
 #pragma unroll
       for (int z = 0; z < 3; ++z) {
         if (!(x | y | z)) continue;
-        if ((x && !sx[x]) || (y && !sy[y]) || (z && !sz[z])) continue;
-        a[c + sx[x] + sy[y] + sz[z]] = v;
+        if (z && !sz[z]) continue;
+        a[cxy + sz[z]] = v;
       }
+      // peer stores (NVLink): the neighbour's ghost plane, including its periodic x / y ghosts
+      if (EXP & EXP_LO) { if (rlo) *reinterpret_cast<double *>(reinterpret_cast<char *>(a + cxy) + g.dlo) = v; }
+      if (EXP & EXP_HI) { if (rhi) *reinterpret_cast<double *>(reinterpret_cast<char *>(a + cxy) + g.dhi) = v; }
+    }
 }
 
 // (curl E)_D at the D-face: forward differences (standard Yee)
@@ -187,6 +213,8 @@ struct HArgs {
   double *Hc[3];
   const double *mu_r;  // cell-centred array or nullptr (uniform)
   double ch_uniform;   // dt / (2 mu0 mu_r) when uniform
+  double cmul;         // 1: half a step (eq. 21); 2: the two adjacent half-steps of a face that no
+                       // magnetic face reads, taken at once with the same curl E
 };
 
 // eq. 21 with M = 0 and the local mu; a PEC wall face stays 0
@@ -198,8 +226,8 @@ __device__ __forceinline__ double h_face(const HArgs &a, int c, bool wall) {
     ch = a.g.dt / (2.0 * kMu0 * mu);
   }
   const double C = curl_e<D>(a.g, c, a.E);
-  // plain load: Hn aliases Hc when the update is done in place (Maxwell-only runs)
-  const double h = a.Hn[D][c] - ch * C;
+  // plain load: Hn aliases Hc when the integer-time H is formed in place (reconstruct_h)
+  const double h = a.Hn[D][c] - (a.cmul * ch) * C;   // cmul = 1, 2: an exact scaling
   return wall ? 0.0 : h;
 }
 
@@ -218,9 +246,9 @@ __global__ void __launch_bounds__(NTHREADS) k_h_update(const __grid_constant__ H
       a.Hc[1][c] = hy;
       a.Hc[2][c] = hz;
       if (col.edge_ij || edge_k(a.g, k)) {
-        store_images_inl(a.Hc[0], a.g, w.i, w.j, k, c, hx);
-        store_images_inl(a.Hc[1], a.g, w.i, w.j, k, c, hy);
-        store_images_inl(a.Hc[2], a.g, w.i, w.j, k, c, hz);
+        store_images_inl<exp_of_h<0>()>(a.Hc[0], a.g, w.i, w.j, k, c, hx);
+        store_images_inl<exp_of_h<1>()>(a.Hc[1], a.g, w.i, w.j, k, c, hy);
+        store_images_inl<exp_of_h<2>()>(a.Hc[2], a.g, w.i, w.j, k, c, hz);
       }
     }
   }
@@ -348,14 +376,14 @@ struct FaceOut {
 //   mn = M^n, mp = M^{r-1}, hn / he = H_EM^n / H_EM^{r-1} (own normal component + the two
 //   four-point averages), C = (curl E)_D, Msf / rMs = face Ms and its reciprocal (0 if Msf = 0),
 //   alf = face alpha, cf = mu0 |gamma_face| dt / 4, ch = dt / (2 mu) of a non-magnetic face.
-// The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces).
-// RECOMP (an iterate r = 2 only): M^1 is not read but recomputed from M^n and H_eff^n -- the very
-// expression the r = 1 sweep evaluated, so the value is the one it would have stored.
-template <int D, bool FIRST, bool ANISO, bool RECOMP = false>
+// The residual is max_c |M^r_c - M^{r-1}_c| / Ms_f (0 on non-magnetic faces); a non-finite M^r
+// (a step far above the Courant limit) gives an infinite residual, so the half-step is never
+// reported as converged.
+template <int D, bool FIRST, bool ANISO>
 __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn, const Vec3 &mp_in,
                                                 Vec3 hn, Vec3 he, double C, double Msf, double rMs,
                                                 double alf, double cf, double ch, bool wall) {
-  Vec3 mp = FIRST ? mn : mp_in;
+  const Vec3 mp = FIRST ? mn : mp_in;
   const double hn_own = comp<D>(hn), hp_own = comp<D>(he);
 
   // ---- magnetic face: eqs. 18-21
@@ -368,10 +396,6 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
     const double p = a.hk * (dot(mn, u) * rMs);
     hn.x += p * u.x; hn.y += p * u.y; hn.z += p * u.z;
   }
-  if (RECOMP) {
-    const Vec3 d1 = llg_increment<true>(mn, hn, hn, cf, alf * rMs, rMs);
-    mp = {mn.x + d1.x, mn.y + d1.y, mn.z + d1.z};
-  }
   // H_eff^{r-1}, lagged; at r = 1 it is H_eff^n
   if (FIRST) {
     he = hn;
@@ -383,7 +407,7 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
     }
   }
   Vec3 dM;
-  if (FIRST && !RECOMP && a.euler)
+  if (FIRST && a.euler)
     dM = llg_euler(mn, hn, 2.0 * cf / (1.0 + alf * alf), alf, rMs);
   else
     dM = llg_increment<FIRST>(mn, hn, he, cf, alf * rMs, rMs);
@@ -391,7 +415,8 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
   // eq. 21, normal component:  H^r = H^n + M^n - M^r - (dt / 2 mu0) curl E
   const double h_mag = hn_own - comp<D>(dM) - a.kh * C;
   // stopping test of PAPER.md:154, per face; reduced by the caller
-  const double e = fmax(fmax(fabs(mr.x - mp.x), fabs(mr.y - mp.y)), fabs(mr.z - mp.z));
+  const double e = fmax(fmax(fabs(mr.x - mp.x), fabs(mr.y - mp.y)), fabs(mr.z - mp.z)) * rMs;
+  const bool finite = fabs(mr.x) + fabs(mr.y) + fabs(mr.z) < INFINITY;   // false for NaN too
 
   // ---- non-magnetic face inside the sweep box: Maxwell update at r = 1, copy afterwards so that
   // both Jacobi buffers hold it.  PEC wall face: H = 0, M = 0 for ever (A13).
@@ -399,7 +424,7 @@ __device__ __forceinline__ FaceOut hm_face_core(const HMArgs &a, const Vec3 &mn,
   FaceOut o;
   o.m = {magnetic ? mr.x : 0.0, magnetic ? mr.y : 0.0, magnetic ? mr.z : 0.0};
   o.h = magnetic ? h_mag : h_non;
-  o.res = (magnetic && !(FIRST && a.euler)) ? e * rMs : 0.0;  // an explicit sweep has no stopping test
+  o.res = (magnetic && !(FIRST && a.euler)) ? (finite ? e : INFINITY) : 0.0;  // an explicit sweep has no stopping test
   return o;
 }
 
@@ -448,7 +473,7 @@ __device__ __forceinline__ void store_face(const HMArgs &a, int c, const FaceOut
 template <int D>
 __device__ __forceinline__ void store_face_images(const HMArgs &a, int i, int j, int k, int c,
                                                   const FaceOut &o) {
-  store_images_inl(a.Hc[D], a.g, i, j, k, c, o.h);
+  store_images_inl<exp_of_h<D>()>(a.Hc[D], a.g, i, j, k, c, o.h);
 }
 
 template <bool FIRST, bool MS_ARR, bool AG_ARR, bool MU_ARR, bool ANISO>
@@ -513,12 +538,14 @@ __global__ void k_set_cond(cudaGraphConditionalHandle h, const unsigned long lon
   cudaGraphSetConditional(h, res < tol ? 0u : 1u);
 }
 
-// 1 thread: close an (H,M) half-step
-__global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, int *r_hist, int max_iter,
-                           double tol, int any_magnetic, int last_of_step) {
+// 1 thread: close an (H,M) half-step of which the iterates 1..r_max were enqueued (fdtd_llg_step:
+// all max_iter of them, those after convergence exit on the flag; fdtd_llg_substep: the caller
+// stops when an iterate met the tolerance)
+__global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, int *r_hist, int r_max,
+                           int max_iter, double tol, int any_magnetic, int last_of_step) {
   if (any_magnetic) {
-    int R = max_iter;
-    for (int r = 1; r <= max_iter; ++r)
+    int R = r_max;
+    for (int r = 1; r <= r_max; ++r)
       if (__longlong_as_double((long long)resid[r]) < tol) { R = r; break; }
     const double res = __longlong_as_double((long long)resid[R]);
     if (!(res < tol)) st->nonconverged++;
@@ -559,7 +586,10 @@ __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ Cano
       for (int d = 0; d < 3; ++d) {
         const double v = __ldg(a.src[d] + c);
         a.dst[d][c] = v;
-        if (edge) store_images_inl(a.dst[d], a.g, w.i, w.j, k, c, v);
+        if (edge) {
+          if (d == 2) store_images_inl<EXP_LO>(a.dst[d], a.g, w.i, w.j, k, c, v);
+          else store_images_inl<EXP_HI>(a.dst[d], a.g, w.i, w.j, k, c, v);
+        }
       }
     }
   }
@@ -661,9 +691,9 @@ __global__ void __launch_bounds__(NTHREADS, 4) k_e_update(const __grid_constant_
       a.Eo[1][c] = ey;
       a.Eo[2][c] = ez;
       if (col.edge_ij || edge_k(a.g, k)) {
-        store_images_inl(a.Eo[0], a.g, w.i, w.j, k, c, ex);
-        store_images_inl(a.Eo[1], a.g, w.i, w.j, k, c, ey);
-        store_images_inl(a.Eo[2], a.g, w.i, w.j, k, c, ez);
+        store_images_inl<exp_of_e<0>()>(a.Eo[0], a.g, w.i, w.j, k, c, ex);
+        store_images_inl<exp_of_e<1>()>(a.Eo[1], a.g, w.i, w.j, k, c, ey);
+        store_images_inl<exp_of_e<2>()>(a.Eo[2], a.g, w.i, w.j, k, c, ez);
       }
     }
   }
@@ -703,16 +733,22 @@ __global__ void k_box_source(const __grid_constant__ BoxSrcArgs a) {
     bool wall = false;
     if (S.kind == 1) {  // E edge: tangential to the walls of the two other axes
       for (int d = 0; d < 3; ++d)
-        if (d != S.comp && !a.g.per[d] && idx[d] == 0) wall = true;
+        if (d != S.comp && a.g.wall[d] && idx[d] == 0) wall = true;
     } else {            // H face: the wall of its own axis
-      wall = !a.g.per[S.comp] && idx[S.comp] == 0;
+      wall = a.g.wall[S.comp] && idx[S.comp] == 0;
     }
     if (wall) continue;
     const double v = a.st->src_amp[a.idx] * (S.profile ? __ldg(S.profile + q) : 1.0);
     const int c = a.g.org + i + a.g.sy * j + a.g.sz * k;
     const double out = S.kind == 2 ? a.F[c] + a.g.dt * v : v;
     a.F[c] = out;
-    store_images_inl(a.F, a.g, i, j, k, c, out);
+    if (S.kind == 1) {  // what the neighbouring slabs read of E: E_x, E_y of the first plane
+      if (S.comp == 2) store_images_inl<EXP_NONE>(a.F, a.g, i, j, k, c, out);
+      else store_images_inl<EXP_LO>(a.F, a.g, i, j, k, c, out);
+    } else {            // of H: H_x, H_y of the last plane, H_z of the first
+      if (S.comp == 2) store_images_inl<EXP_LO>(a.F, a.g, i, j, k, c, out);
+      else store_images_inl<EXP_HI>(a.F, a.g, i, j, k, c, out);
+    }
   }
 }
 
@@ -818,9 +854,9 @@ __global__ void __launch_bounds__(NTHREADS) k_pml(const __grid_constant__ PmlArg
       a.Out[1][c] = v1;
       a.Out[2][c] = v2;
       if (col.edge_ij || edge_k(a.g, k)) {
-        store_images_inl(a.Out[0], a.g, w.i, w.j, k, c, v0);
-        store_images_inl(a.Out[1], a.g, w.i, w.j, k, c, v1);
-        store_images_inl(a.Out[2], a.g, w.i, w.j, k, c, v2);
+        store_images_inl<IS_E ? EXP_LO : EXP_HI>(a.Out[0], a.g, w.i, w.j, k, c, v0);
+        store_images_inl<IS_E ? EXP_LO : EXP_HI>(a.Out[1], a.g, w.i, w.j, k, c, v1);
+        store_images_inl<IS_E ? EXP_NONE : EXP_LO>(a.Out[2], a.g, w.i, w.j, k, c, v2);
       }
     }
   }
@@ -832,19 +868,19 @@ __device__ __forceinline__ Cell make_cell(const GridP &g, int i, int j, int k) {
   Cell q;
   q.i = i; q.j = j; q.k = k;
   q.c = g.org + i + g.sy * j + g.sz * k;
-  q.edge = false;
   return q;
 }
 template <int D> __device__ __forceinline__ bool wall_face(const GridP &g, const Cell &q) {
-  return !g.per[D] && (D == 0 ? q.i : (D == 1 ? q.j : q.k)) == 0;
+  return g.wall[D] && (D == 0 ? q.i : (D == 1 ? q.j : q.k)) == 0;
 }
 template <int D> __device__ __forceinline__ bool wall_edge(const GridP &g, const Cell &q) {
   constexpr int t1 = (D + 1) % 3, t2 = (D + 2) % 3;
   const int v1 = t1 == 0 ? q.i : (t1 == 1 ? q.j : q.k), v2 = t2 == 0 ? q.i : (t2 == 1 ? q.j : q.k);
-  return (!g.per[t1] && v1 == 0) || (!g.per[t2] && v2 == 0);
+  return (g.wall[t1] && v1 == 0) || (g.wall[t2] && v2 == 0);
 }
 
-// ghost layer of one array: periodic axes mirror the opposite interior plane, PEC ghosts are 0
+// ghost layer of one array: periodic axes mirror the opposite interior plane, PEC ghosts are 0;
+// the ghost plane of a slab interface keeps what the caller put there (the neighbour's plane)
 __global__ void k_fill_ghosts(double *__restrict__ a, const __grid_constant__ GridP g) {
   const long long px = g.n[0] + 2, py = g.n[1] + 2, pz = g.n[2] + 2;
   const long long total = px * py * pz;
@@ -857,6 +893,7 @@ __global__ void k_fill_ghosts(double *__restrict__ a, const __grid_constant__ Gr
     for (int d = 0; d < 3; ++d) {
       src[d] = idx[d];
       if (idx[d] < 0 || idx[d] >= g.n[d]) {
+        if (d == 2 && g.ext[idx[d] < 0 ? 0 : 1]) continue;
         ghost = true;
         if (g.per[d]) src[d] = idx[d] < 0 ? g.n[d] - 1 : 0; else zero = true;
       }
@@ -875,11 +912,12 @@ struct FieldsP {
 
 // zero tangential E and normal H on PEC walls
 __global__ void k_enforce_walls(const __grid_constant__ FieldsP a) {
-  const long long total = (long long)a.g.n[0] * a.g.n[1] * a.g.n[2];
+  // the ghost planes of slab interfaces hold the neighbours' values: the x / y walls cut them too
+  const long long total = (long long)a.g.n[0] * a.g.n[1] * (a.g.n[2] + a.g.ext[0] + a.g.ext[1]);
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
        t += (long long)gridDim.x * blockDim.x) {
     const Cell q = make_cell(a.g, (int)(t % a.g.n[0]), (int)((t / a.g.n[0]) % a.g.n[1]),
-                             (int)(t / ((long long)a.g.n[0] * a.g.n[1])));
+                             (int)(t / ((long long)a.g.n[0] * a.g.n[1])) - a.g.ext[0]);
     if (wall_edge<0>(a.g, q)) a.E[0][q.c] = 0.0;
     if (wall_edge<1>(a.g, q)) a.E[1][q.c] = 0.0;
     if (wall_edge<2>(a.g, q)) a.E[2][q.c] = 0.0;
@@ -967,20 +1005,24 @@ __global__ void k_minmax(const double *__restrict__ a, long long n, double *__re
 // box = {lo x,y,z, hi x,y,z (inclusive)}, count
 __global__ void k_mag_box(const double *__restrict__ Ms, const __grid_constant__ GridP g, int *box,
                           unsigned long long *count) {
-  const long long n = (long long)g.n[0] * g.n[1] * g.n[2];
-  int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {-1, -1, -1};
+  // the neighbours' adjacent planes (ghost planes of slab interfaces) count for the box: their
+  // magnetic cells make faces of this slab magnetic or read this slab's H (k = -1 and k = nz)
+  const long long n = (long long)g.n[0] * g.n[1] * (g.n[2] + g.ext[0] + g.ext[1]);
+  int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {INT_MIN, INT_MIN, INT_MIN};
   unsigned long long cnt = 0;
+  bool any = false;
   for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n;
        t += (long long)gridDim.x * blockDim.x) {
     const int i = (int)(t % g.n[0]), j = (int)((t / g.n[0]) % g.n[1]),
-              k = (int)(t / ((long long)g.n[0] * g.n[1]));
+              k = (int)(t / ((long long)g.n[0] * g.n[1])) - g.ext[0];
     if (Ms[g.org + i + g.sy * j + g.sz * k] > 0.0) {
       lo[0] = min(lo[0], i); lo[1] = min(lo[1], j); lo[2] = min(lo[2], k);
       hi[0] = max(hi[0], i); hi[1] = max(hi[1], j); hi[2] = max(hi[2], k);
-      ++cnt;
+      any = true;
+      if (k >= 0 && k < g.n[2]) ++cnt;   // the slab's own magnetic cells (statistics)
     }
   }
-  if (cnt) {
+  if (any) {
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       atomicMin(box + d, lo[d]);

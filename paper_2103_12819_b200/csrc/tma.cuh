@@ -1,5 +1,5 @@
-// tma.cuh -- sm_100a plumbing of the TMA-fed sweeps: mbarrier, cp.async.bulk.tensor (4-D tiles),
-// named barriers.  Inline PTX only; no arithmetic of the method lives here.
+// tma.cuh -- sm_100a plumbing of the TMA-fed sweeps: mbarrier, cp.async.bulk.tensor (4-D tiles).
+// Inline PTX only; no arithmetic of the method lives here.
 //
 // All field and material arrays of a handle are equally spaced in the caller's workspace
 // (kernels.cuh "DEVICE LAYOUT"), so ONE 4-D tensor (x = row pitch sy, y = ny+2, z = nz+2,
@@ -55,19 +55,21 @@ __device__ __forceinline__ bool mbar_try_wait_sleep(uint64_t *b, uint32_t parity
 }
 // Wait for the phase with the given parity.  The waiting warp sleeps in the barrier unit (a
 // polling loop of its own costs issue slots and power: it was 8 % of the sweep's instructions).
-// A pipeline bug must not hang the GPU: about once a millisecond the wait looks at the clock and
-// at *err; after ~1 s, or when another wait has given up, it records `tag` in *err (first writer
-// wins) and returns false; the caller then leaves its loop and the kernel ends (the host reports
-// the error, fdtd_llg_get_stats).
+// A pipeline bug must not hang the GPU: about once a millisecond the wait looks at the wall clock
+// (%globaltimer: independent of the SM clock, of time slicing and of profiler replays) and at
+// *err; after 4 s, or when another wait has given up, it records `tag` in *err (first writer
+// wins) and returns false; the caller then leaves its loop and the kernel ends.  The host reports
+// the error from every call that synchronises (fdtd_llg_read_fields, _get_stats, _step_timed).
 __device__ __forceinline__ bool mbar_wait(uint64_t *b, uint32_t parity, int *err, int tag) {
   if (mbar_try_wait(b, parity)) return true;
   long long t0 = 0;
   for (unsigned spins = 1;; ++spins) {
     if (mbar_try_wait_sleep(b, parity, 20000u)) return true;
     if ((spins & 63u) == 0) {
-      const long long now = clock64();
-      if (t0 == 0) t0 = now;
-      if (now - t0 > 2000000000LL || *(volatile int *)err != 0) {
+      unsigned long long now;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+      if (t0 == 0) t0 = (long long)now;
+      if ((long long)now - t0 > 4000000000LL || *(volatile int *)err != 0) {
         atomicCAS(err, 0, tag);
         return false;
       }
@@ -84,32 +86,8 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, u
       "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
       : "memory");
 }
-// same with an L2 cache-policy hint
-__device__ __forceinline__ void tma_load_4d_hint(void *dst, const CUtensorMap *map, uint64_t *bar,
-                                                 int c0, int c1, int c2, int c3, uint64_t policy) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
-      "[%0], [%1, {%2, %3, %4, %5}], [%6], %7;" ::"r"(smem_u32(dst)),
-      "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)), "l"(policy)
-      : "memory");
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap *map) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
-}
-
-// named barrier over `nthreads` threads of the block (id 1..15; 0 is __syncthreads)
-__device__ __forceinline__ void bar_sync(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 }  // namespace fl

@@ -124,6 +124,8 @@ class Workload:
     pml: Optional[tuple] = None     # (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi) cells of the open boundary layer
     pml_r0: Optional[float] = None
     pml_order: Optional[int] = None
+    slab_ext: tuple = (0, 0)        # this workload is one z-slab of a larger grid: its arrays carry the
+                                    # neighbours' adjacent plane on the flagged sides (slabs.cut_workload)
     seed: int = BASE_SEED
     notes: str = ""
 
@@ -139,7 +141,7 @@ class Workload:
             if t is None:
                 return None
             if isinstance(t, (int, float)):   # uniform material given as a scalar
-                return np.full((self.nz, self.ny, self.nx), float(t))
+                return np.full((self.nz + sum(self.slab_ext), self.ny, self.nx), float(t))
             return t.detach().cpu().numpy()
         return {
             "materials": {k: cv(v) for k, v in self.materials.items()},

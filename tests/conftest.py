@@ -9,7 +9,7 @@ if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
 # keep the CPU suite quick and deterministic on small boxes
-os.environ.setdefault("OMP_NUM_THREADS", str(min(8, os.cpu_count() or 1)))
+os.environ.setdefault("OMP_NUM_THREADS", str(min(16, os.cpu_count() or 1)))
 
 
 def pytest_configure(config):

@@ -37,10 +37,36 @@ def test_header_structs_match_binding(B):
     """Field names of the ctypes mirrors follow the header, in order."""
     txt = (ROOT / "include" / "fdtd_llg.h").read_text()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    for cname, mirror in (("fdtd_llg_options", B.Options), ("fdtd_llg_stats", B.Stats)):
+    for cname, mirror in (("fdtd_llg_options", B.Options), ("fdtd_llg_stats", B.Stats),
+                          ("fdtd_llg_slab_info", B.SlabInfo)):
         body = re.search(r"typedef struct \{([^{}]*)\} %s;" % cname, txt).group(1)
         fields = re.findall(r"\b([a-z_][a-z_0-9]*)(?:\[\d\])?\s*;", body)
         assert fields == [f for f, _ in mirror._fields_], cname
+
+
+def test_struct_layout_as_the_c_compiler_sees_it(B, tmp_path):
+    """A C translation unit includes the header and prints sizeof / offsetof; the ctypes mirrors
+    must agree byte for byte (a mismatch would otherwise only show as wrong numbers on the GPU)."""
+    import subprocess
+    exe = tmp_path / "abi_layout"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", str(ROOT / "include"),
+                    str(ROOT / "tests" / "abi_layout.c"), "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    mirrors = {"fdtd_llg_options": B.Options, "fdtd_llg_stats": B.Stats, "fdtd_llg_slab_info": B.SlabInfo}
+    seen = {k: set() for k in mirrors}
+    for line in out.splitlines():
+        t = line.split()
+        if t[0] == "sizeof":
+            assert C.sizeof(mirrors[t[1]]) == int(t[2]), line
+        elif t[0] == "offsetof":
+            assert getattr(mirrors[t[1]], t[2]).offset == int(t[3]), line
+            seen[t[1]].add(t[2])
+        elif t[:2] == ["enum", "SUB"]:
+            assert [int(v) for v in t[2:]] == [B.SUB_BEGIN, B.SUB_HM1, B.SUB_HM1_END, B.SUB_E, B.SUB_HM2, B.SUB_HM2_END]
+        elif t[:2] == ["enum", "K_NCLASS"]:
+            assert int(t[2]) == len(B.KERNEL_CLASSES)
+    for name, m in mirrors.items():
+        assert seen[name] == {f for f, _ in m._fields_}, name      # every field was checked
 
 
 def test_defaults_and_workspace_budget(B):

@@ -1,8 +1,8 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (default
 kernel path, CUDA-graph replay).
 
-* configs 2 and 3 (256^3, 512x128x128): the oracle runs the whole grid for a few steps; every
-  element is compared.
+* configs 2 and 3 (256^3, 512x128x128): the oracle runs the whole grid, every element is compared
+  after 100 steps: tests/test_parity_at_size_gpu.py (with configs 4, 5 on >= 128^3 grids).
 * configs 4 and 5 (384^3, 768^3): the oracle cannot hold the grid (or would take minutes), so it
   computes SAMPLED outputs instead: a sub-box of the same seeded inputs is cut out and advanced by
   the oracle; the scheme has a finite domain of dependence (per step: R + 1 cells per (H,M)
@@ -84,23 +84,6 @@ def _gpu_window(sim, names, lo, n):
 
 def _scales(ref, groups):
     return {g: max(float(np.max(np.abs(ref[nm]))) for nm in FIELD_GROUPS[g]) or 1.0 for g in groups}
-
-
-@pytest.mark.parametrize("cfg,steps", [(2, 10), (3, 10)])
-def test_full_size_every_element(cfg, steps):
-    """configs 2, 3 at full size: the oracle runs the whole grid."""
-    from paper_2103_12819_b200.binding import from_workload
-    from tests._util import oracle_from_workload, rel_linf
-    w = wl.make_config(cfg)
-    o = oracle_from_workload(w)
-    o.step(steps)
-    ref = o.read_fields()
-    sim = from_workload(w)
-    sim.step(steps)
-    got = {k: v.numpy() for k, v in sim.read_fields(names=FIELD_GROUPS["E"] + FIELD_GROUPS["H"]).items()}
-    for g in ("E", "H"):
-        assert rel_linf(got, ref, g) <= TOL, (g, rel_linf(got, ref, g))
-    assert sim.stats()["steps"] == steps
 
 
 def test_config4_full_size_windows():

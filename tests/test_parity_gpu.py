@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from tests._util import FIELD_GROUPS, oracle_from_workload, rel_linf
+from tests._util import FIELD_GROUPS, oracle_from_workload, record_parity, rel_linf
 from paper_2103_12819_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -35,16 +35,10 @@ def _run_both(w, steps, use_graph=True, chunks=(None,)):
     return got, ref, sim.stats(), o.stats()
 
 
-def _assert_close_to_rounding(got, ref):
-    """kernel_path 4 evaluates the LLG increment twice in one function (M^1 recomputed); the
-    compiler contracts the shared subexpressions differently there, so its increments differ from
-    the other paths' in the last bit: equal to rounding, not bit for bit."""
-    for g in ("E", "H", "M"):
-        assert rel_linf(got, ref, g) < 1e-12, g
-
-
-def _assert_parity(got, ref, llg, tol=TOL):
+def _assert_parity(got, ref, llg, tol=TOL, record=None):
     errs = {g: rel_linf(got, ref, g) for g in ("E", "H") + (("M",) if llg else ())}
+    if record is not None:
+        record_parity(dict(record, **{"err_" + g: e for g, e in errs.items()}))
     for g, e in errs.items():
         assert e <= tol, (g, errs)
     return errs
@@ -62,8 +56,12 @@ def test_parity_100_steps_all_configs(cfg):
         sim = from_workload(w, kernel_path=5)
         assert sim.stats()["staged_sweeps"] == 1 and gs["staged_sweeps"] == 0
         sim.step(100)
-        _assert_parity(_gpu_fields(sim), ref, True)
-    _assert_parity(got, ref, w.enable_llg)
+        _assert_parity(_gpu_fields(sim), ref, True,
+                       record={"test": "parity_100_steps_small", "config": cfg, "shape": list(wl.SMALL_SHAPES[cfg]),
+                               "steps": 100, "path": "staged (kernel_path 5)"})
+    _assert_parity(got, ref, w.enable_llg,
+                   record={"test": "parity_100_steps_small", "config": cfg, "shape": list(wl.SMALL_SHAPES[cfg]),
+                           "steps": 100, "path": "default", "iters": gs["iters_total"]})
     assert gs["steps"] == 100
     if w.enable_llg:
         # same number of LLG iterations, all converged
@@ -121,7 +119,9 @@ def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
             sim.step(c)
         outs.append(_gpu_fields(sim))
         assert sim.stats()["steps"] == 100
-        assert sim.stats()["kernel_launches"] == 100 * sim.stats()["launches_per_step"]
+        st = sim.stats()
+        # + the launches that take the merged faces to t = dt/2 before the first step (<= 6 slabs)
+        assert 0 <= st["kernel_launches"] - 100 * st["launches_per_step"] <= 6
     for other in outs[1:]:
         for n in outs[0]:
             assert np.array_equal(outs[0][n], other[n]), n
@@ -130,27 +130,21 @@ def test_graph_and_plain_launches_agree_bitwise_and_step_chunks():
 @pytest.mark.parametrize("cfg,shape", [(1, (32, 32, 32)), (4, (44, 36, 40)), (5, (40, 44, 36)),
                                        (5, (70, 19, 23)), (4, (33, 8, 50))])
 def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
-    """kernel_path 5 / 3 (staged sweeps: TMA-fed shared-memory ring, thread = cell) and 1 (direct
-    global loads) share the arithmetic (hm_face_core); 4 (staged, M^1 recomputed at r = 2 instead
-    of stored) agrees to rounding:
-    every field and the iteration counts agree bit for bit, on shapes with ragged tiles in x and
-    y and several z chunks."""
+    """kernel_path 5 (staged sweeps: TMA-fed shared-memory ring, thread = cell) and 1 (direct
+    global loads) share the arithmetic (hm_face_core): every field and the iteration counts agree
+    bit for bit, on shapes with ragged tiles in x and y and several z chunks."""
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(cfg, shape=shape)
     outs, stats = [], []
-    for path in (1, 5, 3, 4):
+    for path in (1, 5):
         sim = from_workload(w, kernel_path=path)
         assert sim.stats()["staged_sweeps"] == (path != 1)
         sim.step(25)
         outs.append(_gpu_fields(sim))
         stats.append(sim.stats())
-    for path, other, st in zip((5, 3, 4), outs[1:], stats[1:]):
-        if path == 4:
-            _assert_close_to_rounding(other, outs[0])
-        else:
-            for n in outs[0]:
-                assert np.array_equal(outs[0][n], other[n]), n
-        assert stats[0]["iters_total"] == st["iters_total"] > 0
+    for n in outs[0]:
+        assert np.array_equal(outs[0][n], outs[1][n]), n
+    assert stats[0]["iters_total"] == stats[1]["iters_total"] > 0
 
 
 @pytest.mark.parametrize("cfg,shape", [(5, (200, 176, 300)), (4, (230, 150, 200))])
@@ -162,7 +156,7 @@ def test_kernel_paths_agree_bitwise_with_every_sm_busy(cfg, shape):
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(cfg, shape=shape, device="cuda:0")
     ref = None
-    for path in (1, 0, 0, 3):
+    for path in (1, 0, 0, 5):
         sim = from_workload(w, kernel_path=path)
         sim.step(4)
         got = {k: v for k, v in sim.read_fields(device="cuda:0").items()}
@@ -177,9 +171,8 @@ def test_kernel_paths_agree_bitwise_with_every_sm_busy(cfg, shape):
 
 @pytest.mark.parametrize("tol,iters", [(1e-2, 1), (1e-7, 2)])
 def test_early_stop_after_one_or_two_iterates_on_every_kernel_path(tol, iters):
-    """A loose tolerance stops the iteration at R = 1 (M^1 is the result: kernel_path 4 must then
-    run its full r = 1 sweep after all, because it did not store M^1) or at R = 2 (even R: the
-    result sits in the pong H set and is copied to the canonical one)."""
+    """A loose tolerance stops the iteration at R = 1 or at R = 2 (even R: the result sits in the
+    pong H set and is copied to the canonical one)."""
     from paper_2103_12819_b200.binding import from_workload
     w = wl.make_config(5, shape=(40, 44, 36))
     w.llg_tol = tol
@@ -188,17 +181,15 @@ def test_early_stop_after_one_or_two_iterates_on_every_kernel_path(tol, iters):
     ref = o.read_fields()
     assert int(o.stats()["iters_total"]) == 40 * iters
     outs = []
-    for path in (1, 5, 3, 4):
+    for path in (1, 5):
         sim = from_workload(w, kernel_path=path)
         sim.step(20)
         outs.append(_gpu_fields(sim))
         assert sim.stats()["iters_total"] == 40 * iters and sim.stats()["iters_max"] == iters
     for got in outs:
         _assert_parity(got, ref, True)
-    for other in outs[1:3]:         # paths 0, 3: the same instantiation of the arithmetic
-        for n in outs[0]:
-            assert np.array_equal(outs[0][n], other[n]), n
-    _assert_close_to_rounding(outs[3], outs[0])
+    for n in outs[0]:
+        assert np.array_equal(outs[0][n], outs[1][n]), n
 
 
 @pytest.mark.parametrize("cfg", [1, 4, 5])
@@ -211,7 +202,7 @@ def test_first_order_scheme_parity_100_steps(cfg):
     o.step(100)
     ref = o.read_fields()
     outs = []
-    for path in (5, 1, 3):
+    for path in (5, 1):
         sim = from_workload(w, kernel_path=path, time_scheme=1)
         sim.step(100)
         outs.append(_gpu_fields(sim))
