@@ -12,11 +12,18 @@ Prints ONE JSON line: metric/value (Gcell-updates/s, inputs resident in HBM, CUD
 e2e (same metric through the public API with HOST buffers: H2D of the initial fields, K steps,
 D2H of all 15 result arrays inside the timed region), roofline (dominant kernel, algorithmic
 bytes / CUDA-event duration against the measured HBM peak), cpu_baseline (the oracle as it
-stands, timed on this box's host cores on a bounded sample), clocks, gpu_launches.
+stands, timed on this box's host cores on a bounded sample, all cores and one thread), clocks,
+gpu_launches, and other_configs: the same measurement on the grids shaped like the paper's
+waveguide and tunable-filter runs (BASELINE.json configs 2, 3, 4 at full size and the paper's own
+1024 x 4 x 512 base case).
 
-N > 1 (torchrun): the path is single-GPU by scope (replicas only); each
-rank advances its own replica of the grid, no data-path collective; value = all ranks' cell
-updates / max-over-ranks device time; "scaling": "weak".
+N > 1 (torchrun, one process per GPU): the grid is cut into z-slabs (domain
+decomposition is the paper's parallelism), the halo exchange is done by peer stores inside the
+update kernels over NVLink, one 8-byte NCCL max-allreduce per sub-step merges the LLG stopping
+test and orders the slabs (paper_2103_12819_b200/slabs.py).  --scaling weak (default): every rank
+holds one copy of the config, the copies stacked along z (the paper grows its base case in z the
+same way); --scaling strong: the config's own grid cut into N slabs.  value = all
+ranks' cell updates / max-over-ranks device time.
 
 --impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
@@ -45,9 +52,7 @@ WORDS = {"h_update": 9,      # E 3 + H 3 read, H 3 written
          "hm_second": 39,    # + H^1 3 + M^1 9 read, M^2 9 + H^2 3 written
          "hm_iter": 39,      # r >= 3: as r = 2
          "e_update": 9}      # E 3 + H 3 read, E 3 written
-# kernel_path 4: M^1 never goes to memory -- r = 1 writes H^1 only and r = 2 recomputes M^1 from
-# M^n, H^n (hm_stage.cuh)
-WORDS_LEAN = dict(WORDS, hm_first=18, hm_second=30)
+OTHER_CONFIGS = (2, 3, 4, 6)
 
 
 def _parse():
@@ -63,9 +68,17 @@ def _parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-shape", default="128,128,128")
     ap.add_argument("--cpu-sample-steps", type=int, default=30)
+    ap.add_argument("--cpu-single-shape", default="64,64,64")
+    ap.add_argument("--cpu-single-steps", type=int, default=4)
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the extra measurements on configs 2, 3, 4, 6 (they run with the default config at N = 1)")
+    ap.add_argument("--other-steps", type=int, default=50)
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one copy of the config per rank, stacked in z; strong = the config's grid cut into N slabs")
+    ap.add_argument("--no-merge-h", action="store_true", help="fdtd_llg_options.merge_h = 0 (two H half-steps everywhere)")
     ap.add_argument("--kernel-path", type=int, default=0,
-                    help="fdtd_llg_options.kernel_path: 0 = staged sweeps (default), 1 = direct-load kernels, "
-                         "3 = staged 32x7 tiles, 4 = staged + M^1 recomputed (fewer bytes, more flops)")
+                    help="fdtd_llg_options.kernel_path: 0 = staged sweeps where they apply (default), "
+                         "1 = direct-load kernels, 5 = staged sweeps whatever the box size")
     ap.add_argument("--plain-graph", action="store_true",
                     help="capture the step without the conditional node (use_graph = 2), so that ncu lists "
                          "the kernels of the replayed steps too")
@@ -157,7 +170,7 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": f"{w.name} {full[0]}x{full[1]}x{full[2]}", "sample": sample,
+            "config": {"workload": f"{w.name} {w.nx}x{w.ny}x{w.nz} (bounded sample of {full[0]}x{full[1]}x{full[2]})", "sample": sample,
                        "time_scheme": "first-order" if args.time_scheme else "second-order"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": sample},
@@ -194,11 +207,132 @@ def _ncu_traffic(kernel, workload):
     return None
 
 
+def _oracle_single_thread(cfg, shape, steps, time_scheme):
+    """The oracle on ONE thread (libgomp is told so; restored afterwards)."""
+    import ctypes
+    from oracle.cpu_oracle import omp_threads
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(1)
+    except OSError:
+        return None
+    try:
+        _, rate, dt, _ = _oracle_rate(cfg, shape, steps, time_scheme=time_scheme)
+    finally:
+        gomp.omp_set_num_threads(omp_threads())
+    return {"value": rate * 1e-9, "unit": UNIT, "cores": 1,
+            "sample": f"config {cfg} structure at {shape[0]}x{shape[1]}x{shape[2]}, {steps} steps, {dt:.1f} s"}
+
+
+def _timed_steps(sim, K, W, barrier):
+    """K steps of CUDA-graph replay after W warm-up steps, timed with CUDA events on the library's stream."""
+    import torch
+    stream = sim.stream
+    sim.step(max(W, 1))
+    stream.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.step(K)
+    e1.record(stream)
+    stream.synchronize()
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
+    """roofline block: an event pair around every launch of K more steps (fdtd_llg_step_timed)."""
+    from paper_2103_12819_b200.binding import MAT_BITS
+    st = sim.stats()
+    prof = sim.step_timed(K)
+    box = st["sweep_cells"]
+    mask = st["material_array_mask"]
+    extra = {"h_update": bool(mask & MAT_BITS["mu_r"]),
+             "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
+             "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
+    extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
+    prof = dict(prof)                       # r = 2 and r >= 3 are the same kernel: one class
+    a2, b2 = prof.pop("hm_second"), prof["hm_iter"]
+    prof["hm_iter"] = (a2[0] + b2[0], a2[1] + b2[1])
+    per_class = {}
+    for cls, (cms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        ent = {"launches": cnt, "ms_total": cms, "us_per_launch": 1e3 * cms / cnt}
+        if cls in WORDS:
+            # cells one launch covers: the sweep box (LLG sweeps), the whole grid (E update), the
+            # complement of the box split over its slabs (H update: two half-steps per step, or
+            # one merged update per step)
+            if cls.startswith("hm_"):
+                ncell = box
+            elif cls == "e_update":
+                ncell = cells
+            else:
+                ncell = (cells - box) * (1 if st["merged_h"] else 2) * K / cnt
+            ent["alg_bytes_per_launch"] = 8.0 * (WORDS[cls] + extra[cls]) * ncell
+            ent["alg_GBps"] = ent["alg_bytes_per_launch"] / (cms / cnt * 1e-3) * 1e-9
+        per_class[cls] = ent
+    timed = [c for c in per_class if "alg_GBps" in per_class[c]]
+    dom = max(timed, key=lambda c: per_class[c]["ms_total"])
+    staged = bool(st["staged_sweeps"])
+    dom_kernel = {"h_update": "k_h_update",
+                  "hm_first": "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
+                  "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
+                  "e_update": "k_e_update"}[dom]
+    achieved = per_class[dom]["alg_GBps"]
+    step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
+    traffic = _ncu_traffic(dom_kernel, name)
+    return {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak,
+            "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+            "traffic": traffic,
+            "traffic_source": ("profiles/traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum per launch from the "
+                               "committed ncu --set full capture of this kernel on this workload (not measured in this run)"
+                               if traffic is not None else None),
+            "alg_bytes_per_launch": per_class[dom]["alg_bytes_per_launch"],
+            "us_per_launch": per_class[dom]["us_per_launch"],
+            "share_of_step": per_class[dom]["ms_total"] / sum(v["ms_total"] for v in per_class.values()),
+            "how": f"CUDA events around every launch over {K} steps (fdtd_llg_step_timed, plain launches)",
+            "whole_step": {"alg_bytes_per_step": step_bytes,
+                           "achieved": step_bytes / (ms_step * 1e-3) * 1e-9,
+                           "frac": step_bytes / (ms_step * 1e-3) * 1e-9 / peak},
+            "kernels": per_class}
+
+
+def _measure_other(cfg, K, W, dev, args, peak, peak_src):
+    """One of the other configs at full size: graph replay + the class breakdown, no e2e leg."""
+    import torch
+    from paper_2103_12819_b200 import workloads as wl
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(cfg, device=dev)
+    name, cells = _workload_name(w), w.cells
+    sim = from_workload(w, device=dev, kernel_path=args.kernel_path, merge_h=not args.no_merge_h)
+    del w
+    ms = _timed_steps(sim, K, W, lambda: None)
+    st = sim.stats()
+    roof = _kernel_breakdown(sim, K, cells, ms / K, peak, peak_src, name)
+    out = {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"], "steps": K,
+           "gcell_s": cells * K / (ms * 1e-3) * 1e-9, "ms_per_step": ms / K,
+           "launches_per_step": st["launches_per_step"], "staged_sweeps": st["staged_sweeps"],
+           "merged_h": st["merged_h"],
+           "llg_iterations_per_halfstep": st["iters_total"] / max(1, st["halfsteps"]),
+           "alg_bytes_per_cell_step": roof["whole_step"]["alg_bytes_per_step"] / cells,
+           "whole_step_frac": roof["whole_step"]["frac"], "whole_step_GBps": roof["whole_step"]["achieved"],
+           "dominant_kernel": roof["kernel"], "dominant_frac": roof["frac"],
+           "kernels": {k: {"us_per_launch": v["us_per_launch"], "launches": v["launches"],
+                           "alg_GBps": v.get("alg_GBps")} for k, v in roof["kernels"].items()}}
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2103_12819_b200 import workloads as wl
-    from paper_2103_12819_b200.binding import from_workload
+    from paper_2103_12819_b200.binding import FIELD_NAMES, from_workload
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
@@ -213,11 +347,28 @@ def run_ours(args):
     from paper_2103_12819_b200.replicas import barrier, max_over_ranks, whole_job_rate
 
     K, W = args.steps, max(args.warmup, 0)
+    peak, peak_src = _peak()
     w = wl.make_config(args.config, shape=_shape(args), device=dev)
-    cells = w.cells
     name = _workload_name(w)
-    sim = from_workload(w, device=dev, kernel_path=args.kernel_path, time_scheme=args.time_scheme,
-                        use_graph=2 if args.plain_graph else True)
+    slab = None
+    if world > 1:
+        # z-slabs: weak = one copy of the grid per rank stacked in z, strong = the grid cut in N
+        from paper_2103_12819_b200.slabs import PERIODIC, DistSlab, cut_workload, plan_slabs, stack_copies
+        if args.scaling == "weak":
+            plan = plan_slabs(w.nz * world, world, False)[rank]
+            w = stack_copies(w, plan)
+            name += f" x {world} copies stacked in z"
+        else:
+            plan = plan_slabs(w.nz, world, w.bc[2] == PERIODIC)[rank]
+            w = cut_workload(w, plan)
+            name += f" cut into {world} z-slabs"
+        slab = DistSlab(w, plan, dev, kernel_path=args.kernel_path, merge_h=not args.no_merge_h,
+                        time_scheme=args.time_scheme)
+        sim = slab.sim
+    else:
+        sim = from_workload(w, device=dev, kernel_path=args.kernel_path, time_scheme=args.time_scheme,
+                            use_graph=2 if args.plain_graph else True, merge_h=not args.no_merge_h)
+    cells = w.nx * w.ny * w.nz          # this rank's cells
     stream = sim.stream
 
     # host copies of the initial state for the end-to-end leg (pinned), before the device inputs go
@@ -234,99 +385,77 @@ def run_ours(args):
     sampler = ClockSampler(vis[local] if local < len(vis) else local)
     sampler.start()
 
-    # ---- device-resident throughput: CUDA-graph replay of K steps
-    sim.step(max(W, 1))
-    stream.synchronize()
-    barrier()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # ---- device-resident throughput
     t_a = time.perf_counter()
-    e0.record(stream)
-    sim.step(K)
-    e1.record(stream)
-    stream.synchronize()
-    torch.cuda.synchronize()
-    t_b = time.perf_counter()
-    barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1), dev)
-    st = sim.stats()
+    if slab is None:
+        ms = max_over_ranks(_timed_steps(sim, K, W, barrier), dev)      # CUDA-graph replay of K steps
+        st = sim.stats()
+        launches = K * st["launches_per_step"]
+    else:
+        slab.step(max(W, 1))
+        stream.synchronize()
+        barrier()
+        torch.cuda.synchronize()
+        l0 = sim.stats()["kernel_launches"]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        slab.step(K)
+        e1.record(stream)
+        stream.synchronize()
+        torch.cuda.synchronize()
+        barrier()
+        ms = max_over_ranks(e0.elapsed_time(e1), dev)
+        st = sim.stats()
+        launches = st["kernel_launches"] - l0
     value = whole_job_rate(cells, K, ms * 1e-3, world) * 1e-9
-    launches = K * st["launches_per_step"]
 
-    # ---- roofline of the dominant kernel: an event pair around every launch, K more steps
-    prof = sim.step_timed(K)
+    # ---- roofline
+    if slab is None:
+        roofline = _kernel_breakdown(sim, K, cells, ms / K, peak, peak_src, name)
+    else:
+        # a connected slab has no per-launch timing hook: the whole step against the peak, with the
+        # single-GPU byte model (27 + 39 (R - 1) words per half-step on the sweep box, 9 per
+        # outside update, 9 for the E update; + 1 per material array a kernel reads)
+        from paper_2103_12819_b200.binding import MAT_BITS
+        mask, box = st["material_array_mask"], st["sweep_cells"]
+        R = st["iters_total"] / max(1, st["halfsteps"])
+        xm = sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r"))
+        xe = sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))
+        words = 2 * box * ((27 + xm) + (39 + xm) * max(0.0, R - 1)) \
+            + (cells - box) * (1 if st["merged_h"] else 2) * (9 + bool(mask & MAT_BITS["mu_r"])) \
+            + cells * (9 + xe)
+        ach = 8.0 * words / (ms / K * 1e-3) * 1e-9
+        roofline = {"bound": "hbm", "kernel": "whole step of one rank (z-slab run: no per-launch timing hook)",
+                    "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
+                    "traffic": None, "alg_bytes_per_launch": 8.0 * words,
+                    "how": "algorithmic bytes of one rank's step / max-over-ranks step time (CUDA events)",
+                    "halo": {"bytes_per_plane": 8 * sim.shape[1] * sim.shape[2],
+                             "planes_per_substep": "H_x, H_y up + H_z down per (H,M) sweep; E_x, E_y down per E update",
+                             "allreduces_per_step": slab.merges / max(1, K + max(W, 1)),
+                             "host_checks_per_step": slab.host_checks / max(1, K + max(W, 1))}}
     t_c = time.perf_counter()
-    peak, peak_src = _peak()
-    box = st["sweep_cells"]
-    from paper_2103_12819_b200.binding import MAT_BITS
-    mask = st["material_array_mask"]
-    extra = {"h_update": bool(mask & MAT_BITS["mu_r"]),
-             "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
-             "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
-    extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
-    words = WORDS_LEAN if (args.kernel_path == 4 and st["staged_sweeps"]) else WORDS
-    if words is WORDS and "hm_second" in prof:   # r = 2 and r >= 3 are the same kernel: one class
-        prof = dict(prof)
-        a2, b2 = prof.pop("hm_second"), prof["hm_iter"]
-        prof["hm_iter"] = (a2[0] + b2[0], a2[1] + b2[1])
-    per_class = {}
-    for cls, (cms, cnt) in prof.items():
-        if cnt == 0:
-            continue
-        ent = {"launches": cnt, "ms_total": cms, "us_per_launch": 1e3 * cms / cnt}
-        if cls in words:
-            # cells one launch covers: the sweep box (LLG sweeps), the whole grid (E update), the
-            # complement of the box split over its slabs (H update, 2 half-steps per step)
-            if cls.startswith("hm_"):
-                ncell = box
-            elif cls == "e_update":
-                ncell = cells
-            else:
-                ncell = (cells - box) * 2 * K / cnt
-            ent["alg_bytes_per_launch"] = 8.0 * (words[cls] + extra[cls]) * ncell
-            ent["alg_GBps"] = ent["alg_bytes_per_launch"] / (cms / cnt * 1e-3) * 1e-9
-        per_class[cls] = ent
-    timed = [c for c in per_class if "alg_GBps" in per_class[c]]
-    dom = max(timed, key=lambda c: per_class[c]["ms_total"])
-    lean = words is WORDS_LEAN
-    staged = bool(st["staged_sweeps"])
-    dom_kernel = {"h_update": "k_h_update",
-                  "hm_first": "k_hm_stage<FIRST_H>" if lean else "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
-                  "hm_second": "k_hm_stage<ITER_RE>" if lean else "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
-                  "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
-                  "e_update": "k_e_update"}[dom]
-    achieved = per_class[dom]["alg_GBps"]
-    step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
-    roofline = {"bound": "hbm", "kernel": dom_kernel, "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": _ncu_traffic(dom_kernel, name),
-                "alg_bytes_per_launch": per_class[dom]["alg_bytes_per_launch"],
-                "us_per_launch": per_class[dom]["us_per_launch"],
-                "share_of_step": per_class[dom]["ms_total"] / sum(v["ms_total"] for v in per_class.values()),
-                "how": f"CUDA events around every launch over {K} steps (fdtd_llg_step_timed, plain launches)",
-                "whole_step": {"alg_bytes_per_step": step_bytes,
-                               "achieved": step_bytes / (ms / K * 1e-3) * 1e-9,
-                               "frac": step_bytes / (ms / K * 1e-3) * 1e-9 / peak},
-                "kernels": per_class}
     clocks = sampler.summary(t_a, t_c)
 
     # ---- end to end through the public API with HOST buffers
     e2e = None
     if host_in is not None:
-        from paper_2103_12819_b200.binding import FIELD_NAMES
         out = {nm: torch.empty(sim.shape, dtype=torch.float64).pin_memory() for nm in FIELD_NAMES}
         if not st["magnetic_cells"]:
             out = {k: v for k, v in out.items() if not k.startswith("M")}
         h2d = sum(t.numel() * 8 for g in host_in.values() for t in g if t is not None)
         d2h = sum(t.numel() * 8 for t in out.values())
+        step = (lambda n: sim.step(n)) if slab is None else (lambda n: slab.step(n))
         sim.set_fields(host_in["E"], host_in["H"], host_in["M_cell"])   # warm the path once
-        sim.step(1)
+        barrier()
+        step(1)
         stream.synchronize()
         barrier()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         sim.set_fields(host_in["E"], host_in["H"], host_in["M_cell"])   # H2D from pinned memory
-        sim.step(K)
+        if slab is not None:
+            barrier()            # every slab's ghost planes are in place before a neighbour stores into them
+        step(K)
         sim.read_fields(out=out)                                         # D2H, synchronises
         torch.cuda.synchronize()
         dt = max_over_ranks(time.perf_counter() - t0, dev)
@@ -336,29 +465,55 @@ def run_ours(args):
                "seconds": dt, "what": f"set_fields(host) + step({K}) + read_fields(host), wall clock"}
         del out, host_in
     sampler.stop()
+    iters_per_half = st["iters_total"] / max(1, st["halfsteps"])
+    mag = st["magnetic_cells"]
+    if slab is not None:
+        slab.close()
+    else:
+        sim.close()
+    del sim
+    torch.cuda.empty_cache()
 
-    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1)
+    # ---- the grids shaped like the paper's waveguide / tunable-filter runs (north_star)
+    other = None
+    if rank == 0 and world == 1 and args.config == 5 and args.shape is None and not args.no_other_configs \
+            and not args.time_scheme:
+        other = {}
+        for cfg in OTHER_CONFIGS:
+            try:
+                other[f"config{cfg}"] = _measure_other(cfg, args.other_steps, max(W, 3), dev, args, peak, peak_src)
+            except Exception as e:  # a failure here must not lose the headline line
+                other[f"config{cfg}"] = {"error": repr(e)}
+
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1), all cores and one thread
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         shp = tuple(int(v) for v in args.cpu_sample_shape.split(","))
         _, rate, dt, cores = _oracle_rate(args.config, shp, args.cpu_sample_steps, time_scheme=args.time_scheme)
         cpu = {"value": rate * 1e-9, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"config {args.config} structure at {shp[0]}x{shp[1]}x{shp[2]}, "
-                         f"{args.cpu_sample_steps} steps, {dt:.1f} s"}
+                         f"{args.cpu_sample_steps} steps, {dt:.1f} s",
+               "host_cpus": os.cpu_count(),
+               "single_thread": _oracle_single_thread(args.config, tuple(int(v) for v in args.cpu_single_shape.split(",")),
+                                                      args.cpu_single_steps, args.time_scheme)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
-                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+                "scaling": args.scaling if world > 1 else "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"],
-                           "llg_iterations_per_halfstep": st["iters_total"] / max(1, st["halfsteps"]),
-                           "parallelism": "replicas" if world > 1 else "single-gpu",
+                "config": {"workload": name, "cells": cells * world,
+                           "cells_per_gpu": cells, "magnetic_cells_rank0": mag,
+                           "llg_iterations_per_halfstep": iters_per_half,
+                           "parallelism": f"z-slabs x{world}: peer stores in the update kernels + 8-byte max-allreduce per sub-step"
+                                          if world > 1 else "single-gpu",
                            "l2": "state far larger than L2 (no flush needed)" if cells * 48 > 4e8
                                  else "state fits L2: latency-bound case, no roofline claim",
-                           "time_loop": "CUDA graph replay", "kernel_path": args.kernel_path,
+                           "time_loop": "CUDA graph replay" if world == 1 else "plain launches (sub-steps)",
+                           "kernel_path": args.kernel_path, "merge_h": st["merged_h"],
                            "time_scheme": "first-order" if args.time_scheme else "second-order"},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-                "gpu_launches": launches,
+                "gpu_launches": launches, "other_configs": other,
                 "context": "paper: 59x node-by-node GPU speedup (8x V100 vs 32-core Haswell, "
                            "PAPER.md:229, 277) -- another machine, context only"}
         print(json.dumps(line), flush=True)
