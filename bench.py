@@ -51,7 +51,8 @@ WORDS = {"h_update": 9,      # E 3 + H 3 read, H 3 written
          "hm_first": 27,     # E 3 + H^n 3 + M^n 9 read, M^1 9 + H^1 3 written
          "hm_second": 39,    # + H^1 3 + M^1 9 read, M^2 9 + H^2 3 written
          "hm_iter": 39,      # r >= 3: as r = 2
-         "e_update": 9}      # E 3 + H 3 read, E 3 written
+         "e_update": 9,      # E 3 + H 3 read, E 3 written
+         "eh_fused": 12}     # E 3 + H 3 read, E 3 + H 3 written: eq. 11 fused with the merged H update
 OTHER_CONFIGS = (2, 3, 4, 6)
 
 
@@ -253,6 +254,8 @@ def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
              "hm_first": sum(bool(mask & MAT_BITS[m]) for m in ("Ms", "alpha", "gamma", "mu_r")),
              "e_update": sum(bool(mask & MAT_BITS[m]) for m in ("eps_r", "sigma"))}
     extra["hm_iter"] = extra["hm_second"] = extra["hm_first"]
+    extra["eh_fused"] = extra["e_update"]
+    fused = prof["eh_fused"][1] > 0        # the E phase ran by regions: fused outside the box, E only in it
     prof = dict(prof)                       # r = 2 and r >= 3 are the same kernel: one class
     a2, b2 = prof.pop("hm_second"), prof["hm_iter"]
     prof["hm_iter"] = (a2[0] + b2[0], a2[1] + b2[1])
@@ -268,7 +271,11 @@ def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
             if cls.startswith("hm_"):
                 ncell = box
             elif cls == "e_update":
-                ncell = cells
+                ncell = (box if fused else cells) * K / cnt
+            elif cls == "eh_fused":
+                ncell = (cells - box) * K / cnt
+            elif fused:
+                continue            # left-over faces of a region that could not be fused: not modelled
             else:
                 ncell = (cells - box) * (1 if st["merged_h"] else 2) * K / cnt
             ent["alg_bytes_per_launch"] = 8.0 * (WORDS[cls] + extra[cls]) * ncell
@@ -280,7 +287,8 @@ def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
     dom_kernel = {"h_update": "k_h_update",
                   "hm_first": "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
                   "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
-                  "e_update": "k_e_update"}[dom]
+                  "e_update": "k_eh_stage<E>" if fused else "k_e_update",
+                  "eh_fused": "k_eh_stage<E+H>"}[dom]
     achieved = per_class[dom]["alg_GBps"]
     step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
     traffic = _ncu_traffic(dom_kernel, name)

@@ -142,7 +142,8 @@ enum {
   FDTD_LLG_K_E_UPDATE = 4,   /* eq. 11                                                          */
   FDTD_LLG_K_OTHER = 5,      /* source amplitudes, half-step bookkeeping, canonical-buffer copy */
   FDTD_LLG_K_HM_SECOND = 6,  /* LLG iterate r = 2 that ran                                       */
-  FDTD_LLG_K_NCLASS = 7
+  FDTD_LLG_K_EH_FUSED = 7,   /* eq. 11 fused with the merged H update of the same faces (merge_h) */
+  FDTD_LLG_K_NCLASS = 8
 };
 
 /* Fill *opt with the defaults: PEC x3, LLG on, no bias, no anisotropy (axis z), tol 1e-6

@@ -70,7 +70,8 @@ EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_cre
 # sub-steps of one time step (fdtd_llg.h FDTD_LLG_SUB_*)
 SUB_BEGIN, SUB_HM1, SUB_HM1_END, SUB_E, SUB_HM2, SUB_HM2_END = range(6)
 
-KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other", "hm_second")
+KERNEL_CLASSES = ("h_update", "hm_first", "hm_iter", "hm_skipped", "e_update", "other", "hm_second",
+                  "eh_fused")
 
 _VP = C.c_void_p
 _PP = C.POINTER(C.c_void_p)

@@ -1,0 +1,266 @@
+// eh_stage.cuh -- the staged Maxwell sweep: eq. 11 and, FUSED with it on the
+// faces no magnetic face reads, the H update that follows it (eq. 21 with M = 0).
+//
+// Same arithmetic as k_e_update / k_h_update (kernels.cuh: e_edge_val, h_face_val); what differs is
+// how operands reach it and how often memory is touched.  A persistent block owns a tile of
+// SW x SBY columns and marches in z; THREAD = CELL (its three edges and three faces), warp = tile
+// row, lane = x.  One producer warp stages, per plane, a (SW+4) x (SBY+2) box of every operand
+// array (H^{n+1/2} x3, E^n x3, eps_r, sigma) in shared memory with cp.async.bulk.tensor, in a
+// ring of NS stages under full / empty mbarriers; plane q is computed from stages q-1 and q.
+//
+// FUSE (merged H half-steps, options.merge_h): outside the LLG sweep box the H update that follows
+// the E update -- second half-step of this step and first of the next, both with curl E^{n+1}
+// -- reads nothing but E^{n+1} around the face and its own H.  The block therefore
+// keeps the E^{n+1} plane it just computed in shared memory (with the one-cell rim on the high
+// side, computed by an extra warp) and takes H^{n+1/2} -> H^{n+3/2} in the same pass: per cell and
+// step E 3 + H 3 read, E 3 + H 3 written = 12 words instead of 9 + 9 (and 27 with two half-steps).
+// All inputs are time-n sets that nobody writes during the pass (every update is out of place),
+// so tiles and planes can be visited in any order.
+#pragma once
+#include "hm_stage.cuh"
+
+namespace fl {
+
+constexpr int EW = SW + 4;                   // staged row: x0-2 .. x0+33 (16-byte multiples)
+constexpr int EROWS = SBY + 2;               // rows y0-1 .. y0+16
+constexpr int ESLOT = round16(EROWS * EW);   // doubles per staged array
+constexpr int NROWS = SBY + 1;               // E^{n+1} plane kept for the H update: rows y0 .. y0+16,
+constexpr int NSLOT_D = round16(NROWS * EW); // columns x0 .. x0+32 (row pitch EW)
+
+template <bool FUSE, bool EPS_ARR, bool SIG_ARR>
+struct EhLayout {
+  static constexpr int HH = 0;                          // H x, y, z
+  static constexpr int EE = 3 * ESLOT;                  // E^n x, y, z
+  static constexpr int EP = 6 * ESLOT;                  // eps_r
+  static constexpr int SG = (6 + (EPS_ARR ? 1 : 0)) * ESLOT;   // sigma
+  static constexpr int NARR = 6 + (EPS_ARR ? 1 : 0) + (SIG_ARR ? 1 : 0);
+  static constexpr int STAGE = NARR * ESLOT;
+  static constexpr unsigned BYTES = 8u * NARR * EROWS * EW;    // bytes the TMA writes per stage
+  static constexpr int ENEW = FUSE ? 3 * 3 * NSLOT_D : 0;      // three rotating planes of E^{n+1} x, y, z
+  static constexpr int BUDGET = 220 * 1024 - 8 * ENEW;
+  static constexpr int NS_FIT = BUDGET / (8 * STAGE);
+  static constexpr int NS = NS_FIT > 6 ? 6 : NS_FIT;
+  static constexpr int NCW = SBY + (FUSE ? 1 : 0);      // compute warps (+1: the rim of E^{n+1})
+  static constexpr int NTHREADS = (NCW + 1) * 32;
+  static constexpr size_t SMEM_BYTES = 128 + 8 * (size_t)(NS * STAGE + ENEW) + 8 * (2 * NS) + 4 * NS;
+  static_assert(NS >= 3, "ring too shallow");
+};
+
+struct EHArgs {
+  GridP g;
+  StBox tb;            // the cells this launch updates, cut into work items
+  CUtensorMap map;     // box (EW, EROWS, 1, 1) of the workspace tensor
+  int aE, aH, aEps, aSig;   // array indices (4th tensor coordinate) of E^n_x, H_x, eps_r, sigma
+  double *Eo[3];       // E^{n+1}: the other E set
+  double *Ho[3];       // FUSE: H^{n+3/2}, the other half-time H set
+  double eps_u, sigma_u;    // uniform values (eps_u is eps0 * eps_r)
+  double chm;          // FUSE: cmul * dt / (2 mu) = dt / mu (uniform mu)
+  SourcesP src;
+  const DevState *st;
+  unsigned *work;      // item counter of this launch (zero at launch; k_half_end re-arms it)
+  int *pipe_error;
+};
+
+// the TMA loads of stage pz of the tile at (x0, y0): every array with the same box origin
+template <class L, bool EPS_ARR, bool SIG_ARR>
+__device__ __forceinline__ void eh_issue_stage(const EHArgs &p, double *dst, uint64_t *bar, int x0, int y0, int pz) {
+  const int x = PADL + x0 - 2, y = y0, z = pz + 1;   // tensor coordinates: one ghost layer in y, z
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    tma_load_4d(dst + L::HH + d * ESLOT, &p.map, bar, x, y, z, p.aH + d);
+    tma_load_4d(dst + L::EE + d * ESLOT, &p.map, bar, x, y, z, p.aE + d);
+  }
+  if (EPS_ARR) tma_load_4d(dst + L::EP, &p.map, bar, x, y, z, p.aEps);
+  if (SIG_ARR) tma_load_4d(dst + L::SG, &p.map, bar, x, y, z, p.aSig);
+}
+
+// soft sources on the D-edge of cell (i,j,k)
+template <int D>
+__device__ __forceinline__ double eh_source(const EHArgs &a, int i, int j, int k) {
+  double J = 0.0;
+  for (int s = 0; s < a.src.count; ++s) {
+    const SourceP &S = a.src.s[s];
+    if (S.kind != 0 || S.comp != D) continue;
+    if (i < S.lo[0] || i >= S.hi[0] || j < S.lo[1] || j >= S.hi[1] || k < S.lo[2] || k >= S.hi[2])
+      continue;
+    double pr = 1.0;
+    if (S.profile) {
+      const long long bx = S.hi[0] - S.lo[0], by = S.hi[1] - S.lo[1];
+      pr = __ldg(S.profile + (i - S.lo[0]) + bx * ((j - S.lo[1]) + by * (long long)(k - S.lo[2])));
+    }
+    J += a.st->src_amp[s] * pr;
+  }
+  return J;
+}
+
+// E^{n+1} on the D-edge at staged position t (A = stage q-1, B = stage q), grid position (i,j,k):
+// the operands of e_edge_val in the order k_e_update fetches them
+template <class L, int D, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
+__device__ __forceinline__ double eh_edge(const EHArgs &a, const double *A, const double *B, int t, int i,
+                                          int j, int k) {
+  constexpr int HX = L::HH, HY = L::HH + ESLOT, HZ = L::HH + 2 * ESLOT;
+  // offsets of the two transverse neighbours: s1 = stride of axis D+1, s2 = stride of axis D+2
+  double h2, h2m, h1, h1m, e0, m00 = 0, m10 = 0, m01 = 0, m11 = 0, g00 = 0, g10 = 0, g01 = 0, g11 = 0;
+  if (D == 0) {         // s1 = y, s2 = z
+    h2 = B[HZ + t]; h2m = B[HZ + t - EW]; h1 = B[HY + t]; h1m = A[HY + t];
+    e0 = B[L::EE + t];
+    if (EPS_ARR) { m00 = B[L::EP + t]; m10 = B[L::EP + t - EW]; m01 = A[L::EP + t]; m11 = A[L::EP + t - EW]; }
+    if (SIG_ARR) { g00 = B[L::SG + t]; g10 = B[L::SG + t - EW]; g01 = A[L::SG + t]; g11 = A[L::SG + t - EW]; }
+  } else if (D == 1) {  // s1 = z, s2 = x
+    h2 = B[HX + t]; h2m = A[HX + t]; h1 = B[HZ + t]; h1m = B[HZ + t - 1];
+    e0 = B[L::EE + ESLOT + t];
+    if (EPS_ARR) { m00 = B[L::EP + t]; m10 = A[L::EP + t]; m01 = B[L::EP + t - 1]; m11 = A[L::EP + t - 1]; }
+    if (SIG_ARR) { g00 = B[L::SG + t]; g10 = A[L::SG + t]; g01 = B[L::SG + t - 1]; g11 = A[L::SG + t - 1]; }
+  } else {              // s1 = x, s2 = y
+    h2 = B[HY + t]; h2m = B[HY + t - 1]; h1 = B[HX + t]; h1m = B[HX + t - EW];
+    e0 = B[L::EE + 2 * ESLOT + t];
+    if (EPS_ARR) { m00 = B[L::EP + t]; m10 = B[L::EP + t - 1]; m01 = B[L::EP + t - EW]; m11 = B[L::EP + t - EW - 1]; }
+    if (SIG_ARR) { g00 = B[L::SG + t]; g10 = B[L::SG + t - 1]; g01 = B[L::SG + t - EW]; g11 = B[L::SG + t - EW - 1]; }
+  }
+  double eps = a.eps_u, sig = a.sigma_u;
+  if (EPS_ARR) eps = kEps0 * (0.25 * ((m00 + m10) + (m01 + m11)));   // four-cell means
+  if (SIG_ARR) sig = 0.25 * ((g00 + g10) + (g01 + g11));
+  double J = 0.0;
+  if (HAS_SRC) J = eh_source<D>(a, i, j, k);
+  // wall-tangential edges stay 0: the lower walls, and index n of a PEC axis (the
+  // upper wall, which the rim of a tile at the end of the grid reaches)
+  constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
+  const int idx[3] = {i, j, k};
+  const bool wall = (a.g.wall[d1] && idx[d1] == 0) || (a.g.wall[d2] && idx[d2] == 0) ||
+                    (a.g.wallhi[d1] && idx[d1] == a.g.n[d1]) || (a.g.wallhi[d2] && idx[d2] == a.g.n[d2]);
+  return e_edge_val<D>(a.g, eps, sig, J, e0, h2, h2m, h1, h1m, wall);
+}
+
+template <bool FUSE, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
+__global__ void __launch_bounds__(EhLayout<FUSE, EPS_ARR, SIG_ARR>::NTHREADS, 1)
+k_eh_stage(const __grid_constant__ EHArgs p) {
+  using L = EhLayout<FUSE, EPS_ARR, SIG_ARR>;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double *const ring = reinterpret_cast<double *>(smem_raw);
+  double *const enew = ring + L::NS * L::STAGE;                 // FUSE: 3 planes x 3 components
+  uint64_t *const full = reinterpret_cast<uint64_t *>(enew + L::ENEW);
+  uint64_t *const empty = full + L::NS;
+  int *const meta = reinterpret_cast<int *>(empty + L::NS);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < L::NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, L::NCW); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  const StBox &T = p.tb;
+  const GridP &g = p.g;
+  // planes staged per item: q = k0-1 .. k1-1, and k1 too when the H update needs E^{n+1}(k1)
+  constexpr int XTRA = FUSE ? 1 : 0;
+  if (warp == L::NCW) {
+    // ===== producer
+    if (lane == 0) {
+      tma_prefetch_desc(&p.map);
+      unsigned n = 0;
+      for (;;) {
+        const int it = (int)atomicAdd(p.work, 1u);
+        const bool end = it >= T.items;
+        const StItem w = st_decode(T, end ? 0 : it);
+        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1 + XTRA); ++pz, ++n) {
+          const unsigned s = n % L::NS, u = n / L::NS;
+          if (!mbar_wait(empty + s, (u & 1) ^ 1, p.pipe_error, 4)) return;
+          meta[s] = end ? -1 : it;
+          if (end) {
+            mbar_arrive(full + s);
+            break;
+          }
+          mbar_expect_tx(full + s, L::BYTES);
+          eh_issue_stage<L, EPS_ARR, SIG_ARR>(p, ring + s * L::STAGE, full + s, w.x0, w.y0, pz);
+        }
+        if (end) break;
+      }
+    }
+    return;
+  }
+  // ===== compute warps.  warp < SBY: tile row `warp`, lane = x, thread = cell.  warp == SBY (FUSE):
+  // the rim of the E^{n+1} plane the H update reads on the high side: row y0 + SBY (E_x, E_z) and
+  // column x0 + SW (E_y, E_z)
+  const bool rim = FUSE && warp == SBY;
+  const int t0 = (warp + 1) * EW + lane + 2;   // own staged position
+  const int u0 = warp * EW + lane;             // own position in the E^{n+1} plane
+  unsigned n = 0;
+  for (;;) {
+    if (!mbar_wait(full + n % L::NS, (n / L::NS) & 1, p.pipe_error, 5)) return;
+    const int it = *(volatile int *)(meta + n % L::NS);
+    if (it < 0) break;
+    const StItem w = st_decode(T, it);
+    const int i = w.x0 + lane, j = w.y0 + warp;
+    const bool valid = !rim && i < T.hi[0] && j < T.hi[1];
+    const Column col = make_column(g, i, j);
+    int c = g.org + i + g.sy * j + g.sz * w.k0;
+    double ex_p = 0.0, ey_p = 0.0, ez_p = 0.0;   // own E^{n+1} of the previous plane (FUSE)
+    for (int q = w.k0; q < w.k1 + XTRA; ++q, ++n) {
+      const double *A = ring + (n % L::NS) * L::STAGE;
+      const double *B = ring + ((n + 1) % L::NS) * L::STAGE;
+      if (!mbar_wait(full + (n + 1) % L::NS, ((n + 1) / L::NS) & 1, p.pipe_error, 6)) return;
+      double *N = enew + (FUSE ? (q % 3) * 3 * NSLOT_D : 0);
+      double ex = 0.0, ey = 0.0, ez = 0.0;
+      if (!rim) {
+        ex = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
+        ey = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
+        ez = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
+        if (FUSE) { N[u0] = ex; N[NSLOT_D + u0] = ey; N[2 * NSLOT_D + u0] = ez; }
+        if (valid && q < w.k1) {
+          p.Eo[0][c] = ex;
+          p.Eo[1][c] = ey;
+          p.Eo[2][c] = ez;
+          if (col.edge_ij || edge_k(g, q)) {
+            store_images_inl<exp_of_e<0>()>(p.Eo[0], g, i, j, q, c, ex);
+            store_images_inl<exp_of_e<1>()>(p.Eo[1], g, i, j, q, c, ey);
+            store_images_inl<exp_of_e<2>()>(p.Eo[2], g, i, j, q, c, ez);
+          }
+        }
+      } else {
+        {  // row y0 + SBY: E_x, E_z at (x0 + lane, y0 + SBY)
+          const int tr = (SBY + 1) * EW + lane + 2, ur = SBY * EW + lane;
+          N[ur] = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q);
+          N[2 * NSLOT_D + ur] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q);
+        }
+        if (lane < SBY) {  // column x0 + SW: E_y, E_z at (x0 + SW, y0 + lane)
+          const int tc = (lane + 1) * EW + SW + 2, uc = lane * EW + SW;
+          N[NSLOT_D + uc] = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q);
+          N[2 * NSLOT_D + uc] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q);
+        }
+      }
+      if (FUSE) {
+        // every warp's part of E^{n+1}(q) is in shared memory; the plane q-1 the H update reads was
+        // completed one barrier earlier, and the plane written next (q+1) was last read two
+        // barriers ago: three rotating planes, one barrier per plane
+        asm volatile("bar.sync 1, %0;" ::"n"(L::NCW * 32) : "memory");
+        if (valid && q > w.k0) {
+          const double *P = enew + ((q - 1) % 3) * 3 * NSLOT_D;
+          const int cm = c - g.sz;   // plane q-1
+          // (curl E^{n+1})_D at the D-face of plane q-1: forward differences, as curl_e (kernels.cuh)
+          const double cx = (P[2 * NSLOT_D + u0 + EW] - ez_p) * g.rd[1] - (ey - ey_p) * g.rd[2];
+          const double cy = (ex - ex_p) * g.rd[2] - (P[2 * NSLOT_D + u0 + 1] - ez_p) * g.rd[0];
+          const double cz = (P[NSLOT_D + u0 + 1] - ey_p) * g.rd[0] - (P[u0 + EW] - ex_p) * g.rd[1];
+          const double hx = h_face_val(A[L::HH + t0], p.chm, cx, col.wall[0]);
+          const double hy = h_face_val(A[L::HH + ESLOT + t0], p.chm, cy, col.wall[1]);
+          const double hz = h_face_val(A[L::HH + 2 * ESLOT + t0], p.chm, cz, wall_k(g, q - 1));
+          p.Ho[0][cm] = hx;
+          p.Ho[1][cm] = hy;
+          p.Ho[2][cm] = hz;
+          if (col.edge_ij || edge_k(g, q - 1)) {
+            store_images_inl<exp_of_h<0>()>(p.Ho[0], g, i, j, q - 1, cm, hx);
+            store_images_inl<exp_of_h<1>()>(p.Ho[1], g, i, j, q - 1, cm, hy);
+            store_images_inl<exp_of_h<2>()>(p.Ho[2], g, i, j, q - 1, cm, hz);
+          }
+        }
+        ex_p = ex; ey_p = ey; ez_p = ez;
+      }
+      c += g.sz;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + n % L::NS);  // stage q-1 is done with
+    }
+    if (lane == 0) mbar_arrive(empty + n % L::NS);    // the item's last stage: the next item starts afresh
+    ++n;
+  }
+}
+
+}  // namespace fl

@@ -16,6 +16,7 @@
 #include "../../include/fdtd_llg.h"
 #include "kernels.cuh"
 #include "hm_stage.cuh"
+#include "eh_stage.cuh"
 
 using namespace fl;
 
@@ -67,6 +68,10 @@ struct fdtd_llg {
   bool staged = false;  // the LLG iterates run the staged sweep (hm_stage.cuh)
   StBox st_box{}, st_box_first{};  // work items of the iterates r >= 2 / of the r = 1 sweep
   CUtensorMap mapT{}, mapPM{};
+  // staged Maxwell sweeps (eh_stage.cuh): the E update, fused with the merged H update outside the box
+  bool eh_ok = false;        // tensor map built, kernels configured (no PML, kernel_path != 1)
+  CUtensorMap mapEH{};
+  unsigned *work_eh = nullptr;  // [8] item counters, one per staged launch of a step
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
   // open boundary: split parts of E and H, damping tables, the layer's slabs
@@ -494,6 +499,43 @@ int setup_hm_stage(fdtd_llg *s) {
   return FDTD_LLG_OK;
 }
 
+// ---- staged Maxwell sweeps (eh_stage.cuh) ----------------------------------------------------
+
+template <bool FUSE>
+int launch_eh_stage(fdtd_llg *s, const EHArgs &p) {
+  const bool ea = s->eps_r.is_array, sa = s->sigma.is_array;
+  bool hs = false;
+  for (int q = 0; q < s->src.count; ++q) hs = hs || s->src.s[q].kind == FDTD_LLG_SRC_SOFT_E;
+  const int grid = std::max(1, std::min(p.tb.items, s->num_sms));   // one persistent block per SM
+#define EK(EA, SA, HS)                                                                          \
+  if (ea == EA && sa == SA && hs == HS) {                                                       \
+    using L = EhLayout<FUSE, EA, SA>;                                                           \
+    k_eh_stage<FUSE, EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);           \
+    return FDTD_LLG_OK;                                                                         \
+  }
+  EK(false, false, false) EK(false, false, true) EK(false, true, false) EK(false, true, true)
+  EK(true, false, false) EK(true, false, true) EK(true, true, false) EK(true, true, true)
+#undef EK
+  return FDTD_LLG_OK;
+}
+
+int setup_eh_stage(fdtd_llg *s) {
+#define SA(FUSE, EA, SA_, HS)                                                                   \
+  CU(s, cudaFuncSetAttribute(k_eh_stage<FUSE, EA, SA_, HS>,                                     \
+                             cudaFuncAttributeMaxDynamicSharedMemorySize,                       \
+                             (int)EhLayout<FUSE, EA, SA_>::SMEM_BYTES));
+#define SA8(FUSE) SA(FUSE, false, false, false) SA(FUSE, false, false, true) SA(FUSE, false, true, false) \
+  SA(FUSE, false, true, true) SA(FUSE, true, false, false) SA(FUSE, true, false, true)          \
+  SA(FUSE, true, true, false) SA(FUSE, true, true, true)
+  SA8(false) SA8(true)
+#undef SA8
+#undef SA
+  int rc = make_map(s, &s->mapEH, EW, EROWS, 1);
+  if (rc) return rc;
+  s->eh_ok = true;
+  return FDTD_LLG_OK;
+}
+
 // ---- open boundary (A26) ---------------------------------------------
 
 // decay rate s_a(x) of the layer on axis a at position x (host, long double)
@@ -673,7 +715,18 @@ bool merge_allowed(const fdtd_llg *s) {
 
 // Maxwell update of the faces outside the sweep box (eq. 21 with M = 0):
 // set `out` = set `in` - cmul (dt / 2 mu) curl E; cmul = 1: half a step, 2: two half-steps at once
-int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul, bool exports, int *launches) {
+// The E phase by regions.  The LLG sweep box and the slabs of its complement each get one launch:
+//   staged  the TMA-fed sweep of eh_stage.cuh (else the direct-load kernel k_e_update);
+//   fuse    the sweep also takes the merged H update of the region (merge_h): its faces are then
+//           skipped by the second half-step's enqueue_outside.
+struct ERegion {
+  int lo[3], hi[3];
+  bool staged, fuse;
+};
+int plan_e_regions(const fdtd_llg *s, ERegion *out);
+int count_sources(const fdtd_llg *s, int kind);
+int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul, bool exports, int *launches,
+                    bool skip_fused = false) {
   const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
@@ -682,8 +735,25 @@ int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul,
   h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
   h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
   h.cmul = cmul;
-  for (int b = 0; b < s->n_out; ++b) {
-    h.box = s->box_out[b];
+  BoxP boxes[16];
+  int nb = 0;
+  if (!skip_fused) {
+    for (int b = 0; b < s->n_out; ++b) boxes[nb++] = s->box_out[b];
+  } else {  // the faces whose merged update the E phase did not take along
+    ERegion reg[16];
+    const int nr = plan_e_regions(s, reg);
+    const bool whole = nr == 1 && !reg[0].staged && reg[0].lo[0] == 0 && reg[0].hi[0] == s->g.n[0] &&
+                       reg[0].lo[1] == 0 && reg[0].hi[1] == s->g.n[1] && reg[0].lo[2] == 0 && reg[0].hi[2] == s->g.n[2];
+    if (whole) {
+      for (int b = 0; b < s->n_out; ++b) boxes[nb++] = s->box_out[b];
+    } else {
+      const int nreg_out = nr - (s->llg ? 1 : 0);   // the last region is the sweep box
+      for (int r = 0; r < nreg_out; ++r)
+        if (!reg[r].fuse) boxes[nb++] = make_box(s, reg[r].lo, reg[r].hi);
+    }
+  }
+  for (int b = 0; b < nb; ++b) {
+    h.box = boxes[b];
     if (h.box.items == 0) continue;
     const int grid = grid_for(s, h.box, 0);
     prof_begin(s, FDTD_LLG_K_H_UPDATE, 0);
@@ -703,7 +773,7 @@ int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul,
 int enqueue_half_pre(fdtd_llg *s, double *const *E, int in, int out, int merged_to, int *launches) {
   int rc = FDTD_LLG_OK;
   if (!s->merge) rc = enqueue_outside(s, E, in, out, 1.0, true, launches);
-  else if (merged_to >= 0) rc = enqueue_outside(s, E, in, merged_to, 2.0, true, launches);
+  else if (merged_to >= 0) rc = enqueue_outside(s, E, in, merged_to, 2.0, true, launches, true);
   if (rc) return rc;
   return enqueue_pml(s, false, E, s->Hset[out], launches);
 }
@@ -770,7 +840,7 @@ int enqueue_sweep(fdtd_llg *s, double *const *E, int in, int out, int tmp, int m
 int enqueue_half_end(fdtd_llg *s, int out, int tmp, int r_max, bool last, int *launches) {
   const dim3 blk(TX, TY, 1);
   prof_begin(s, FDTD_LLG_K_OTHER, 0);
-  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->r_hist, r_max, s->opt.llg_max_iter,
+  k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->work_eh, s->r_hist, r_max, s->opt.llg_max_iter,
                                      s->opt.llg_tol, s->llg ? 1 : 0, last ? 1 : 0);
   ++*launches;
   if (s->llg && r_max >= 2) {
@@ -824,11 +894,12 @@ int count_sources(const fdtd_llg *s, int kind) {
   return n;
 }
 
-int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int *launches) {
+// eq. 11 on one region of the grid with the direct-load kernel
+int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, const BoxP &box, int *launches) {
   const dim3 blk(TX, TY, 1);
   EArgs a{};
   a.g = s->g;
-  a.box = s->box_all;
+  a.box = box;
   for (int d = 0; d < 3; ++d) { a.E[d] = Ein[d]; a.Eo[d] = Eout[d]; a.H[d] = s->Hset[hset][d]; }
   a.eps_r = s->eps_r.dev; a.sigma = s->sigma.dev;
   a.eps_u = kEps0 * s->eps_r.uniform; a.sigma_u = s->sigma.uniform;
@@ -844,6 +915,81 @@ int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, in
 #undef EK
   prof_end(s);
   ++*launches;
+  CU(s, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
+
+int plan_e_regions(const fdtd_llg *s, ERegion *out) {
+  const int zero[3] = {0, 0, 0};
+  auto put = [&](int n, const int *lo, const int *hi, bool staged, bool fuse) {
+    for (int d = 0; d < 3; ++d) { out[n].lo[d] = lo[d]; out[n].hi[d] = hi[d]; }
+    out[n].staged = staged;
+    out[n].fuse = fuse;
+    return n + 1;
+  };
+  const bool can_fuse = s->merge && !s->mu_r.is_array && count_sources(s, FDTD_LLG_SRC_HARD_E) == 0;
+  int n = 0;
+  long long items = 0;
+  if (s->eh_ok) {
+    for (int b = 0; b < s->n_out; ++b) {
+      const BoxP &B = s->box_out[b];
+      if (B.items == 0) continue;
+      const bool st = (B.lo[0] & 1) == 0;   // staged boxes begin on 16-byte boundaries
+      int hi[3] = {B.hi[0], B.hi[1], B.hi[2]};
+      if (st && can_fuse && s->g.ext[1] && hi[2] == s->g.n[2]) {
+        // a slab's last plane needs E^{n+1} of the upper neighbour's first plane, which arrives with
+        // that neighbour's E phase: its H update stays in the second half-step
+        const int lo_top[3] = {B.lo[0], B.lo[1], std::max(B.lo[2], hi[2] - 1)};
+        n = put(n, lo_top, hi, false, false);
+        hi[2] -= 1;
+        if (hi[2] <= B.lo[2]) continue;
+      }
+      n = put(n, B.lo, hi, st, st && can_fuse);
+      if (st) items += make_stbox(B.lo, hi, SBY, 32).items;
+    }
+    if (s->llg) {
+      const bool st = (s->lo[0] & 1) == 0;
+      n = put(n, s->lo, s->hi, st, false);
+      if (st) items += make_stbox(s->lo, s->hi, SBY, 32).items;
+    }
+  }
+  // a grid that cannot give every SM an item is latency bound: one direct-load launch serves it better
+  if (!s->eh_ok || (items < s->num_sms && s->opt.kernel_path != 5)) return put(0, zero, s->g.n, false, false);
+  return n;
+}
+
+int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int hset_next, int *launches) {
+  ERegion reg[16];
+  const int nr = plan_e_regions(s, reg);
+  int widx = 0;
+  for (int r = 0; r < nr; ++r) {
+    if (!reg[r].staged) {
+      int rc = enqueue_e(s, Ein, Eout, hset, make_box(s, reg[r].lo, reg[r].hi), launches);
+      if (rc) return rc;
+      continue;
+    }
+    EHArgs p{};
+    p.g = s->g;
+    p.tb = make_stbox(reg[r].lo, reg[r].hi, SBY, 32);
+    p.map = s->mapEH;
+    p.aE = array_index(s, Ein[0]);
+    p.aH = array_index(s, s->Hset[hset][0]);
+    p.aEps = s->eps_r.is_array ? array_index(s, s->eps_r.dev) : 0;
+    p.aSig = s->sigma.is_array ? array_index(s, s->sigma.dev) : 0;
+    for (int d = 0; d < 3; ++d) { p.Eo[d] = Eout[d]; p.Ho[d] = s->Hset[hset_next][d]; }
+    p.eps_u = kEps0 * s->eps_r.uniform;
+    p.sigma_u = s->sigma.uniform;
+    p.chm = 2.0 * (s->dt / (2.0 * kMu0 * s->mu_r.uniform));   // cmul * ch of k_h_update, cmul = 2
+    p.src = s->src;
+    p.st = s->dstate;
+    p.work = s->work_eh + widx++;
+    p.pipe_error = &s->dstate->pipe_error;
+    prof_begin(s, reg[r].fuse ? FDTD_LLG_K_EH_FUSED : FDTD_LLG_K_E_UPDATE, 0);
+    int rc = reg[r].fuse ? launch_eh_stage<true>(s, p) : launch_eh_stage<false>(s, p);
+    prof_end(s);
+    if (rc) return rc;
+    ++*launches;
+  }
   CU(s, cudaGetLastError());
   return FDTD_LLG_OK;
 }
@@ -898,7 +1044,7 @@ int enqueue_begin(fdtd_llg *s, int *launches) {
 int enqueue_e_phase(fdtd_llg *s, int par, int *launches) {
   double *const *Ea = e_set(s, par), *const *Eb = e_set(s, par ^ 1);
   const int h1 = set_half(s, par);
-  int rc = enqueue_e(s, Ea, Eb, h1, launches);
+  int rc = enqueue_e_regions(s, Ea, Eb, h1, set_half(s, par ^ 1), launches);
   if (rc) return rc;
   rc = enqueue_pml(s, true, s->Hset[h1], Eb, launches);
   if (rc) return rc;
@@ -1062,6 +1208,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   for (int d = 0; d < 3; ++d) {
     s->g.per[d] = opt->bc[d] == FDTD_LLG_PERIODIC;
     s->g.wall[d] = opt->bc[d] == FDTD_LLG_PEC;
+    s->g.wallhi[d] = s->g.wall[d];
     s->g.rd[d] = 1.0 / s->d[d];
   }
   // a slab interface is neither wall nor wrap; with one interface the other z side keeps its wall
@@ -1069,6 +1216,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->g.ext[0] = opt->slab_ext[0];
   s->g.ext[1] = opt->slab_ext[1];
   if (s->g.ext[0]) s->g.wall[2] = 0;
+  if (s->g.ext[1]) s->g.wallhi[2] = 0;
   s->is_slab = s->g.ext[0] || s->g.ext[1];
   s->g.dt = dt;
   s->dt = dt;
@@ -1105,6 +1253,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->dstate = reinterpret_cast<DevState *>(p); p += 4096;
   s->resid = reinterpret_cast<unsigned long long *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8;
   s->work = reinterpret_cast<unsigned *>(p); p += padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 4096;
+  s->work_eh = s->work + 2 * padded((size_t)(s->opt.llg_max_iter + 2));   // in the 4 KB behind the sweeps' counters
   s->scratch = reinterpret_cast<double *>(p); p += (2 * 1024 + 64) * 8;
   s->profile_pool = reinterpret_cast<double *>(p); s->profile_cap = ((size_t)1 << 20) / 8; p += (size_t)1 << 20;
   s->r_hist = reinterpret_cast<int *>(p); p += (size_t)R_HIST * sizeof(int);
@@ -1142,6 +1291,7 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
               (s->lo[0] & 1) == 0 && opt->kernel_path != 1;
   if (s->staged && (rc = setup_hm_stage(s))) return bail(rc);
   s->merge = merge_allowed(s);
+  if (!s->has_pml && opt->kernel_path != 1 && (rc = setup_eh_stage(s))) return bail(rc);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
   *out = s;
@@ -1183,7 +1333,7 @@ int fdtd_llg_set_fields(fdtd_llg *s, const double *const *E, const double *const
   // reset run state
   CU(s, cudaMemsetAsync(s->dstate, 0, sizeof(DevState), s->stream));
   CU(s, cudaMemsetAsync(s->resid, 0, (size_t)(s->opt.llg_max_iter + 2) * 8, s->stream));
-  CU(s, cudaMemsetAsync(s->work, 0, (size_t)(s->opt.llg_max_iter + 2) * 4, s->stream));
+  CU(s, cudaMemsetAsync(s->work, 0, padded((size_t)(s->opt.llg_max_iter + 2)) * 8 + 64, s->stream));
   if (s->opt.enable_llg) {
     InitMP a{};
     a.g = s->g;

@@ -49,7 +49,8 @@ constexpr double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
 struct GridP {
   int n[3];    // nx, ny, nz
   int per[3];  // 1 = periodic (the ghost layer mirrors the opposite interior plane)
-  int wall[3]; // 1 = PEC wall at index 0 and at index n
+  int wall[3]; // 1 = PEC wall at index 0
+  int wallhi[3]; // 1 = PEC wall at index n (differs from wall[2] on a slab with one interface)
   int ext[2];  // z-low / z-high side is an interface to a neighbouring slab (neither of the above)
   int sy, sz;  // element strides of j and k (the stride of i is 1)
   int org;     // offset of cell (0,0,0)
@@ -217,6 +218,13 @@ struct HArgs {
                        // magnetic face reads, taken at once with the same curl E
 };
 
+// eq. 21 with M = 0 on one face: hn = H on the face, chm = cmul dt / (2 mu), C =
+// (curl E)_D there; a PEC wall face stays 0.  Shared by k_h_update and k_eh_stage.
+__device__ __forceinline__ double h_face_val(double hn, double chm, double C, bool wall) {
+  const double h = hn - chm * C;
+  return wall ? 0.0 : h;
+}
+
 // eq. 21 with M = 0 and the local mu; a PEC wall face stays 0
 template <int D, bool MU_ARR>
 __device__ __forceinline__ double h_face(const HArgs &a, int c, bool wall) {
@@ -226,9 +234,9 @@ __device__ __forceinline__ double h_face(const HArgs &a, int c, bool wall) {
     ch = a.g.dt / (2.0 * kMu0 * mu);
   }
   const double C = curl_e<D>(a.g, c, a.E);
-  // plain load: Hn aliases Hc when the integer-time H is formed in place (reconstruct_h)
-  const double h = a.Hn[D][c] - (a.cmul * ch) * C;   // cmul = 1, 2: an exact scaling
-  return wall ? 0.0 : h;
+  // plain load: Hn aliases Hc when the integer-time H is formed in place (reconstruct_h);
+  // cmul = 1, 2: an exact scaling
+  return h_face_val(a.Hn[D][c], a.cmul * ch, C, wall);
 }
 
 template <bool MU_ARR>
@@ -541,8 +549,10 @@ __global__ void k_set_cond(cudaGraphConditionalHandle h, const unsigned long lon
 // 1 thread: close an (H,M) half-step of which the iterates 1..r_max were enqueued (fdtd_llg_step:
 // all max_iter of them, those after convergence exit on the flag; fdtd_llg_substep: the caller
 // stops when an iterate met the tolerance)
-__global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, int *r_hist, int r_max,
-                           int max_iter, double tol, int any_magnetic, int last_of_step) {
+__global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, unsigned *work_eh,
+                           int *r_hist, int r_max, int max_iter, double tol, int any_magnetic,
+                           int last_of_step) {
+  for (int q = 0; q < 8; ++q) work_eh[q] = 0u;   // item counters of the staged Maxwell sweeps
   if (any_magnetic) {
     int R = r_max;
     for (int r = 1; r <= r_max; ++r)
@@ -599,7 +609,7 @@ __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ Cano
 
 struct EArgs {
   GridP g;
-  BoxP box;  // the whole grid
+  BoxP box;  // the cells this launch updates (the whole grid, or one region of it)
   const double *E[3];  // E^n
   double *Eo[3];       // E^{n+1}: the other E set (out of place)
   const double *H[3];
@@ -609,9 +619,21 @@ struct EArgs {
   const DevState *st;
 };
 
-// eq. 11 on the D-edge of the cell at offset c; a wall-tangential edge stays 0
-// (PAPER.md:187).  J = soft source term of this edge; e0 = E^n on the edge; (curl H)_D at the edge
-// by backward differences: h2 - h2m along d1 = D+1, h1 - h1m along d2 = D+2.
+// eq. 11 on a D-edge from its operands: eps, sig = the edge's four-cell means, J =
+// soft source term, e0 = E^n on the edge, (curl H)_D by backward differences: h2 - h2m along
+// d1 = D+1, h1 - h1m along d2 = D+2.  A wall-tangential edge stays 0.
+// Shared by k_e_update and k_eh_stage.
+template <int D>
+__device__ __forceinline__ double e_edge_val(const GridP &g, double eps, double sig, double J, double e0,
+                                             double h2, double h2m, double h1, double h1m, bool wall) {
+  constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
+  const double curl = (h2 - h2m) * g.rd[d1] - (h1 - h1m) * g.rd[d2];
+  const double edt = eps * (1.0 / g.dt), hs = 0.5 * sig;  // 1/dt is loop invariant: one division per edge
+  const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
+  return wall ? 0.0 : e1;
+}
+
+// eq. 11 on the D-edge of the cell at offset c, operands by direct loads
 template <int D, bool EPS_ARR, bool SIG_ARR>
 __device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, double J, double e0,
                                          double h2, double h2m, double h1, double h1m) {
@@ -625,10 +647,7 @@ __device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, doubl
   if (SIG_ARR)
     sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c - s1)) +
                   (__ldg(a.sigma + c - s2) + __ldg(a.sigma + c - s1 - s2)));
-  const double curl = (h2 - h2m) * a.g.rd[d1] - (h1 - h1m) * a.g.rd[d2];
-  const double edt = eps * (1.0 / a.g.dt), hs = 0.5 * sig;  // 1/dt is loop invariant: one division per edge
-  const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
-  return wall ? 0.0 : e1;
+  return e_edge_val<D>(a.g, eps, sig, J, e0, h2, h2m, h1, h1m, wall);
 }
 
 // everything the three edges of one cell read

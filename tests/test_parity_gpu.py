@@ -51,14 +51,14 @@ def test_parity_100_steps_all_configs(cfg):
     default at the sizes of test_fullsize_gpu.py and of the every-SM-busy test."""
     w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
     got, ref, gs, os_ = _run_both(w, 100)
+    from paper_2103_12819_b200.binding import from_workload
+    sim = from_workload(w, kernel_path=5)     # staged LLG sweeps and staged / fused Maxwell sweeps forced
     if w.enable_llg:
-        from paper_2103_12819_b200.binding import from_workload
-        sim = from_workload(w, kernel_path=5)
         assert sim.stats()["staged_sweeps"] == 1 and gs["staged_sweeps"] == 0
-        sim.step(100)
-        _assert_parity(_gpu_fields(sim), ref, True,
-                       record={"test": "parity_100_steps_small", "config": cfg, "shape": list(wl.SMALL_SHAPES[cfg]),
-                               "steps": 100, "path": "staged (kernel_path 5)"})
+    sim.step(100)
+    _assert_parity(_gpu_fields(sim), ref, w.enable_llg,
+                   record={"test": "parity_100_steps_small", "config": cfg, "shape": list(wl.SMALL_SHAPES[cfg]),
+                           "steps": 100, "path": "staged (kernel_path 5)"})
     _assert_parity(got, ref, w.enable_llg,
                    record={"test": "parity_100_steps_small", "config": cfg, "shape": list(wl.SMALL_SHAPES[cfg]),
                            "steps": 100, "path": "default", "iters": gs["iters_total"]})
@@ -145,6 +145,50 @@ def test_staged_and_tma_sweeps_equal_direct_load_kernels_bitwise(cfg, shape):
     for n in outs[0]:
         assert np.array_equal(outs[0][n], outs[1][n]), n
     assert stats[0]["iters_total"] == stats[1]["iters_total"] > 0
+
+
+@pytest.mark.parametrize("cfg,shape", [(2, (40, 36, 28)), (3, (72, 40, 36)), (3, (70, 33, 50)), (4, (44, 36, 40)),
+                                       (5, (70, 19, 23)), (2, (33, 17, 40))])
+def test_fused_maxwell_sweep_equals_the_separate_kernels_bitwise(cfg, shape):
+    """kernel_path 5 forces the staged sweeps of eh_stage.cuh (eq. 11 from a TMA-fed ring, fused with
+    the merged H update outside the LLG box); kernel_path 1 runs k_e_update + k_h_update with direct
+    loads.  They share e_edge_val / h_face_val: the same bits, on ragged tiles, with material
+    arrays (config 3), a soft source, periodic and PEC ends."""
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(cfg, shape=shape)
+    outs = []
+    for path in (1, 5):
+        sim = from_workload(w, kernel_path=path)
+        assert sim.stats()["merged_h"] == 1
+        sim.step(30)
+        outs.append(_gpu_fields(sim))
+    for n in outs[0]:
+        assert np.array_equal(outs[0][n], outs[1][n]), (n, float(np.max(np.abs(outs[0][n] - outs[1][n]))))
+
+
+def test_merged_h_equals_two_half_steps_to_rounding_and_reads_do_not_disturb():
+    """merge_h: one update instead of two half-steps with the same curl E: equal up to rounding
+    (1 ulp per step), and reading the fields mid-run (which forms the integer-time H) changes nothing."""
+    from paper_2103_12819_b200.binding import from_workload
+    for cfg in (3, 4):
+        w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
+        a = from_workload(w, merge_h=False)
+        b = from_workload(w, merge_h=True)
+        c = from_workload(w, merge_h=True)
+        assert a.stats()["merged_h"] == 0 and b.stats()["merged_h"] == 1
+        a.step(60)
+        b.step(60)
+        for n in (7, 1, 22, 30):
+            c.step(n)
+            mid = _gpu_fields(c)
+            again = _gpu_fields(c)          # a second read of the same state
+            for k in mid:
+                assert np.array_equal(mid[k], again[k]), k
+        fa, fb, fc = _gpu_fields(a), _gpu_fields(b), _gpu_fields(c)
+        for k in fb:
+            assert np.array_equal(fb[k], fc[k]), k
+        for g_ in ("E", "H") + (("M",) if w.enable_llg else ()):
+            assert rel_linf(fb, fa, g_) < 1e-13, (cfg, g_, rel_linf(fb, fa, g_))
 
 
 @pytest.mark.parametrize("cfg,shape", [(5, (200, 176, 300)), (4, (230, 150, 200))])
