@@ -54,6 +54,8 @@ struct EHArgs {
   double *Eo[3];       // E^{n+1}: the other E set
   double *Ho[3];       // FUSE: H^{n+3/2}, the other half-time H set
   double eps_u, sigma_u;    // uniform values (eps_u is eps0 * eps_r)
+  double rdt;               // 1 / dt
+  ECoef k_u;                // e_coef(eps_u, sigma_u, rdt): the coefficients when both maps are uniform
   double chm;          // FUSE: cmul * dt / (2 mu) = dt / mu (uniform mu)
   SourcesP src;
   const DevState *st;
@@ -95,9 +97,11 @@ __device__ __forceinline__ double eh_source(const EHArgs &a, int i, int j, int k
 
 // E^{n+1} on the D-edge at staged position t (A = stage q-1, B = stage q), grid position (i,j,k):
 // the operands of e_edge_val in the order k_e_update fetches them
+// `wall`: the edge is tangential to a PEC wall and stays 0: the lower walls, and
+// index n of a PEC axis (the upper wall, which the rim of a tile at the end of the grid reaches)
 template <class L, int D, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
 __device__ __forceinline__ double eh_edge(const EHArgs &a, const double *A, const double *B, int t, int i,
-                                          int j, int k) {
+                                          int j, int k, bool wall) {
   constexpr int HX = L::HH, HY = L::HH + ESLOT, HZ = L::HH + 2 * ESLOT;
   // offsets of the two transverse neighbours: s1 = stride of axis D+1, s2 = stride of axis D+2
   double h2, h2m, h1, h1m, e0, m00 = 0, m10 = 0, m01 = 0, m11 = 0, g00 = 0, g10 = 0, g01 = 0, g11 = 0;
@@ -122,13 +126,14 @@ __device__ __forceinline__ double eh_edge(const EHArgs &a, const double *A, cons
   if (SIG_ARR) sig = 0.25 * ((g00 + g10) + (g01 + g11));
   double J = 0.0;
   if (HAS_SRC) J = eh_source<D>(a, i, j, k);
-  // wall-tangential edges stay 0: the lower walls, and index n of a PEC axis (the
-  // upper wall, which the rim of a tile at the end of the grid reaches)
-  constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
-  const int idx[3] = {i, j, k};
-  const bool wall = (a.g.wall[d1] && idx[d1] == 0) || (a.g.wall[d2] && idx[d2] == 0) ||
-                    (a.g.wallhi[d1] && idx[d1] == a.g.n[d1]) || (a.g.wallhi[d2] && idx[d2] == a.g.n[d2]);
-  return e_edge_val<D>(a.g, eps, sig, J, e0, h2, h2m, h1, h1m, wall);
+  ECoef kc = a.k_u;
+  if (EPS_ARR || SIG_ARR) kc = e_coef(eps, sig, a.rdt);
+  return e_edge_val<D>(a.g, kc, J, e0, h2, h2m, h1, h1m, wall);
+}
+
+// index idx lies on a PEC wall of axis d (lower wall at 0, upper wall at n)
+__device__ __forceinline__ bool on_wall(const GridP &g, int d, int idx) {
+  return (g.wall[d] && idx == 0) || (g.wallhi[d] && idx == g.n[d]);
 }
 
 template <bool FUSE, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
@@ -157,14 +162,14 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
     // ===== producer
     if (lane == 0) {
       tma_prefetch_desc(&p.map);
-      unsigned n = 0;
+      unsigned s = 0, ph = 1;   // ring position and the parity its empty barrier is waited on
       for (;;) {
         const int it = (int)atomicAdd(p.work, 1u);
         const bool end = it >= T.items;
         const StItem w = st_decode(T, end ? 0 : it);
-        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1 + XTRA); ++pz, ++n) {
-          const unsigned s = n % L::NS, u = n / L::NS;
-          if (!mbar_wait(empty + s, (u & 1) ^ 1, p.pipe_error, 4)) return;
+        // (an L2 tensor prefetch running 3-10 planes ahead of the ring was measured: it costs 3-25 %)
+        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1 + XTRA); ++pz) {
+          if (!mbar_wait(empty + s, ph, p.pipe_error, 4)) return;
           meta[s] = end ? -1 : it;
           if (end) {
             mbar_arrive(full + s);
@@ -172,6 +177,7 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
           }
           mbar_expect_tx(full + s, L::BYTES);
           eh_issue_stage<L, EPS_ARR, SIG_ARR>(p, ring + s * L::STAGE, full + s, w.x0, w.y0, pz);
+          if (++s == (unsigned)L::NS) { s = 0; ph ^= 1u; }
         }
         if (end) break;
       }
@@ -184,28 +190,39 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
   const bool rim = FUSE && warp == SBY;
   const int t0 = (warp + 1) * EW + lane + 2;   // own staged position
   const int u0 = warp * EW + lane;             // own position in the E^{n+1} plane
-  unsigned n = 0;
+  // ring position of stage q-1 (sa) and its phase; advanced by hand (no division in the march)
+  unsigned sa = 0, pa = 0;
+  auto next = [](unsigned &st, unsigned &ph) { if (++st == (unsigned)L::NS) { st = 0; ph ^= 1u; } };
   for (;;) {
-    if (!mbar_wait(full + n % L::NS, (n / L::NS) & 1, p.pipe_error, 5)) return;
-    const int it = *(volatile int *)(meta + n % L::NS);
+    if (!mbar_wait(full + sa, pa, p.pipe_error, 5)) return;
+    const int it = *(volatile int *)(meta + sa);
     if (it < 0) break;
     const StItem w = st_decode(T, it);
     const int i = w.x0 + lane, j = w.y0 + warp;
     const bool valid = !rim && i < T.hi[0] && j < T.hi[1];
     const Column col = make_column(g, i, j);
+    // walls of this thread's edges, per column (the z part per plane below)
+    const bool wi = on_wall(g, 0, i), wj = on_wall(g, 1, j);
+    const bool wj_rim = on_wall(g, 1, w.y0 + SBY), wi_rimrow = on_wall(g, 0, w.x0 + lane);   // row y0 + SBY
+    const bool wi_rim = on_wall(g, 0, w.x0 + SW), wj_rimcol = on_wall(g, 1, w.y0 + lane);    // column x0 + SW
     int c = g.org + i + g.sy * j + g.sz * w.k0;
     double ex_p = 0.0, ey_p = 0.0, ez_p = 0.0;   // own E^{n+1} of the previous plane (FUSE)
-    for (int q = w.k0; q < w.k1 + XTRA; ++q, ++n) {
-      const double *A = ring + (n % L::NS) * L::STAGE;
-      const double *B = ring + ((n + 1) % L::NS) * L::STAGE;
-      if (!mbar_wait(full + (n + 1) % L::NS, ((n + 1) / L::NS) & 1, p.pipe_error, 6)) return;
-      double *N = enew + (FUSE ? (q % 3) * 3 * NSLOT_D : 0);
+    // E^{n+1} planes in shared memory: written this plane (Nw), read by the H update (Np = the one
+    // written last plane), and a third one in between so that one barrier per plane suffices
+    double *Np = enew, *Nw = enew + 3 * NSLOT_D, *Nx = enew + 6 * NSLOT_D;
+    for (int q = w.k0; q < w.k1 + XTRA; ++q) {
+      unsigned sb = sa, pb = pa;
+      next(sb, pb);
+      const double *A = ring + sa * L::STAGE;
+      const double *B = ring + sb * L::STAGE;
+      if (!mbar_wait(full + sb, pb, p.pipe_error, 6)) return;
+      const bool wk = on_wall(g, 2, q);
       double ex = 0.0, ey = 0.0, ez = 0.0;
       if (!rim) {
-        ex = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
-        ey = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
-        ez = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q);
-        if (FUSE) { N[u0] = ex; N[NSLOT_D + u0] = ey; N[2 * NSLOT_D + u0] = ez; }
+        ex = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wj || wk);
+        ey = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wk || wi);
+        ez = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wi || wj);
+        if (FUSE) { Nw[u0] = ex; Nw[NSLOT_D + u0] = ey; Nw[2 * NSLOT_D + u0] = ez; }
         if (valid && q < w.k1) {
           p.Eo[0][c] = ex;
           p.Eo[1][c] = ey;
@@ -219,13 +236,13 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
       } else {
         {  // row y0 + SBY: E_x, E_z at (x0 + lane, y0 + SBY)
           const int tr = (SBY + 1) * EW + lane + 2, ur = SBY * EW + lane;
-          N[ur] = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q);
-          N[2 * NSLOT_D + ur] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q);
+          Nw[ur] = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q, wj_rim || wk);
+          Nw[2 * NSLOT_D + ur] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q, wi_rimrow || wj_rim);
         }
         if (lane < SBY) {  // column x0 + SW: E_y, E_z at (x0 + SW, y0 + lane)
           const int tc = (lane + 1) * EW + SW + 2, uc = lane * EW + SW;
-          N[NSLOT_D + uc] = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q);
-          N[2 * NSLOT_D + uc] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q);
+          Nw[NSLOT_D + uc] = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wk || wi_rim);
+          Nw[2 * NSLOT_D + uc] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wi_rim || wj_rimcol);
         }
       }
       if (FUSE) {
@@ -234,12 +251,11 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
         // barriers ago: three rotating planes, one barrier per plane
         asm volatile("bar.sync 1, %0;" ::"n"(L::NCW * 32) : "memory");
         if (valid && q > w.k0) {
-          const double *P = enew + ((q - 1) % 3) * 3 * NSLOT_D;
           const int cm = c - g.sz;   // plane q-1
           // (curl E^{n+1})_D at the D-face of plane q-1: forward differences, as curl_e (kernels.cuh)
-          const double cx = (P[2 * NSLOT_D + u0 + EW] - ez_p) * g.rd[1] - (ey - ey_p) * g.rd[2];
-          const double cy = (ex - ex_p) * g.rd[2] - (P[2 * NSLOT_D + u0 + 1] - ez_p) * g.rd[0];
-          const double cz = (P[NSLOT_D + u0 + 1] - ey_p) * g.rd[0] - (P[u0 + EW] - ex_p) * g.rd[1];
+          const double cx = (Np[2 * NSLOT_D + u0 + EW] - ez_p) * g.rd[1] - (ey - ey_p) * g.rd[2];
+          const double cy = (ex - ex_p) * g.rd[2] - (Np[2 * NSLOT_D + u0 + 1] - ez_p) * g.rd[0];
+          const double cz = (Np[NSLOT_D + u0 + 1] - ey_p) * g.rd[0] - (Np[u0 + EW] - ex_p) * g.rd[1];
           const double hx = h_face_val(A[L::HH + t0], p.chm, cx, col.wall[0]);
           const double hy = h_face_val(A[L::HH + ESLOT + t0], p.chm, cy, col.wall[1]);
           const double hz = h_face_val(A[L::HH + 2 * ESLOT + t0], p.chm, cz, wall_k(g, q - 1));
@@ -253,13 +269,15 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
           }
         }
         ex_p = ex; ey_p = ey; ez_p = ez;
+        double *const tmp = Np; Np = Nw; Nw = Nx; Nx = tmp;   // rotate: written -> read, spare -> written
       }
       c += g.sz;
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty + n % L::NS);  // stage q-1 is done with
+      if (lane == 0) mbar_arrive(empty + sa);  // stage q-1 is done with
+      sa = sb; pa = pb;
     }
-    if (lane == 0) mbar_arrive(empty + n % L::NS);    // the item's last stage: the next item starts afresh
-    ++n;
+    if (lane == 0) mbar_arrive(empty + sa);    // the item's last stage: the next item starts afresh
+    next(sa, pa);
   }
 }
 

@@ -607,6 +607,16 @@ __global__ void __launch_bounds__(NTHREADS) k_canon(const __grid_constant__ Cano
 
 // ------------------------------------------------------------------ E update (eq. 11)
 
+// Coefficients of eq. 11 on an edge with permittivity eps and conductivity sig (the
+// four-cell means): km = sig/2 - eps/dt, rden = 1 / (sig/2 + eps/dt).  The division of eq. 11 is
+// taken as a multiplication by this reciprocal (reading A28): with uniform maps the host
+// evaluates the very same expressions once, so folding a uniform map changes no bit.
+struct ECoef { double km, rden; };
+__host__ __device__ __forceinline__ ECoef e_coef(double eps, double sig, double rdt) {
+  const double edt = eps * rdt, hs = 0.5 * sig;
+  return {hs - edt, 1.0 / (hs + edt)};
+}
+
 struct EArgs {
   GridP g;
   BoxP box;  // the cells this launch updates (the whole grid, or one region of it)
@@ -615,21 +625,21 @@ struct EArgs {
   const double *H[3];
   const double *eps_r, *sigma;  // cell-centred arrays or nullptr (uniform)
   double eps_u, sigma_u;        // uniform values (eps_u is eps0*eps_r)
+  double rdt;                   // 1 / dt
+  ECoef k_u;                    // e_coef(eps_u, sigma_u, rdt): the coefficients when both maps are uniform
   SourcesP src;
   const DevState *st;
 };
 
-// eq. 11 on a D-edge from its operands: eps, sig = the edge's four-cell means, J =
-// soft source term, e0 = E^n on the edge, (curl H)_D by backward differences: h2 - h2m along
-// d1 = D+1, h1 - h1m along d2 = D+2.  A wall-tangential edge stays 0.
-// Shared by k_e_update and k_eh_stage.
+// eq. 11 on a D-edge from its operands: k = the edge's coefficients, J = soft source term, e0 = E^n
+// on the edge, (curl H)_D by backward differences: h2 - h2m along d1 = D+1, h1 - h1m along
+// d2 = D+2.  A wall-tangential edge stays 0.  Shared by k_e_update and k_eh_stage.
 template <int D>
-__device__ __forceinline__ double e_edge_val(const GridP &g, double eps, double sig, double J, double e0,
+__device__ __forceinline__ double e_edge_val(const GridP &g, const ECoef &k, double J, double e0,
                                              double h2, double h2m, double h1, double h1m, bool wall) {
   constexpr int d1 = (D + 1) % 3, d2 = (D + 2) % 3;
   const double curl = (h2 - h2m) * g.rd[d1] - (h1 - h1m) * g.rd[d2];
-  const double edt = eps * (1.0 / g.dt), hs = 0.5 * sig;  // 1/dt is loop invariant: one division per edge
-  const double e1 = (curl - (hs - edt) * e0 - J) / (hs + edt);
+  const double e1 = (curl - k.km * e0 - J) * k.rden;
   return wall ? 0.0 : e1;
 }
 
@@ -647,7 +657,9 @@ __device__ __forceinline__ double e_edge(const EArgs &a, int c, bool wall, doubl
   if (SIG_ARR)
     sig = 0.25 * ((__ldg(a.sigma + c) + __ldg(a.sigma + c - s1)) +
                   (__ldg(a.sigma + c - s2) + __ldg(a.sigma + c - s1 - s2)));
-  return e_edge_val<D>(a.g, eps, sig, J, e0, h2, h2m, h1, h1m, wall);
+  ECoef k = a.k_u;
+  if (EPS_ARR || SIG_ARR) k = e_coef(eps, sig, a.rdt);
+  return e_edge_val<D>(a.g, k, J, e0, h2, h2m, h1, h1m, wall);
 }
 
 // everything the three edges of one cell read
