@@ -347,10 +347,17 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    local %= max(1, torch.cuda.device_count())      # more ranks than GPUs: share (smoke tests, gloo)
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        # NCCL over NVLink is the product path; FDTD_LLG_DIST_BACKEND=gloo carries the 8-byte words
+        # through the host instead (ranks sharing one GPU, where NCCL refuses to run)
+        backend = os.environ.get("FDTD_LLG_DIST_BACKEND", "nccl")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(backend)
 
     from paper_2103_12819_b200.replicas import barrier, max_over_ranks, whole_job_rate
 

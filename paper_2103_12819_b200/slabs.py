@@ -120,31 +120,52 @@ def cut_workload(w, plan: SlabPlan):
 
 
 def stack_copies(w, plan: SlabPlan):
-    """Weak-scaling input: the global grid is `world` identical copies of workload w stacked along
-    z (PAPER.md:209 grows its base case in z the same way), walls only at the global ends.  The
-    slab of rank r is one copy; its neighbours' adjacent planes are the copy's own last / first
-    plane."""
+    """Weak-scaling input: the global grid is `world` copies of workload w stacked along z
+    (PAPER.md:209 grows its base case in z the same way), walls only at the global ends.  The
+    material maps and the initial magnetisation of every second copy are MIRRORED in z, so that
+    like meets like at the interfaces (a magnet continues across one interface, vacuum across the
+    next): every rank then has the same sweep box, i.e. the same work.  The E and H arrays are the
+    copy's own everywhere (seeded noise or zero in the configs).  The slab of rank r is one copy;
+    its neighbours' adjacent planes are cut from the neighbouring copies."""
     import torch
     if plan.world == 1:
         return w
     if w.bc[2] == PERIODIC:
         raise ValueError("stack_copies: a periodic z axis has no ends to stack on")
 
-    def ext(t):
+    def copy_of(t, rank, mirrored_kind):
+        return t.flip(0) if (mirrored_kind and rank % 2 == 1) else t
+
+    def ext(t, mirrored_kind):
         if t is None or isinstance(t, (int, float)):
             return t
-        parts = ([t[-1:]] if plan.lo is not None else []) + [t] + ([t[:1]] if plan.hi is not None else [])
+        parts = [copy_of(t, plan.rank, mirrored_kind)]
+        if plan.lo is not None:
+            parts.insert(0, copy_of(t, plan.lo, mirrored_kind)[-1:])
+        if plan.hi is not None:
+            parts.append(copy_of(t, plan.hi, mirrored_kind)[:1])
         return torch.cat(parts, 0).contiguous()
 
     s = copy.copy(w)
     s.name = f"{w.name}[copy {plan.rank} of {plan.world} stacked in z]"
     s.slab_ext = plan.ext
-    s.materials = {k: ext(v) for k, v in w.materials.items()}
-    s.E = [ext(t) for t in w.E]
-    s.H = [ext(t) for t in w.H]
-    s.M_cell = [ext(t) for t in w.M_cell]
+    s.materials = {k: ext(v, True) for k, v in w.materials.items()}
+    s.E = [ext(t, False) for t in w.E]
+    s.H = [ext(t, False) for t in w.H]
+    s.M_cell = [ext(t, True) for t in w.M_cell]
+    if plan.rank % 2 == 1:      # the sources go with the structure
+        s.sources = []
+        for q in w.sources:
+            c = copy.copy(q)
+            c.lo = (q.lo[0], q.lo[1], w.nz - q.hi[2])
+            c.hi = (q.hi[0], q.hi[1], w.nz - q.lo[2])
+            if q.profile is not None:
+                c.profile = q.profile.flip(0).contiguous()
+            s.sources.append(c)
     if getattr(w, "pml", None) is not None:
         p = list(w.pml)
+        if plan.rank % 2 == 1:
+            p[4], p[5] = p[5], p[4]
         if plan.lo is not None:
             p[4] = 0
         if plan.hi is not None:

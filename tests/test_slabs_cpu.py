@@ -56,13 +56,24 @@ def test_cut_workload_carries_the_neighbours_planes_and_clips_sources(cfg, world
         assert all(s.materials["alpha"] == 0.01 for s in slabs)
 
 
-def test_stack_copies_uses_the_copys_own_end_planes():
+def test_stack_copies_mirrors_every_second_copy_so_that_like_meets_like():
     w = wl.make_config(5, shape=(10, 8, 12))
     plans = plan_slabs(3 * w.nz, 3, False)
-    mid = stack_copies(w, plans[1])
+    Ms = w.materials["Ms"]
+    low, mid, top = (stack_copies(w, p) for p in plans)
     assert mid.slab_ext == (1, 1) and mid.nz == w.nz
+    # copy 0 as it is (magnet in the lower half), copy 1 mirrored (magnet in the upper half), copy 2 as it is
+    assert torch.equal(low.materials["Ms"][:-1], Ms) and torch.equal(mid.materials["Ms"][1:-1], Ms.flip(0))
+    # interface 0|1: vacuum on both sides; interface 1|2: magnet on both sides
+    assert float(low.materials["Ms"][-2].max()) == 0.0 and float(low.materials["Ms"][-1].max()) == 0.0
+    assert float(mid.materials["Ms"][-2].min()) > 0.0 and float(mid.materials["Ms"][-1].min()) > 0.0
+    # the ghost planes are the neighbours' edge planes
+    assert torch.equal(low.materials["Ms"][-1], mid.materials["Ms"][1])
+    assert torch.equal(mid.materials["Ms"][0], low.materials["Ms"][-2])
+    assert torch.equal(mid.materials["Ms"][-1], top.materials["Ms"][1])
+    assert torch.equal(mid.M_cell[2][-1], top.M_cell[2][1]) and torch.equal(top.M_cell[2][0], mid.M_cell[2][-2])
+    # fields are the copy's own
     assert torch.equal(mid.E[0][0], w.E[0][-1]) and torch.equal(mid.E[0][-1], w.E[0][0])
-    assert torch.equal(mid.materials["Ms"][1:-1], w.materials["Ms"])
     assert stack_copies(w, plans[0]).E[0].shape[0] == w.nz + 1
 
 
