@@ -29,6 +29,7 @@ constexpr int NSLOT_D = round16(NROWS * EW); // columns x0 .. x0+32 (row pitch E
 
 template <bool FUSE, bool EPS_ARR, bool SIG_ARR>
 struct EhLayout {
+  static constexpr int SLOT = ESLOT;
   static constexpr int HH = 0;                          // H x, y, z
   static constexpr int EE = 3 * ESLOT;                  // E^n x, y, z
   static constexpr int EP = 6 * ESLOT;                  // eps_r
@@ -69,8 +70,8 @@ __device__ __forceinline__ void eh_issue_stage(const EHArgs &p, double *dst, uin
   const int x = PADL + x0 - 2, y = y0, z = pz + 1;   // tensor coordinates: one ghost layer in y, z
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    tma_load_4d(dst + L::HH + d * ESLOT, &p.map, bar, x, y, z, p.aH + d);
-    tma_load_4d(dst + L::EE + d * ESLOT, &p.map, bar, x, y, z, p.aE + d);
+    tma_load_4d(dst + L::HH + d * L::SLOT, &p.map, bar, x, y, z, p.aH + d);
+    tma_load_4d(dst + L::EE + d * L::SLOT, &p.map, bar, x, y, z, p.aE + d);
   }
   if (EPS_ARR) tma_load_4d(dst + L::EP, &p.map, bar, x, y, z, p.aEps);
   if (SIG_ARR) tma_load_4d(dst + L::SG, &p.map, bar, x, y, z, p.aSig);
@@ -102,7 +103,7 @@ __device__ __forceinline__ double eh_source(const EHArgs &a, int i, int j, int k
 template <class L, int D, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
 __device__ __forceinline__ double eh_edge(const EHArgs &a, const double *A, const double *B, int t, int i,
                                           int j, int k, bool wall) {
-  constexpr int HX = L::HH, HY = L::HH + ESLOT, HZ = L::HH + 2 * ESLOT;
+  constexpr int HX = L::HH, HY = L::HH + L::SLOT, HZ = L::HH + 2 * L::SLOT;
   // offsets of the two transverse neighbours: s1 = stride of axis D+1, s2 = stride of axis D+2
   double h2, h2m, h1, h1m, e0, m00 = 0, m10 = 0, m01 = 0, m11 = 0, g00 = 0, g10 = 0, g01 = 0, g11 = 0;
   if (D == 0) {         // s1 = y, s2 = z
@@ -112,12 +113,12 @@ __device__ __forceinline__ double eh_edge(const EHArgs &a, const double *A, cons
     if (SIG_ARR) { g00 = B[L::SG + t]; g10 = B[L::SG + t - EW]; g01 = A[L::SG + t]; g11 = A[L::SG + t - EW]; }
   } else if (D == 1) {  // s1 = z, s2 = x
     h2 = B[HX + t]; h2m = A[HX + t]; h1 = B[HZ + t]; h1m = B[HZ + t - 1];
-    e0 = B[L::EE + ESLOT + t];
+    e0 = B[L::EE + L::SLOT + t];
     if (EPS_ARR) { m00 = B[L::EP + t]; m10 = A[L::EP + t]; m01 = B[L::EP + t - 1]; m11 = A[L::EP + t - 1]; }
     if (SIG_ARR) { g00 = B[L::SG + t]; g10 = A[L::SG + t]; g01 = B[L::SG + t - 1]; g11 = A[L::SG + t - 1]; }
   } else {              // s1 = x, s2 = y
     h2 = B[HY + t]; h2m = B[HY + t - 1]; h1 = B[HX + t]; h1m = B[HX + t - EW];
-    e0 = B[L::EE + 2 * ESLOT + t];
+    e0 = B[L::EE + 2 * L::SLOT + t];
     if (EPS_ARR) { m00 = B[L::EP + t]; m10 = B[L::EP + t - 1]; m01 = B[L::EP + t - EW]; m11 = B[L::EP + t - EW - 1]; }
     if (SIG_ARR) { g00 = B[L::SG + t]; g10 = B[L::SG + t - 1]; g01 = B[L::SG + t - EW]; g11 = B[L::SG + t - EW - 1]; }
   }
@@ -278,6 +279,242 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
     }
     if (lane == 0) mbar_arrive(empty + sa);    // the item's last stage: the next item starts afresh
     next(sa, pa);
+  }
+}
+
+// ------------------------------------------------------------------ the fused sweep, warp-specialised
+// k_eh_stage<FUSE> above does the E phase and the H phase of a plane in the SAME 16 + 1 warps, in
+// lockstep with one block barrier per plane: 18 warps per SM, each carrying ~375 instructions per
+// plane, wait on fixed latencies more than they issue (ncu: issue slots 52 % busy, DRAM 73 %).
+// k_eh_fused gives the two phases to two sets of warps: 16 + 1 E warps compute E^{n+1}(q) into one
+// of three rotating planes in shared memory and store it; 16 H warps take H(q-1) from E^{n+1}(q-1)
+// and E^{n+1}(q).  The sets are coupled by two rings of mbarriers (efull / eempty per plane) instead
+// of a block barrier, so the E warps run up to two planes ahead; 34 warps per SM.  Same arithmetic,
+// same bits.
+// A block has at most 32 warps: 15 tile rows (15 + 1 E warps, 15 H warps, the producer).
+constexpr int FBY = 15;
+constexpr int FROWS = FBY + 2;                // staged rows y0-1 .. y0+15
+constexpr int FSLOT = round16(FROWS * EW);    // doubles per staged array
+constexpr int FNSLOT = round16((FBY + 1) * EW);   // E^{n+1} plane: rows y0 .. y0+15, columns x0 .. x0+32
+
+template <bool EPS_ARR, bool SIG_ARR>
+struct EfStage {   // one stage of the ring (as EhLayout, 17 rows)
+  static constexpr int SLOT = FSLOT;
+  static constexpr int HH = 0;
+  static constexpr int EE = 3 * FSLOT;
+  static constexpr int EP = 6 * FSLOT;
+  static constexpr int SG = (6 + (EPS_ARR ? 1 : 0)) * FSLOT;
+  static constexpr int NARR = 6 + (EPS_ARR ? 1 : 0) + (SIG_ARR ? 1 : 0);
+  static constexpr int STAGE = NARR * FSLOT;
+  static constexpr unsigned BYTES = 8u * NARR * FROWS * EW;
+};
+
+template <bool EPS_ARR, bool SIG_ARR>
+struct EfLayout {
+  using S = EfStage<EPS_ARR, SIG_ARR>;          // stage layout and byte counts
+  static constexpr int NEB = 3;                 // rotating E^{n+1} planes
+  static constexpr int ENEW = NEB * 3 * FNSLOT;
+  static constexpr int BUDGET = 220 * 1024 - 8 * ENEW;
+  static constexpr int NS_FIT = BUDGET / (8 * S::STAGE);
+  static constexpr int NS = NS_FIT > 6 ? 6 : NS_FIT;
+  static constexpr int NEW_ = FBY + 1;          // E warps: the tile rows + the rim
+  static constexpr int NHW = FBY;               // H warps
+  static constexpr int NCW = NEW_ + NHW;        // warps that release a stage
+  static constexpr int NTHREADS = (NCW + 1) * 32;
+  static constexpr size_t SMEM_BYTES = 128 + 8 * (size_t)(NS * S::STAGE + ENEW) + 8 * (2 * NS + 2 * NEB) + 4 * NS;
+  static_assert(NS >= 3, "ring too shallow");
+};
+
+template <bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
+__global__ void __launch_bounds__(EfLayout<EPS_ARR, SIG_ARR>::NTHREADS, 1)
+k_eh_fused(const __grid_constant__ EHArgs p) {
+  using L = EfLayout<EPS_ARR, SIG_ARR>;
+  using S = typename L::S;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  double *const ring = reinterpret_cast<double *>(smem_raw);
+  double *const enew = ring + L::NS * S::STAGE;
+  uint64_t *const full = reinterpret_cast<uint64_t *>(enew + L::ENEW);
+  uint64_t *const empty = full + L::NS;
+  uint64_t *const efull = empty + L::NS;     // E^{n+1} plane b is complete (17 E warps arrive)
+  uint64_t *const eempty = efull + L::NEB;   // ... is no longer read (16 H warps arrive)
+  int *const meta = reinterpret_cast<int *>(eempty + L::NEB);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < L::NS; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, L::NCW); }
+    for (int b = 0; b < L::NEB; ++b) { mbar_init(efull + b, L::NEW_); mbar_init(eempty + b, L::NHW); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  const StBox &T = p.tb;
+  const GridP &g = p.g;
+  auto next = [](unsigned &st, unsigned &ph) { if (++st == (unsigned)L::NS) { st = 0; ph ^= 1u; } };
+  auto nextb = [](unsigned &b, unsigned &ph) { if (++b == (unsigned)L::NEB) { b = 0; ph ^= 1u; } };
+
+  if (warp == L::NCW) {
+    // ===== producer: stages k0-1 .. k1 of every item it draws
+    if (lane == 0) {
+      tma_prefetch_desc(&p.map);
+      unsigned s = 0, ph = 1;
+      for (;;) {
+        const int it = (int)atomicAdd(p.work, 1u);
+        const bool end = it >= T.items;
+        const StItem w = st_decode_by(T, end ? 0 : it, FBY);
+        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1 + 1); ++pz) {
+          if (!mbar_wait(empty + s, ph, p.pipe_error, 7)) return;
+          meta[s] = end ? -1 : it;
+          if (end) {
+            mbar_arrive(full + s);
+            break;
+          }
+          mbar_expect_tx(full + s, S::BYTES);
+          eh_issue_stage<S, EPS_ARR, SIG_ARR>(p, ring + s * S::STAGE, full + s, w.x0, w.y0, pz);
+          next(s, ph);
+        }
+        if (end) break;
+      }
+    }
+    return;
+  }
+
+  if (warp < L::NEW_) {
+    // ===== E warps.  warp < FBY: tile row, lane = x.  warp == FBY: the rim of the E^{n+1} plane on
+    // the high side: row y0 + FBY (E_x, E_z) and column x0 + SW (E_y, E_z)
+    const bool rim = warp == FBY;
+    const int t0 = (warp + 1) * EW + lane + 2;   // own staged position
+    const int u0 = warp * EW + lane;             // own position in the E^{n+1} plane
+    double *const eo0 = p.Eo[0], *const eo1 = p.Eo[1], *const eo2 = p.Eo[2];
+    unsigned sa = 0, pa = 0;     // ring position of stage q-1
+    unsigned eb = 0, ep = 1;     // E^{n+1} plane written next, the parity its eempty barrier is waited on
+    for (;;) {
+      if (!mbar_wait(full + sa, pa, p.pipe_error, 8)) return;
+      const int it = *(volatile int *)(meta + sa);
+      if (it < 0) break;
+      const StItem w = st_decode_by(T, it, FBY);
+      const int i = w.x0 + lane, j = w.y0 + warp;
+      const bool valid = !rim && i < T.hi[0] && j < T.hi[1];
+      const Column col = make_column(g, i, j);
+      const bool wi = on_wall(g, 0, i), wj = on_wall(g, 1, j);
+      const bool wj_rim = on_wall(g, 1, w.y0 + FBY), wi_rimrow = on_wall(g, 0, w.x0 + lane);
+      const bool wi_rim = on_wall(g, 0, w.x0 + SW), wj_rimcol = on_wall(g, 1, w.y0 + lane);
+      int c = g.org + i + g.sy * j + g.sz * w.k0;
+      for (int q = w.k0; q <= w.k1; ++q) {
+        unsigned sb = sa, pb = pa;
+        next(sb, pb);
+        const double *A = ring + sa * S::STAGE;
+        const double *B = ring + sb * S::STAGE;
+        if (!mbar_wait(full + sb, pb, p.pipe_error, 9)) return;
+        if (!mbar_wait(eempty + eb, ep, p.pipe_error, 10)) return;   // the H warps are done with this plane
+        double *const N = enew + eb * (3 * FNSLOT);
+        const bool wk = on_wall(g, 2, q);
+        if (!rim) {
+          const double ex = eh_edge<S, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wj || wk);
+          const double ey = eh_edge<S, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wk || wi);
+          const double ez = eh_edge<S, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wi || wj);
+          N[u0] = ex; N[FNSLOT + u0] = ey; N[2 * FNSLOT + u0] = ez;
+          if (valid && q < w.k1) {
+            eo0[c] = ex;
+            eo1[c] = ey;
+            eo2[c] = ez;
+            if (col.edge_ij || edge_k(g, q)) {
+              store_images_inl<exp_of_e<0>()>(eo0, g, i, j, q, c, ex);
+              store_images_inl<exp_of_e<1>()>(eo1, g, i, j, q, c, ey);
+              store_images_inl<exp_of_e<2>()>(eo2, g, i, j, q, c, ez);
+            }
+          }
+        } else {
+          {  // row y0 + FBY: E_x, E_z at (x0 + lane, y0 + FBY)
+            const int tr = (FBY + 1) * EW + lane + 2, ur = FBY * EW + lane;
+            N[ur] = eh_edge<S, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + FBY, q, wj_rim || wk);
+            N[2 * FNSLOT + ur] = eh_edge<S, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + FBY, q, wi_rimrow || wj_rim);
+          }
+          if (lane < FBY) {  // column x0 + SW: E_y, E_z at (x0 + SW, y0 + lane)
+            const int tc = (lane + 1) * EW + SW + 2, uc = lane * EW + SW;
+            N[FNSLOT + uc] = eh_edge<S, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wk || wi_rim);
+            N[2 * FNSLOT + uc] = eh_edge<S, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wi_rim || wj_rimcol);
+          }
+        }
+        c += g.sz;
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(efull + eb);   // this warp's part of E^{n+1}(q) is in shared memory
+          mbar_arrive(empty + sa);   // stage q-1 is done with (on the E side)
+        }
+        sa = sb; pa = pb;
+        nextb(eb, ep);
+      }
+      if (lane == 0) mbar_arrive(empty + sa);    // the item's last stage
+      next(sa, pa);
+    }
+    return;
+  }
+
+  // ===== H warps: tile row warp - NEW_, lane = x; H(h) for h = k0 .. k1-1 from E^{n+1}(h), E^{n+1}(h+1)
+  {
+    const int row = warp - L::NEW_;
+    const int t0 = (row + 1) * EW + lane + 2;
+    const int u0 = row * EW + lane;
+    double *const ho0 = p.Ho[0], *const ho1 = p.Ho[1], *const ho2 = p.Ho[2];
+    const double chm = p.chm, rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
+    unsigned sh = 0, ph = 0;     // ring position of the stage looked at next
+    unsigned hb = 0, hp = 0;     // E^{n+1} plane h and the parity its efull barrier is waited on
+    for (;;) {
+      if (!mbar_wait(full + sh, ph, p.pipe_error, 11)) return;
+      const int it = *(volatile int *)(meta + sh);
+      if (it < 0) break;
+      const StItem w = st_decode_by(T, it, FBY);
+      const int i = w.x0 + lane, j = w.y0 + row;
+      const bool valid = i < T.hi[0] && j < T.hi[1];
+      const Column col = make_column(g, i, j);
+      int c = g.org + i + g.sy * j + g.sz * w.k0;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + sh);    // stage k0-1 holds nothing an H face reads
+      next(sh, ph);
+      if (!mbar_wait(efull + hb, hp, p.pipe_error, 12)) return;   // E^{n+1}(k0)
+      for (int h = w.k0; h < w.k1; ++h) {
+        const double *A = ring + sh * S::STAGE;   // stage h: this face's own H
+        if (!mbar_wait(full + sh, ph, p.pipe_error, 13)) return;
+        unsigned nb = hb, np = hp;
+        nextb(nb, np);
+        if (!mbar_wait(efull + nb, np, p.pipe_error, 14)) return;  // E^{n+1}(h+1)
+        if (valid) {
+          const double *P = enew + hb * (3 * FNSLOT), *Q = enew + nb * (3 * FNSLOT);
+          const double ex_h = P[u0], ey_h = P[FNSLOT + u0], ez_h = P[2 * FNSLOT + u0];
+          // (curl E^{n+1})_D at the D-face of plane h: forward differences, as curl_e (kernels.cuh)
+          const double cx = (P[2 * FNSLOT + u0 + EW] - ez_h) * rdy - (Q[FNSLOT + u0] - ey_h) * rdz;
+          const double cy = (Q[u0] - ex_h) * rdz - (P[2 * FNSLOT + u0 + 1] - ez_h) * rdx;
+          const double cz = (P[FNSLOT + u0 + 1] - ey_h) * rdx - (P[u0 + EW] - ex_h) * rdy;
+          const double hx = h_face_val(A[S::HH + t0], chm, cx, col.wall[0]);
+          const double hy = h_face_val(A[S::HH + FSLOT + t0], chm, cy, col.wall[1]);
+          const double hz = h_face_val(A[S::HH + 2 * FSLOT + t0], chm, cz, wall_k(g, h));
+          ho0[c] = hx;
+          ho1[c] = hy;
+          ho2[c] = hz;
+          if (col.edge_ij || edge_k(g, h)) {
+            store_images_inl<exp_of_h<0>()>(ho0, g, i, j, h, c, hx);
+            store_images_inl<exp_of_h<1>()>(ho1, g, i, j, h, c, hy);
+            store_images_inl<exp_of_h<2>()>(ho2, g, i, j, h, c, hz);
+          }
+        }
+        c += g.sz;
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(eempty + hb);  // E^{n+1}(h) is done with
+          mbar_arrive(empty + sh);   // stage h is done with (on the H side)
+        }
+        next(sh, ph);
+        hb = nb; hp = np;
+      }
+      // E^{n+1}(k1) was read as the plane above the item's last faces; stage k1 holds nothing an H
+      // face of this item reads (it was filled: the E warps waited for it before they wrote that plane)
+      if (lane == 0) {
+        mbar_arrive(eempty + hb);
+        mbar_arrive(empty + sh);
+      }
+      next(sh, ph);
+      nextb(hb, hp);
+    }
   }
 }
 

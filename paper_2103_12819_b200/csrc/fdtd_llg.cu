@@ -70,7 +70,7 @@ struct fdtd_llg {
   CUtensorMap mapT{}, mapPM{};
   // staged Maxwell sweeps (eh_stage.cuh): the E update, fused with the merged H update outside the box
   bool eh_ok = false;        // tensor map built, kernels configured (no PML, kernel_path != 1)
-  CUtensorMap mapEH{};
+  CUtensorMap mapEH{}, mapEF{};   // boxes of k_eh_stage (18 rows) and of k_eh_fused (17 rows)
   unsigned *work_eh = nullptr;  // [8] item counters, one per staged launch of a step
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
@@ -503,13 +503,18 @@ int setup_hm_stage(fdtd_llg *s) {
 
 // Work items of a staged Maxwell sweep.  Long items amortise the two extra planes a fused item
 // stages (k0-1 and k1) and its cold start; short ones balance the SMs when the region has few
-// tiles and keep the blocks that run together on the same few planes.  Measured: 256^3 is fastest
-// at 16 planes (4.3 TB/s; 4.0 at 32, 3.5 at 64), 384^3 at 32-64 (5.1-5.2 TB/s; 4.9 at 16), the
-// upper half of 768^3 at 32 (4.5 TB/s; 4.1 at 64): the longest of 32, 16, 8 planes that still
-// gives every SM ten items.
-StBox make_ehbox(const fdtd_llg *s, const int lo[3], const int hi[3]) {
-  StBox b = make_stbox(lo, hi, SBY, 32);
-  for (int kz = 16; kz >= 8 && b.items < 10 * s->num_sms; kz /= 2) b = make_stbox(lo, hi, SBY, kz);
+// tiles and keep the blocks that run together on the same few planes.  Measured (k_eh_fused):
+// 256^3 4.7-4.9 TB/s at 8-24 planes, 4.4 at 32, 3.8 at 64; 512x128x128 (two material arrays) 3.8 at
+// 8, 4.0 at 12-24; 384^3 4.7 at 8, 5.0 at 12-16, 5.2-5.3 at 24-32: the longest of 32, 24, 16, 12
+// planes that still gives every SM eight items.
+StBox make_ehbox(const fdtd_llg *s, const int lo[3], const int hi[3], bool fuse) {
+  const int by = fuse ? FBY : SBY;   // tile rows of k_eh_fused / k_eh_stage
+  const int cand[4] = {32, 24, 16, 12};
+  StBox b{};
+  for (int q = 0; q < 4; ++q) {
+    b = make_stbox(lo, hi, by, cand[q]);
+    if (b.items >= 8 * s->num_sms) break;
+  }
   return b;
 }
 
@@ -521,8 +526,13 @@ int launch_eh_stage(fdtd_llg *s, const EHArgs &p) {
   const int grid = std::max(1, std::min(p.tb.items, s->num_sms));   // one persistent block per SM
 #define EK(EA, SA, HS)                                                                          \
   if (ea == EA && sa == SA && hs == HS) {                                                       \
-    using L = EhLayout<FUSE, EA, SA>;                                                           \
-    k_eh_stage<FUSE, EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);           \
+    if (FUSE) {                                                                                 \
+      using L = EfLayout<EA, SA>;                                                               \
+      k_eh_fused<EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);               \
+    } else {                                                                                    \
+      using L = EhLayout<false, EA, SA>;                                                        \
+      k_eh_stage<false, EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);        \
+    }                                                                                           \
     return FDTD_LLG_OK;                                                                         \
   }
   EK(false, false, false) EK(false, false, true) EK(false, true, false) EK(false, true, true)
@@ -532,18 +542,19 @@ int launch_eh_stage(fdtd_llg *s, const EHArgs &p) {
 }
 
 int setup_eh_stage(fdtd_llg *s) {
-#define SA(FUSE, EA, SA_, HS)                                                                   \
-  CU(s, cudaFuncSetAttribute(k_eh_stage<FUSE, EA, SA_, HS>,                                     \
+#define SA(EA, SA_, HS)                                                                         \
+  CU(s, cudaFuncSetAttribute(k_eh_stage<false, EA, SA_, HS>,                                    \
                              cudaFuncAttributeMaxDynamicSharedMemorySize,                       \
-                             (int)EhLayout<FUSE, EA, SA_>::SMEM_BYTES));
-#define SA8(FUSE) SA(FUSE, false, false, false) SA(FUSE, false, false, true) SA(FUSE, false, true, false) \
-  SA(FUSE, false, true, true) SA(FUSE, true, false, false) SA(FUSE, true, false, true)          \
-  SA(FUSE, true, true, false) SA(FUSE, true, true, true)
-  SA8(false) SA8(true)
-#undef SA8
+                             (int)EhLayout<false, EA, SA_>::SMEM_BYTES));                       \
+  CU(s, cudaFuncSetAttribute(k_eh_fused<EA, SA_, HS>,                                           \
+                             cudaFuncAttributeMaxDynamicSharedMemorySize,                       \
+                             (int)EfLayout<EA, SA_>::SMEM_BYTES));
+  SA(false, false, false) SA(false, false, true) SA(false, true, false) SA(false, true, true)
+  SA(true, false, false) SA(true, false, true) SA(true, true, false) SA(true, true, true)
 #undef SA
   int rc = make_map(s, &s->mapEH, EW, EROWS, 1);
   if (rc) return rc;
+  if ((rc = make_map(s, &s->mapEF, EW, FROWS, 1))) return rc;
   s->eh_ok = true;
   return FDTD_LLG_OK;
 }
@@ -959,12 +970,12 @@ int plan_e_regions(const fdtd_llg *s, ERegion *out) {
         if (hi[2] <= B.lo[2]) continue;
       }
       n = put(n, B.lo, hi, st, st && can_fuse);
-      if (st) items += make_ehbox(s, B.lo, hi).items;
+      if (st) items += make_ehbox(s, B.lo, hi, st && can_fuse).items;
     }
     if (s->llg) {
       const bool st = (s->lo[0] & 1) == 0;
       n = put(n, s->lo, s->hi, st, false);
-      if (st) items += make_ehbox(s, s->lo, s->hi).items;
+      if (st) items += make_ehbox(s, s->lo, s->hi, false).items;
     }
   }
   // a grid that cannot give every SM an item is latency bound: one direct-load launch serves it better
@@ -984,8 +995,8 @@ int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int 
     }
     EHArgs p{};
     p.g = s->g;
-    p.tb = make_ehbox(s, reg[r].lo, reg[r].hi);
-    p.map = s->mapEH;
+    p.tb = make_ehbox(s, reg[r].lo, reg[r].hi, reg[r].fuse);
+    p.map = reg[r].fuse ? s->mapEF : s->mapEH;
     p.aE = array_index(s, Ein[0]);
     p.aH = array_index(s, s->Hset[hset][0]);
     p.aEps = s->eps_r.is_array ? array_index(s, s->eps_r.dev) : 0;

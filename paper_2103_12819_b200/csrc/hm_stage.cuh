@@ -211,6 +211,15 @@ __device__ __forceinline__ void s_issue_stage(const HMSArgs &p, double *dst, uin
 struct StItem {
   int x0, y0, k0, k1;
 };
+__device__ __forceinline__ StItem st_decode_by(const StBox &T, int it, int by) {
+  const int tx = it % T.ntx, q = it / T.ntx, ty = q % T.nty, tz = q / T.nty;
+  StItem w;
+  w.x0 = T.lo[0] + tx * SW;
+  w.y0 = T.lo[1] + ty * by;
+  w.k0 = T.lo[2] + tz * T.kz;
+  w.k1 = min(w.k0 + T.kz, T.hi[2]);
+  return w;
+}
 __device__ __forceinline__ StItem st_decode(const StBox &T, int it) {
   const int tx = it % T.ntx, q = it / T.ntx, ty = q % T.nty, tz = q / T.nty;
   StItem w;
