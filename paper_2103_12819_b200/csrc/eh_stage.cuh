@@ -1,21 +1,22 @@
-// eh_stage.cuh -- the staged Maxwell sweep: eq. 11 and, FUSED with it on the
+// eh_stage.cuh -- the staged Maxwell sweeps: eq. 11 and, FUSED with it on the
 // faces no magnetic face reads, the H update that follows it (eq. 21 with M = 0).
 //
 // Same arithmetic as k_e_update / k_h_update (kernels.cuh: e_edge_val, h_face_val); what differs is
-// how operands reach it and how often memory is touched.  A persistent block owns a tile of
-// SW x SBY columns and marches in z; THREAD = CELL (its three edges and three faces), warp = tile
-// row, lane = x.  One producer warp stages, per plane, a (SW+4) x (SBY+2) box of every operand
-// array (H^{n+1/2} x3, E^n x3, eps_r, sigma) in shared memory with cp.async.bulk.tensor, in a
-// ring of NS stages under full / empty mbarriers; plane q is computed from stages q-1 and q.
+// how operands reach it and how often memory is touched.  A persistent block owns a tile of columns
+// and marches in z; THREAD = CELL, warp = tile row, lane = x.  One producer lane stages, per plane,
+// a (SW+4) x (rows+2) box of every operand array (H^{n+1/2} x3, E^n x3, eps_r, sigma) in shared
+// memory with cp.async.bulk.tensor, in a ring of NS stages under full / empty mbarriers; plane q is
+// computed from stages q-1 and q.
 //
-// FUSE (merged H half-steps, options.merge_h): outside the LLG sweep box the H update that follows
-// the E update -- second half-step of this step and first of the next, both with curl E^{n+1}
-// -- reads nothing but E^{n+1} around the face and its own H.  The block therefore
-// keeps the E^{n+1} plane it just computed in shared memory (with the one-cell rim on the high
-// side, computed by an extra warp) and takes H^{n+1/2} -> H^{n+3/2} in the same pass: per cell and
-// step E 3 + H 3 read, E 3 + H 3 written = 12 words instead of 9 + 9 (and 27 with two half-steps).
-// All inputs are time-n sets that nobody writes during the pass (every update is out of place),
-// so tiles and planes can be visited in any order.
+//   k_eh_stage  E only, tile 32 x 16: the LLG sweep box, whose H lives at integer time.
+//   k_eh_fused  E + H, tile 32 x 15 (merged H half-steps, options.merge_h): outside the sweep box
+//     the H update that follows the E update -- second half-step of this step and first of the
+//     next, both with curl E^{n+1} -- reads nothing but E^{n+1} around the face and
+//     its own H.  The block keeps the E^{n+1} plane it just computed in shared memory (with the
+//     one-cell rim on the high side) and takes H^{n+1/2} -> H^{n+3/2} in the same pass: per cell
+//     and step E 3 + H 3 read, E 3 + H 3 written = 12 words instead of 9 + 9 (27 with two
+//     half-steps).  All inputs are sets nobody writes during the pass (every update is out of
+//     place), so tiles and planes can be visited in any order.
 #pragma once
 #include "hm_stage.cuh"
 
@@ -24,11 +25,9 @@ namespace fl {
 constexpr int EW = SW + 4;                   // staged row: x0-2 .. x0+33 (16-byte multiples)
 constexpr int EROWS = SBY + 2;               // rows y0-1 .. y0+16
 constexpr int ESLOT = round16(EROWS * EW);   // doubles per staged array
-constexpr int NROWS = SBY + 1;               // E^{n+1} plane kept for the H update: rows y0 .. y0+16,
-constexpr int NSLOT_D = round16(NROWS * EW); // columns x0 .. x0+32 (row pitch EW)
 
-template <bool FUSE, bool EPS_ARR, bool SIG_ARR>
-struct EhLayout {
+template <bool EPS_ARR, bool SIG_ARR>
+struct EhLayout {   // k_eh_stage: one stage of the ring, the ring, the block
   static constexpr int SLOT = ESLOT;
   static constexpr int HH = 0;                          // H x, y, z
   static constexpr int EE = 3 * ESLOT;                  // E^n x, y, z
@@ -37,13 +36,11 @@ struct EhLayout {
   static constexpr int NARR = 6 + (EPS_ARR ? 1 : 0) + (SIG_ARR ? 1 : 0);
   static constexpr int STAGE = NARR * ESLOT;
   static constexpr unsigned BYTES = 8u * NARR * EROWS * EW;    // bytes the TMA writes per stage
-  static constexpr int ENEW = FUSE ? 3 * 3 * NSLOT_D : 0;      // three rotating planes of E^{n+1} x, y, z
-  static constexpr int BUDGET = 220 * 1024 - 8 * ENEW;
-  static constexpr int NS_FIT = BUDGET / (8 * STAGE);
+  static constexpr int NS_FIT = 220 * 1024 / (8 * STAGE);
   static constexpr int NS = NS_FIT > 6 ? 6 : NS_FIT;
-  static constexpr int NCW = SBY + (FUSE ? 1 : 0);      // compute warps (+1: the rim of E^{n+1})
+  static constexpr int NCW = SBY;                       // compute warps
   static constexpr int NTHREADS = (NCW + 1) * 32;
-  static constexpr size_t SMEM_BYTES = 128 + 8 * (size_t)(NS * STAGE + ENEW) + 8 * (2 * NS) + 4 * NS;
+  static constexpr size_t SMEM_BYTES = 128 + 8 * (size_t)(NS * STAGE) + 8 * (2 * NS) + 4 * NS;
   static_assert(NS >= 3, "ring too shallow");
 };
 
@@ -137,14 +134,14 @@ __device__ __forceinline__ bool on_wall(const GridP &g, int d, int idx) {
   return (g.wall[d] && idx == 0) || (g.wallhi[d] && idx == g.n[d]);
 }
 
-template <bool FUSE, bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
-__global__ void __launch_bounds__(EhLayout<FUSE, EPS_ARR, SIG_ARR>::NTHREADS, 1)
+// ------------------------------------------------------------------ E only (the LLG sweep box)
+template <bool EPS_ARR, bool SIG_ARR, bool HAS_SRC>
+__global__ void __launch_bounds__(EhLayout<EPS_ARR, SIG_ARR>::NTHREADS, 1)
 k_eh_stage(const __grid_constant__ EHArgs p) {
-  using L = EhLayout<FUSE, EPS_ARR, SIG_ARR>;
+  using L = EhLayout<EPS_ARR, SIG_ARR>;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   double *const ring = reinterpret_cast<double *>(smem_raw);
-  double *const enew = ring + L::NS * L::STAGE;                 // FUSE: 3 planes x 3 components
-  uint64_t *const full = reinterpret_cast<uint64_t *>(enew + L::ENEW);
+  uint64_t *const full = reinterpret_cast<uint64_t *>(ring + L::NS * L::STAGE);
   uint64_t *const empty = full + L::NS;
   int *const meta = reinterpret_cast<int *>(empty + L::NS);
 
@@ -157,10 +154,9 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
 
   const StBox &T = p.tb;
   const GridP &g = p.g;
-  // planes staged per item: q = k0-1 .. k1-1, and k1 too when the H update needs E^{n+1}(k1)
-  constexpr int XTRA = FUSE ? 1 : 0;
+  auto next = [](unsigned &st, unsigned &ph) { if (++st == (unsigned)L::NS) { st = 0; ph ^= 1u; } };
   if (warp == L::NCW) {
-    // ===== producer
+    // ===== producer: stages k0-1 .. k1-1 of every item it draws
     if (lane == 0) {
       tma_prefetch_desc(&p.map);
       unsigned s = 0, ph = 1;   // ring position and the parity its empty barrier is waited on
@@ -169,7 +165,7 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
         const bool end = it >= T.items;
         const StItem w = st_decode(T, end ? 0 : it);
         // (an L2 tensor prefetch running 3-10 planes ahead of the ring was measured: it costs 3-25 %)
-        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1 + XTRA); ++pz) {
+        for (int pz = w.k0 - 1; pz < (end ? w.k0 : w.k1); ++pz) {
           if (!mbar_wait(empty + s, ph, p.pipe_error, 4)) return;
           meta[s] = end ? -1 : it;
           if (end) {
@@ -178,99 +174,46 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
           }
           mbar_expect_tx(full + s, L::BYTES);
           eh_issue_stage<L, EPS_ARR, SIG_ARR>(p, ring + s * L::STAGE, full + s, w.x0, w.y0, pz);
-          if (++s == (unsigned)L::NS) { s = 0; ph ^= 1u; }
+          next(s, ph);
         }
         if (end) break;
       }
     }
     return;
   }
-  // ===== compute warps.  warp < SBY: tile row `warp`, lane = x, thread = cell.  warp == SBY (FUSE):
-  // the rim of the E^{n+1} plane the H update reads on the high side: row y0 + SBY (E_x, E_z) and
-  // column x0 + SW (E_y, E_z)
-  const bool rim = FUSE && warp == SBY;
+  // ===== compute warps: warp = tile row, lane = x, thread = cell
   const int t0 = (warp + 1) * EW + lane + 2;   // own staged position
-  const int u0 = warp * EW + lane;             // own position in the E^{n+1} plane
-  // ring position of stage q-1 (sa) and its phase; advanced by hand (no division in the march)
-  unsigned sa = 0, pa = 0;
-  auto next = [](unsigned &st, unsigned &ph) { if (++st == (unsigned)L::NS) { st = 0; ph ^= 1u; } };
+  double *const eo0 = p.Eo[0], *const eo1 = p.Eo[1], *const eo2 = p.Eo[2];
+  unsigned sa = 0, pa = 0;   // ring position of stage q-1 and its phase (advanced by hand: no division in the march)
   for (;;) {
     if (!mbar_wait(full + sa, pa, p.pipe_error, 5)) return;
     const int it = *(volatile int *)(meta + sa);
     if (it < 0) break;
     const StItem w = st_decode(T, it);
     const int i = w.x0 + lane, j = w.y0 + warp;
-    const bool valid = !rim && i < T.hi[0] && j < T.hi[1];
+    const bool valid = i < T.hi[0] && j < T.hi[1];
     const Column col = make_column(g, i, j);
-    // walls of this thread's edges, per column (the z part per plane below)
-    const bool wi = on_wall(g, 0, i), wj = on_wall(g, 1, j);
-    const bool wj_rim = on_wall(g, 1, w.y0 + SBY), wi_rimrow = on_wall(g, 0, w.x0 + lane);   // row y0 + SBY
-    const bool wi_rim = on_wall(g, 0, w.x0 + SW), wj_rimcol = on_wall(g, 1, w.y0 + lane);    // column x0 + SW
+    const bool wi = on_wall(g, 0, i), wj = on_wall(g, 1, j);   // walls of this thread's edges, per column
     int c = g.org + i + g.sy * j + g.sz * w.k0;
-    double ex_p = 0.0, ey_p = 0.0, ez_p = 0.0;   // own E^{n+1} of the previous plane (FUSE)
-    // E^{n+1} planes in shared memory: written this plane (Nw), read by the H update (Np = the one
-    // written last plane), and a third one in between so that one barrier per plane suffices
-    double *Np = enew, *Nw = enew + 3 * NSLOT_D, *Nx = enew + 6 * NSLOT_D;
-    for (int q = w.k0; q < w.k1 + XTRA; ++q) {
+    for (int q = w.k0; q < w.k1; ++q) {
       unsigned sb = sa, pb = pa;
       next(sb, pb);
       const double *A = ring + sa * L::STAGE;
       const double *B = ring + sb * L::STAGE;
       if (!mbar_wait(full + sb, pb, p.pipe_error, 6)) return;
       const bool wk = on_wall(g, 2, q);
-      double ex = 0.0, ey = 0.0, ez = 0.0;
-      if (!rim) {
-        ex = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wj || wk);
-        ey = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wk || wi);
-        ez = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wi || wj);
-        if (FUSE) { Nw[u0] = ex; Nw[NSLOT_D + u0] = ey; Nw[2 * NSLOT_D + u0] = ez; }
-        if (valid && q < w.k1) {
-          p.Eo[0][c] = ex;
-          p.Eo[1][c] = ey;
-          p.Eo[2][c] = ez;
-          if (col.edge_ij || edge_k(g, q)) {
-            store_images_inl<exp_of_e<0>()>(p.Eo[0], g, i, j, q, c, ex);
-            store_images_inl<exp_of_e<1>()>(p.Eo[1], g, i, j, q, c, ey);
-            store_images_inl<exp_of_e<2>()>(p.Eo[2], g, i, j, q, c, ez);
-          }
+      const double ex = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wj || wk);
+      const double ey = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wk || wi);
+      const double ez = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, t0, i, j, q, wi || wj);
+      if (valid) {
+        eo0[c] = ex;
+        eo1[c] = ey;
+        eo2[c] = ez;
+        if (col.edge_ij || edge_k(g, q)) {
+          store_images_inl<exp_of_e<0>()>(eo0, g, i, j, q, c, ex);
+          store_images_inl<exp_of_e<1>()>(eo1, g, i, j, q, c, ey);
+          store_images_inl<exp_of_e<2>()>(eo2, g, i, j, q, c, ez);
         }
-      } else {
-        {  // row y0 + SBY: E_x, E_z at (x0 + lane, y0 + SBY)
-          const int tr = (SBY + 1) * EW + lane + 2, ur = SBY * EW + lane;
-          Nw[ur] = eh_edge<L, 0, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q, wj_rim || wk);
-          Nw[2 * NSLOT_D + ur] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tr, w.x0 + lane, w.y0 + SBY, q, wi_rimrow || wj_rim);
-        }
-        if (lane < SBY) {  // column x0 + SW: E_y, E_z at (x0 + SW, y0 + lane)
-          const int tc = (lane + 1) * EW + SW + 2, uc = lane * EW + SW;
-          Nw[NSLOT_D + uc] = eh_edge<L, 1, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wk || wi_rim);
-          Nw[2 * NSLOT_D + uc] = eh_edge<L, 2, EPS_ARR, SIG_ARR, HAS_SRC>(p, A, B, tc, w.x0 + SW, w.y0 + lane, q, wi_rim || wj_rimcol);
-        }
-      }
-      if (FUSE) {
-        // every warp's part of E^{n+1}(q) is in shared memory; the plane q-1 the H update reads was
-        // completed one barrier earlier, and the plane written next (q+1) was last read two
-        // barriers ago: three rotating planes, one barrier per plane
-        asm volatile("bar.sync 1, %0;" ::"n"(L::NCW * 32) : "memory");
-        if (valid && q > w.k0) {
-          const int cm = c - g.sz;   // plane q-1
-          // (curl E^{n+1})_D at the D-face of plane q-1: forward differences, as curl_e (kernels.cuh)
-          const double cx = (Np[2 * NSLOT_D + u0 + EW] - ez_p) * g.rd[1] - (ey - ey_p) * g.rd[2];
-          const double cy = (ex - ex_p) * g.rd[2] - (Np[2 * NSLOT_D + u0 + 1] - ez_p) * g.rd[0];
-          const double cz = (Np[NSLOT_D + u0 + 1] - ey_p) * g.rd[0] - (Np[u0 + EW] - ex_p) * g.rd[1];
-          const double hx = h_face_val(A[L::HH + t0], p.chm, cx, col.wall[0]);
-          const double hy = h_face_val(A[L::HH + ESLOT + t0], p.chm, cy, col.wall[1]);
-          const double hz = h_face_val(A[L::HH + 2 * ESLOT + t0], p.chm, cz, wall_k(g, q - 1));
-          p.Ho[0][cm] = hx;
-          p.Ho[1][cm] = hy;
-          p.Ho[2][cm] = hz;
-          if (col.edge_ij || edge_k(g, q - 1)) {
-            store_images_inl<exp_of_h<0>()>(p.Ho[0], g, i, j, q - 1, cm, hx);
-            store_images_inl<exp_of_h<1>()>(p.Ho[1], g, i, j, q - 1, cm, hy);
-            store_images_inl<exp_of_h<2>()>(p.Ho[2], g, i, j, q - 1, cm, hz);
-          }
-        }
-        ex_p = ex; ey_p = ey; ez_p = ez;
-        double *const tmp = Np; Np = Nw; Nw = Nx; Nx = tmp;   // rotate: written -> read, spare -> written
       }
       c += g.sz;
       __syncwarp();
@@ -282,15 +225,16 @@ k_eh_stage(const __grid_constant__ EHArgs p) {
   }
 }
 
-// ------------------------------------------------------------------ the fused sweep, warp-specialised
-// k_eh_stage<FUSE> above does the E phase and the H phase of a plane in the SAME 16 + 1 warps, in
-// lockstep with one block barrier per plane: 18 warps per SM, each carrying ~375 instructions per
-// plane, wait on fixed latencies more than they issue (ncu: issue slots 52 % busy, DRAM 73 %).
-// k_eh_fused gives the two phases to two sets of warps: 16 + 1 E warps compute E^{n+1}(q) into one
-// of three rotating planes in shared memory and store it; 16 H warps take H(q-1) from E^{n+1}(q-1)
-// and E^{n+1}(q).  The sets are coupled by two rings of mbarriers (efull / eempty per plane) instead
-// of a block barrier, so the E warps run up to two planes ahead; 34 warps per SM.  Same arithmetic,
-// same bits.
+// ------------------------------------------------------------------ E + H fused, warp-specialised
+// A first version did the E phase and the H phase of a plane in the SAME 16 + 1 warps, in lockstep
+// with one block barrier per plane: 18 warps per SM, each carrying ~375 instructions per plane,
+// waited on fixed latencies more than they issued (ncu, profiles/r02_notes.md: issue slots 52 %
+// busy, 4.3 TB/s at 256^3).  k_eh_fused gives the two phases to two sets of warps: 15 + 1 E warps
+// compute E^{n+1}(q) into one of three rotating planes in shared memory and store it (the 16th
+// computes the rim: row y0 + 15 and column x0 + 32); 15 H warps take H(q-1) from E^{n+1}(q-1) and
+// E^{n+1}(q).  The sets are coupled by two rings of mbarriers (efull / eempty per plane) instead of
+// a block barrier, so the E warps run up to two planes ahead: 32 warps per SM (the most a block
+// can have, hence 15 rows), 4.8 TB/s at 256^3.  Same arithmetic, same bits.
 // A block has at most 32 warps: 15 tile rows (15 + 1 E warps, 15 H warps, the producer).
 constexpr int FBY = 15;
 constexpr int FROWS = FBY + 2;                // staged rows y0-1 .. y0+15

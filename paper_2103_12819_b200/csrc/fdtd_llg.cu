@@ -530,8 +530,8 @@ int launch_eh_stage(fdtd_llg *s, const EHArgs &p) {
       using L = EfLayout<EA, SA>;                                                               \
       k_eh_fused<EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);               \
     } else {                                                                                    \
-      using L = EhLayout<false, EA, SA>;                                                        \
-      k_eh_stage<false, EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);        \
+      using L = EhLayout<EA, SA>;                                                               \
+      k_eh_stage<EA, SA, HS><<<grid, L::NTHREADS, L::SMEM_BYTES, s->stream>>>(p);               \
     }                                                                                           \
     return FDTD_LLG_OK;                                                                         \
   }
@@ -543,9 +543,9 @@ int launch_eh_stage(fdtd_llg *s, const EHArgs &p) {
 
 int setup_eh_stage(fdtd_llg *s) {
 #define SA(EA, SA_, HS)                                                                         \
-  CU(s, cudaFuncSetAttribute(k_eh_stage<false, EA, SA_, HS>,                                    \
+  CU(s, cudaFuncSetAttribute(k_eh_stage<EA, SA_, HS>,                                           \
                              cudaFuncAttributeMaxDynamicSharedMemorySize,                       \
-                             (int)EhLayout<false, EA, SA_>::SMEM_BYTES));                       \
+                             (int)EhLayout<EA, SA_>::SMEM_BYTES));                              \
   CU(s, cudaFuncSetAttribute(k_eh_fused<EA, SA_, HS>,                                           \
                              cudaFuncAttributeMaxDynamicSharedMemorySize,                       \
                              (int)EfLayout<EA, SA_>::SMEM_BYTES));
