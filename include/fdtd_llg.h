@@ -131,6 +131,9 @@ typedef struct {
                                        or a sweep box too small to give every SM a work item)   */
   int merged_h;                     /* 1: the H half-steps outside the sweep box are merged
                                        (options.merge_h and no PML, no H source)                */
+  int staged_maxwell;               /* the E phase runs the staged sweeps (eh_stage.cuh): 0 no (small
+                                       grid, PML, kernel_path 1: k_e_update), 1 yes, 2 yes and fused
+                                       with the merged H update outside the sweep box            */
 } fdtd_llg_stats;
 
 /* kernel classes of fdtd_llg_step_timed */

@@ -42,7 +42,7 @@ class Stats(C.Structure):
                 ("kernel_launches", C.c_longlong), ("magnetic_cells", C.c_longlong),
                 ("launches_per_step", C.c_int), ("sweep_cells", C.c_longlong),
                 ("material_array_mask", C.c_uint), ("staged_sweeps", C.c_int),
-                ("merged_h", C.c_int)]
+                ("merged_h", C.c_int), ("staged_maxwell", C.c_int)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

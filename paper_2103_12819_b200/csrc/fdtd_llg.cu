@@ -1562,6 +1562,12 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
     return fail(s, FDTD_LLG_ESTATE, "a TMA pipeline wait timed out (wait tag %d): results are invalid", h.pipe_error);
   std::memset(out, 0, sizeof *out);
   out->merged_h = s->merge ? 1 : 0;
+  {
+    ERegion reg[16];
+    const int nr = plan_e_regions(s, reg);
+    for (int r = 0; r < nr; ++r)
+      out->staged_maxwell = std::max(out->staged_maxwell, reg[r].fuse ? 2 : (reg[r].staged ? 1 : 0));
+  }
   out->steps = h.steps;
   out->time = (double)h.steps * s->dt;
   out->iters_last = h.iters_last;

@@ -24,7 +24,7 @@ int main(void) {
   F(fdtd_llg_stats, halfsteps); F(fdtd_llg_stats, courant); F(fdtd_llg_stats, kernel_launches);
   F(fdtd_llg_stats, magnetic_cells); F(fdtd_llg_stats, launches_per_step);
   F(fdtd_llg_stats, sweep_cells); F(fdtd_llg_stats, material_array_mask);
-  F(fdtd_llg_stats, staged_sweeps); F(fdtd_llg_stats, merged_h);
+  F(fdtd_llg_stats, staged_sweeps); F(fdtd_llg_stats, merged_h); F(fdtd_llg_stats, staged_maxwell);
   S(fdtd_llg_slab_info);
   F(fdtd_llg_slab_info, fields_offset); F(fdtd_llg_slab_info, array_stride);
   F(fdtd_llg_slab_info, nx); F(fdtd_llg_slab_info, ny); F(fdtd_llg_slab_info, nz);

@@ -43,7 +43,9 @@ def _run(cfg, shape, steps=100):
     got = {k: v.numpy() for k, v in sim.read_fields(names=names).items()}
     st = sim.stats()
     rec = {"test": "parity_at_size", "config": cfg, "shape": [w.nx, w.ny, w.nz], "steps": steps,
-           "path": "default (staged sweeps)" if st["staged_sweeps"] else "default (direct-load sweeps)",
+           "path": "default: " + ("LLG sweeps " + ("staged" if st["staged_sweeps"] else "direct-load") + ", "
+                                   if w.enable_llg else "")
+                   + "Maxwell sweeps " + ("direct-load", "staged", "staged + fused")[st["staged_maxwell"]],
            "merged_h": st["merged_h"], "time_loop": "CUDA graph replay"}
     for g in ("E", "H") + (("M",) if w.enable_llg else ()):
         rec["err_" + g] = rel_linf(got, ref, g)
