@@ -323,11 +323,12 @@ def _measure_other(cfg, K, W, dev, args, peak, peak_src):
     out = {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"], "steps": K,
            "gcell_s": cells * K / (ms * 1e-3) * 1e-9, "ms_per_step": ms / K,
            "launches_per_step": st["launches_per_step"], "staged_sweeps": st["staged_sweeps"],
-           "merged_h": st["merged_h"],
+           "merged_h": st["merged_h"], "staged_maxwell": st["staged_maxwell"],
            "llg_iterations_per_halfstep": st["iters_total"] / max(1, st["halfsteps"]),
            "alg_bytes_per_cell_step": roof["whole_step"]["alg_bytes_per_step"] / cells,
            "whole_step_frac": roof["whole_step"]["frac"], "whole_step_GBps": roof["whole_step"]["achieved"],
            "dominant_kernel": roof["kernel"], "dominant_frac": roof["frac"],
+           "dominant_traffic": roof["traffic"],
            "kernels": {k: {"us_per_launch": v["us_per_launch"], "launches": v["launches"],
                            "alg_GBps": v.get("alg_GBps")} for k, v in roof["kernels"].items()}}
     sim.close()
@@ -526,6 +527,7 @@ def run_ours(args):
                                  else "state fits L2: latency-bound case, no roofline claim",
                            "time_loop": "CUDA graph replay" if world == 1 else "plain launches (sub-steps)",
                            "kernel_path": args.kernel_path, "merge_h": st["merged_h"],
+                           "staged_sweeps": st["staged_sweeps"], "staged_maxwell": st["staged_maxwell"],
                            "time_scheme": "first-order" if args.time_scheme else "second-order"},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
                 "gpu_launches": launches, "other_configs": other,
