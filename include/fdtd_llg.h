@@ -277,6 +277,9 @@ typedef struct {
   int ny;
   int nz;
   int n_arrays;                     /* field arrays at that stride (E, H, M sets)                */
+  int merged_h;                     /* the handle's merge_h state: all slabs of a grid must agree (a
+                                       PML or an H source switches it off for the handle that has it:
+                                       create the other slabs with options.merge_h = 0 then)       */
 } fdtd_llg_slab_info;
 
 /* Layout facts a neighbour needs (HOST struct out). */
@@ -284,7 +287,8 @@ int fdtd_llg_get_slab_info(fdtd_llg *s, fdtd_llg_slab_info *out);
 
 /* Connect the interfaces.  lo / hi: the lower / upper neighbour's info (NULL on a side that is not
  * an interface), lo_workspace / hi_workspace: DEVICE address of that neighbour's workspace as seen
- * from this process and this GPU.  EINVAL if the shapes differ.  Invalidates the captured step. */
+ * from this process and this GPU.  EINVAL if the shapes or the merge_h states differ.  Sources of H
+ * (which switch merge_h off) must be added before connecting.  Invalidates the captured step. */
 int fdtd_llg_slab_connect(fdtd_llg *s, const fdtd_llg_slab_info *lo, void *lo_workspace,
                           const fdtd_llg_slab_info *hi, void *hi_workspace);
 

@@ -50,7 +50,8 @@ class Stats(C.Structure):
 
 class SlabInfo(C.Structure):
     _fields_ = [("fields_offset", C.c_ulonglong), ("array_stride", C.c_ulonglong),
-                ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("n_arrays", C.c_int)]
+                ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("n_arrays", C.c_int),
+                ("merged_h", C.c_int)]
 
     def as_tuple(self):
         return tuple(getattr(self, k) for k, _ in self._fields_)

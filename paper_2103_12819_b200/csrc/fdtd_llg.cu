@@ -1430,6 +1430,9 @@ int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const in
         return fail(s, FDTD_LLG_EINVAL, "hard / soft field sources must lie outside the PML");
   if (s->sub_next != FDTD_LLG_SUB_BEGIN) return fail(s, FDTD_LLG_ESTATE, "a time step is open (fdtd_llg_substep)");
   if (kind == FDTD_LLG_SRC_SOFT_H || kind == FDTD_LLG_SRC_HARD_H) {  // these act on H at integer time
+    if (s->merge && (s->g.dlo != 0 || s->g.dhi != 0))
+      return fail(s, FDTD_LLG_ESTATE, "an H source switches merge_h off, which all slabs of a grid must agree on: "
+                  "add it before fdtd_llg_slab_connect (or create the slabs with options.merge_h = 0)");
     int rc = unmerge(s);
     if (rc) return rc;
   }
@@ -1613,6 +1616,7 @@ int fdtd_llg_get_slab_info(fdtd_llg *s, fdtd_llg_slab_info *out) {
   out->array_stride = (unsigned long long)s->stride;
   out->nx = s->g.n[0]; out->ny = s->g.n[1]; out->nz = s->g.n[2];
   out->n_arrays = 6 + 3 * (s->opt.enable_llg ? 3 : 2) + (s->opt.enable_llg ? 18 : 0);
+  out->merged_h = s->merge ? 1 : 0;
   return FDTD_LLG_OK;
 }
 
@@ -1633,6 +1637,9 @@ int fdtd_llg_slab_connect(fdtd_llg *s, const fdtd_llg_slab_info *lo, void *lo_wo
         nb[sd]->array_stride != me.array_stride || nb[sd]->n_arrays != me.n_arrays)
       return fail(s, FDTD_LLG_EINVAL, "slabs must have the same nx, ny, nz and field storage (neighbour: %d x %d x %d, %d arrays)",
                   nb[sd]->nx, nb[sd]->ny, nb[sd]->nz, nb[sd]->n_arrays);
+    if (nb[sd]->merged_h != me.merged_h)
+      return fail(s, FDTD_LLG_EINVAL, "slabs disagree on merge_h (%d here, %d there): a PML or an H source switches it off for "
+                  "one handle; create all slabs of the grid with options.merge_h = 0 then", me.merged_h, nb[sd]->merged_h);
     const char *theirs = static_cast<const char *>(ws[sd]) + nb[sd]->fields_offset;
     const long long base = (long long)(theirs - reinterpret_cast<const char *>(s->E[0]));
     const long long plane = 8LL * s->g.sz * s->g.n[2];

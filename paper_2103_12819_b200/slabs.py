@@ -70,6 +70,13 @@ def _planes(plan: SlabPlan, nz_global: int) -> list:
     return ks
 
 
+def merge_ok(w) -> bool:
+    """merge_h is a property of the whole grid: a PML or an H source anywhere switches it off on the
+    handle that has it, and all slabs must agree (fdtd_llg_slab_connect checks)."""
+    pml = getattr(w, "pml", None)
+    return not (pml is not None and any(pml)) and not any(getattr(q, "kind", 0) in (2, 3) for q in w.sources)
+
+
 def cut_workload(w, plan: SlabPlan):
     """The slab-local workload: every array cut to the slab's planes plus the neighbours' adjacent
     planes, source boxes clipped to the slab (slab coordinates), the z boundary type kept only
@@ -88,6 +95,7 @@ def cut_workload(w, plan: SlabPlan):
         return t.index_select(0, torch.tensor(ks, device=t.device)).contiguous()
 
     s = copy.copy(w)
+    s.merge_ok = merge_ok(w)
     s.name = f"{w.name}[slab {plan.rank}/{plan.world}]"
     s.nz = plan.nz
     s.bc = (w.bc[0], w.bc[1], PEC)
@@ -147,6 +155,7 @@ def stack_copies(w, plan: SlabPlan):
         return torch.cat(parts, 0).contiguous()
 
     s = copy.copy(w)
+    s.merge_ok = merge_ok(w)
     s.name = f"{w.name}[copy {plan.rank} of {plan.world} stacked in z]"
     s.slab_ext = plan.ext
     s.materials = {k: ext(v, True) for k, v in w.materials.items()}
@@ -241,7 +250,7 @@ class LocalSlabs(SlabStepper):
         self.plans = plan_slabs(w.nz, world, w.bc[2] == PERIODIC)
         self.stream = torch.cuda.Stream(device)
         sims = [from_workload(cut_workload(w, p), device=device, stream=self.stream, use_graph=False,
-                              kernel_path=kernel_path, merge_h=merge_h, time_scheme=time_scheme,
+                              kernel_path=kernel_path, merge_h=merge_h and merge_ok(w), time_scheme=time_scheme,
                               slab_ext=p.ext) for p in self.plans]
         for p, s in zip(self.plans, sims):
             nb = [None if q is None else (sims[q].slab_info(), sims[q].workspace.data_ptr())
@@ -249,7 +258,8 @@ class LocalSlabs(SlabStepper):
             if world > 1:
                 s.connect(nb[0], nb[1])
         any_llg = any(s.stats()["sweep_cells"] > 0 for s in sims)
-        super().__init__(sims, any_llg, w.llg_max_iter if w.enable_llg else 1, w.llg_tol)
+        # the first-order scheme takes one explicit sweep per half-step (no iteration)
+        super().__init__(sims, any_llg, w.llg_max_iter if (w.enable_llg and not time_scheme) else 1, w.llg_tol)
         self._words = {}
 
     def _word(self, r):
@@ -296,7 +306,8 @@ class DistSlab(SlabStepper):
         self.stream = torch.cuda.Stream(self.device)
         w = slab_workload
         sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,
-                            kernel_path=kernel_path, merge_h=merge_h, time_scheme=time_scheme,
+                            kernel_path=kernel_path, merge_h=merge_h and getattr(w, "merge_ok", True),
+                            time_scheme=time_scheme,
                             slab_ext=plan.ext)
         self.sim = sim
         self._mapped = {}
@@ -319,7 +330,8 @@ class DistSlab(SlabStepper):
                             device="cpu" if self._gloo() else self.device)
         if plan.world > 1:
             dist.all_reduce(flag, op=dist.ReduceOp.MAX, group=group)
-        super().__init__([sim], bool(flag.item() > 0), w.llg_max_iter if w.enable_llg else 1, w.llg_tol)
+        super().__init__([sim], bool(flag.item() > 0),
+                         w.llg_max_iter if (w.enable_llg and not time_scheme) else 1, w.llg_tol)
         self._words = {}
         if plan.world > 1:
             dist.barrier(group=group)

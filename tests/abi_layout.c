@@ -28,7 +28,7 @@ int main(void) {
   S(fdtd_llg_slab_info);
   F(fdtd_llg_slab_info, fields_offset); F(fdtd_llg_slab_info, array_stride);
   F(fdtd_llg_slab_info, nx); F(fdtd_llg_slab_info, ny); F(fdtd_llg_slab_info, nz);
-  F(fdtd_llg_slab_info, n_arrays);
+  F(fdtd_llg_slab_info, n_arrays); F(fdtd_llg_slab_info, merged_h);
   printf("enum SUB %d %d %d %d %d %d\n", FDTD_LLG_SUB_BEGIN, FDTD_LLG_SUB_HM1, FDTD_LLG_SUB_HM1_END,
          FDTD_LLG_SUB_E, FDTD_LLG_SUB_HM2, FDTD_LLG_SUB_HM2_END);
   printf("enum K_NCLASS %d\n", FDTD_LLG_K_NCLASS);

@@ -365,3 +365,37 @@ def test_errors_are_reported_not_thrown_from_c():
         sim.step(-1)
     st = sim.stats()
     assert st["courant"] == pytest.approx(1e-15 / wl.courant_dt(1.0, 1e-6, 1e-6, 1e-6))
+
+
+def test_h_source_added_mid_run_leaves_the_merged_mode_and_restart_with_set_fields():
+    """merge_h keeps H at half-integer time outside the sweep box; an H source acts on H at integer
+    time, so adding one converts the state back (unmerge).  Oracle: the same source added after the
+    same number of steps.  Then set_fields on the used handle gives what a fresh handle gives."""
+    from paper_2103_12819_b200.binding import from_workload
+    for cfg in (4, 3):
+        w = wl.make_config(cfg, shape=wl.SMALL_SHAPES[cfg])
+        o = oracle_from_workload(w)
+        sim = from_workload(w)
+        assert sim.stats()["merged_h"] == 1
+        o.step(17)
+        sim.step(17)
+        f0, tp = 5e12, 20 * w.dt
+        lo, hi = (3, 2, 5), (w.nx - 2, w.ny - 1, 9)
+        o.set_source(1, lo, hi, None, 3e2, f0, 40 * w.dt, tp, kind=3)           # hard H_y
+        sim.set_source(1, lo, hi, None, 3e2, f0, 40 * w.dt, tp, kind=3)
+        assert sim.stats()["merged_h"] == 0
+        o.step(25)
+        sim.step(25)
+        _assert_parity(_gpu_fields(sim), o.read_fields(), w.enable_llg)
+        assert sim.stats()["steps"] == 42
+    # restart: set_fields resets the clock, the statistics and the half-time state of the merged faces
+    w = wl.make_config(4, shape=wl.SMALL_SHAPES[4])
+    a, b = from_workload(w), from_workload(w)
+    a.step(13)
+    a.set_fields(w.E, w.H, w.M_cell)
+    a.step(20)
+    b.step(20)
+    fa, fb = _gpu_fields(a), _gpu_fields(b)
+    for k in fa:
+        assert np.array_equal(fa[k], fb[k]), k
+    assert a.stats()["steps"] == 20

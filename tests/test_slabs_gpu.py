@@ -148,6 +148,19 @@ def test_out_of_order_substeps_and_step_on_a_connected_slab_are_refused():
     with pytest.raises(B.FdtdLlgError) as e:
         grp.sims[1].connect((other.slab_info(), other.workspace.data_ptr()), None)
     assert e.value.code in (B.EINVAL, B.ESTATE)
+    # merge_h is a property of the whole grid: slabs that disagree are refused, and so is an H source
+    # (which switches it off) on a connected slab
+    from paper_2103_12819_b200.slabs import cut_workload, plan_slabs
+    plans = plan_slabs(w.nz, 2, False)
+    lo = B.from_workload(cut_workload(w, plans[0]), use_graph=False, merge_h=True)
+    hi = B.from_workload(cut_workload(w, plans[1]), use_graph=False, merge_h=False)
+    with pytest.raises(B.FdtdLlgError) as e:
+        lo.connect(None, (hi.slab_info(), hi.workspace.data_ptr()))
+    assert e.value.code == B.EINVAL and "merge_h" in str(e.value)
+    grp2 = LocalSlabs(w, 2)
+    with pytest.raises(B.FdtdLlgError) as e:
+        grp2.sims[0].set_source(0, (0, 0, 0), (4, 4, 2), kind=3)
+    assert e.value.code == B.ESTATE and "merge_h" in str(e.value)
 
 
 def _free_port():
@@ -177,3 +190,28 @@ def test_two_processes_map_each_other_with_cuda_ipc(cfg, shape, tmp_path):
         assert np.array_equal(got, ref[n]), n
     if w.enable_llg:
         assert int(parts[0]["iters_total"]) == st["iters_total"]
+
+
+def test_slabs_first_order_scheme_and_open_boundary_with_hard_h_source():
+    """The other step variants across cuts: the first-order scheme (one explicit sweep per half-step),
+    and the paper's tunable-filter set-up in small (PML at the z-low end, hard H source on the last
+    plane, LLG slab on a side wall, dielectric array: two H half-steps everywhere, k_pml on the end
+    slab only)."""
+    from paper_2103_12819_b200.slabs import LocalSlabs
+    w = wl.make_config(5, shape=(40, 44, 36))
+    ref, st = _single(w, 10, time_scheme=1)
+    grp = LocalSlabs(w, 3, time_scheme=1)
+    grp.step(10)
+    got = grp.read_fields()
+    for n in ALL:
+        assert np.array_equal(got[n], ref[n]), n
+    w = wl.paper_tunable_filter(nx=96, ny=4, nz=48, npml=8)
+    ref, st = _single(w, 40)
+    assert st["merged_h"] == 0
+    for world in (2, 3):
+        grp = LocalSlabs(w, world)
+        grp.step(40)
+        got = grp.read_fields()
+        for n in ALL:
+            assert np.array_equal(got[n], ref[n]), (world, n)
+    assert max(float(np.max(np.abs(ref[n]))) for n in FIELD_GROUPS["M"]) > 0
