@@ -289,6 +289,10 @@ class LocalSlabs(SlabStepper):
         return {k: np.concatenate([p[k] for p in parts], 0) for k in parts[0]}
 
 
+class SlabSetupError(RuntimeError):
+    """Raised on EVERY rank when the slabs of a grid could not be created and connected."""
+
+
 class DistSlab(SlabStepper):
     """One slab per rank of a ``torch.distributed`` group, one process per GPU.  The neighbours'
     workspaces are mapped with CUDA IPC (peer access over NVLink); ``merge`` is an 8-byte
@@ -305,27 +309,52 @@ class DistSlab(SlabStepper):
         self.device = torch.device(device)
         self.stream = torch.cuda.Stream(self.device)
         w = slab_workload
-        sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,
-                            kernel_path=kernel_path, merge_h=merge_h and getattr(w, "merge_ok", True),
-                            time_scheme=time_scheme,
-                            slab_ext=plan.ext)
-        self.sim = sim
-        self._mapped = {}
+        self.sim, self._mapped = None, {}
+        # Set-up in lockstep: every step that can fail locally (creating the handle, exporting its
+        # workspace, mapping a neighbour's) is followed by a collective in which ALL ranks learn
+        # whether it worked, so that a failure on one rank raises SlabSetupError on every rank
+        # instead of leaving the others in a collective.
+        err, mine = None, None
+        try:
+            import os
+            if os.environ.get("FDTD_LLG_TEST_FAIL_RANK") == str(plan.rank):   # test hook: a rank that cannot set up
+                raise RuntimeError("FDTD_LLG_TEST_FAIL_RANK")
+            self.sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,
+                                     kernel_path=kernel_path, merge_h=merge_h and getattr(w, "merge_ok", True),
+                                     time_scheme=time_scheme, slab_ext=plan.ext)
+            if plan.world > 1:
+                mine = (self.sim.slab_info().as_tuple(),) + self.sim.ipc_export()
+        except Exception as e:          # noqa: BLE001  (reported to all ranks below)
+            err = e
         if plan.world > 1:
-            mine = (sim.slab_info().as_tuple(),) + sim.ipc_export()
             everyone = [None] * plan.world
             dist.all_gather_object(everyone, mine, group=group)
-            nb = []
-            for q in (plan.lo, plan.hi):
-                if q is None:
-                    nb.append(None)
-                    continue
-                info, handle, off = everyone[q]
-                if q not in self._mapped:
-                    with torch.cuda.device(self.device):
-                        self._mapped[q] = (fdtd_llg_ipc_open(handle, off), off)
-                nb.append((SlabInfo.from_tuple(info), self._mapped[q][0]))
-            sim.connect(nb[0], nb[1])
+            if err is None:
+                try:
+                    nb = []
+                    for q in (plan.lo, plan.hi):
+                        if q is None:
+                            nb.append(None)
+                            continue
+                        if everyone[q] is None:
+                            raise RuntimeError(f"rank {q} could not create or export its slab")
+                        info, handle, off = everyone[q]
+                        if q not in self._mapped:
+                            with torch.cuda.device(self.device):
+                                self._mapped[q] = (fdtd_llg_ipc_open(handle, off), off)
+                        nb.append((SlabInfo.from_tuple(info), self._mapped[q][0]))
+                    self.sim.connect(nb[0], nb[1])
+                except Exception as e:  # noqa: BLE001
+                    err = e
+            ok = torch.tensor([0.0 if err is not None else 1.0], dtype=torch.float64,
+                              device="cpu" if self._gloo() else self.device)
+            dist.all_reduce(ok, op=dist.ReduceOp.MIN, group=group)
+            if float(ok.item()) == 0.0:
+                self._release()
+                raise SlabSetupError(repr(err) if err is not None else "the slab set-up failed on another rank")
+        elif err is not None:
+            raise err
+        sim = self.sim
         flag = torch.tensor([float(sim.stats()["sweep_cells"] > 0)], dtype=torch.float64,
                             device="cpu" if self._gloo() else self.device)
         if plan.world > 1:
@@ -335,6 +364,17 @@ class DistSlab(SlabStepper):
         self._words = {}
         if plan.world > 1:
             dist.barrier(group=group)
+
+    def _release(self):
+        for p, off in self._mapped.values():
+            try:
+                fdtd_llg_ipc_close(p, off)
+            except Exception:           # noqa: BLE001
+                pass
+        self._mapped = {}
+        if self.sim is not None:
+            self.sim.close()
+            self.sim = None
 
     def _gloo(self):
         return self.dist.get_backend(self.group) == "gloo"
@@ -368,7 +408,4 @@ class DistSlab(SlabStepper):
         self.stream.synchronize()
         if self.plan.world > 1:
             self.dist.barrier(group=self.group)      # nobody still stores into a workspace that goes away
-        for p, off in self._mapped.values():
-            fdtd_llg_ipc_close(p, off)
-        self._mapped = {}
-        self.sim.close()
+        self._release()
