@@ -57,8 +57,15 @@ struct EHArgs {
   double chm;          // FUSE: cmul * dt / (2 mu) = dt / mu (uniform mu)
   SourcesP src;
   const DevState *st;
-  unsigned *work;      // item counter of this launch (zero at launch; k_half_end re-arms it)
+  unsigned *work;      // item counter of this launch (zero at launch; re-armed by k_half_end, or by the
+                       // next step's launch when the bookkeeping is folded in, see `book`)
   int *pipe_error;
+  // A Maxwell-only step whose E phase is ONE fused launch needs no other kernel: the launch also
+  // closes the two H half-steps in the run state (what k_half_end does) and re-arms the item
+  // counters of the OTHER step parity (nobody draws from them during this step).
+  DevState *book;      // nullptr: k_half_end does the bookkeeping
+  unsigned *work_other;  // [8] counters of the other step parity
+  int *r_hist;
 };
 
 // the TMA loads of stage pz of the tile at (x0, y0): every array with the same box origin
@@ -291,6 +298,16 @@ k_eh_fused(const __grid_constant__ EHArgs p) {
   }
   __syncthreads();
 
+  if (p.book && blockIdx.x == 0 && threadIdx.x == 0) {   // the step's bookkeeping (k_half_end, twice)
+    DevState *st = p.book;
+    st->iters_last = 0;
+    st->last_R_even = 0;
+    p.r_hist[st->halfsteps % 4096] = 0;
+    p.r_hist[(st->halfsteps + 1) % 4096] = 0;
+    st->halfsteps += 2;
+    st->steps++;
+    for (int q = 0; q < 8; ++q) p.work_other[q] = 0u;
+  }
   const StBox &T = p.tb;
   const GridP &g = p.g;
   auto next = [](unsigned &st, unsigned &ph) { if (++st == (unsigned)L::NS) { st = 0; ph ^= 1u; } };

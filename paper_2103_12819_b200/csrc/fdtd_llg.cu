@@ -71,7 +71,7 @@ struct fdtd_llg {
   // staged Maxwell sweeps (eh_stage.cuh): the E update, fused with the merged H update outside the box
   bool eh_ok = false;        // tensor map built, kernels configured (no PML, kernel_path != 1)
   CUtensorMap mapEH{}, mapEF{};   // boxes of k_eh_stage (18 rows) and of k_eh_fused (17 rows)
-  unsigned *work_eh = nullptr;  // [8] item counters, one per staged launch of a step
+  unsigned *work_eh = nullptr;  // [2][8] item counters: one per staged launch of a step, by step parity
   BoxP box_out[6]{};     // the complement of the sweep box, as slabs
   int n_out = 0;
   // open boundary: split parts of E and H, damping tables, the layer's slabs
@@ -747,6 +747,7 @@ struct ERegion {
   bool staged, fuse;
 };
 int plan_e_regions(const fdtd_llg *s, ERegion *out);
+bool fold_bookkeeping(const fdtd_llg *s);
 int count_sources(const fdtd_llg *s, int kind);
 int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul, bool exports, int *launches,
                     bool skip_fused = false) {
@@ -861,6 +862,10 @@ int enqueue_sweep(fdtd_llg *s, double *const *E, int in, int out, int tmp, int m
 // (H,M) half-step, part 3: iteration count and statistics from the residual words of the r_max
 // iterates that were enqueued, the canonical H set
 int enqueue_half_end(fdtd_llg *s, int out, int tmp, int r_max, bool last, int *launches) {
+  if (fold_bookkeeping(s)) {   // done by the step's fused Maxwell launch
+    if (s->prof) s->prof_half++;
+    return FDTD_LLG_OK;
+  }
   const dim3 blk(TX, TY, 1);
   prof_begin(s, FDTD_LLG_K_OTHER, 0);
   k_half_end<<<1, 1, 0, s->stream>>>(s->dstate, s->resid, s->work, s->work_eh, s->r_hist, r_max, s->opt.llg_max_iter,
@@ -983,10 +988,20 @@ int plan_e_regions(const fdtd_llg *s, ERegion *out) {
   return n;
 }
 
-int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int hset_next, int *launches) {
+// A step without magnetic cells whose E phase is one fused launch over the whole grid: that launch
+// also does the bookkeeping of the two H half-steps, and k_half_end is not launched (EHArgs::book)
+bool fold_bookkeeping(const fdtd_llg *s) {
+  if (s->llg || s->has_pml) return false;
+  ERegion reg[16];
+  return plan_e_regions(s, reg) == 1 && reg[0].fuse;
+}
+
+int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int hset_next, int par,
+                      int *launches) {
   ERegion reg[16];
   const int nr = plan_e_regions(s, reg);
-  int widx = 0;
+  const bool fold = fold_bookkeeping(s);
+  int widx = 8 * par;   // the staged launches of a step draw from the eight counters of its parity
   for (int r = 0; r < nr; ++r) {
     if (!reg[r].staged) {
       int rc = enqueue_e(s, Ein, Eout, hset, make_box(s, reg[r].lo, reg[r].hi), launches);
@@ -1011,6 +1026,9 @@ int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int 
     p.st = s->dstate;
     p.work = s->work_eh + widx++;
     p.pipe_error = &s->dstate->pipe_error;
+    p.book = fold ? s->dstate : nullptr;
+    p.work_other = s->work_eh + 8 * (par ^ 1);
+    p.r_hist = s->r_hist;
     prof_begin(s, reg[r].fuse ? FDTD_LLG_K_EH_FUSED : FDTD_LLG_K_E_UPDATE, 0);
     int rc = reg[r].fuse ? launch_eh_stage<true>(s, p) : launch_eh_stage<false>(s, p);
     prof_end(s);
@@ -1071,7 +1089,7 @@ int enqueue_begin(fdtd_llg *s, int *launches) {
 int enqueue_e_phase(fdtd_llg *s, int par, int *launches) {
   double *const *Ea = e_set(s, par), *const *Eb = e_set(s, par ^ 1);
   const int h1 = set_half(s, par);
-  int rc = enqueue_e_regions(s, Ea, Eb, h1, set_half(s, par ^ 1), launches);
+  int rc = enqueue_e_regions(s, Ea, Eb, h1, set_half(s, par ^ 1), par, launches);
   if (rc) return rc;
   rc = enqueue_pml(s, true, s->Hset[h1], Eb, launches);
   if (rc) return rc;

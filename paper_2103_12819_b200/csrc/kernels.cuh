@@ -552,7 +552,7 @@ __global__ void k_set_cond(cudaGraphConditionalHandle h, const unsigned long lon
 __global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *work, unsigned *work_eh,
                            int *r_hist, int r_max, int max_iter, double tol, int any_magnetic,
                            int last_of_step) {
-  for (int q = 0; q < 8; ++q) work_eh[q] = 0u;   // item counters of the staged Maxwell sweeps
+  for (int q = 0; q < 16; ++q) work_eh[q] = 0u;  // item counters of the staged Maxwell sweeps (both step parities)
   if (any_magnetic) {
     int R = r_max;
     for (int r = 1; r <= r_max; ++r)
