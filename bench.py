@@ -308,7 +308,7 @@ def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
             "kernels": per_class}
 
 
-def _measure_other(cfg, K, W, dev, args, peak, peak_src):
+def _measure_other(cfg, K, W, dev, args, peak, peak_src, vis_index):
     """One of the other configs at full size: graph replay + the class breakdown, no e2e leg."""
     import torch
     from paper_2103_12819_b200 import workloads as wl
@@ -317,10 +317,23 @@ def _measure_other(cfg, K, W, dev, args, peak, peak_src):
     name, cells = _workload_name(w), w.cells
     sim = from_workload(w, device=dev, kernel_path=args.kernel_path, merge_h=not args.no_merge_h)
     del w
-    ms = _timed_steps(sim, K, W, lambda: None)
+    # These grids step in 0.2-3 ms: a timed region of K = 50 steps would be over before the GPU has
+    # left the clock / power state of the run before it (right after the 768^3 run the SM clock is
+    # still at the power-capped 1.4 GHz and a 17 ms measurement comes out 15 % low).  A pilot sets
+    # the step count so that the warm-up lasts >= 0.25 s and the timed region >= 0.5 s.
+    pilot = _timed_steps(sim, 10, max(W, 3), lambda: None) / 10.0
+    Kt = int(min(4000, max(K, 500.0 / pilot)))
+    sampler = ClockSampler(vis_index)
+    sampler.start()
+    t0 = time.perf_counter()
+    ms = _timed_steps(sim, Kt, int(max(W, 250.0 / pilot)), lambda: None)
+    t1 = time.perf_counter()
+    clocks = sampler.summary(t0, t1)
+    sampler.stop()
     st = sim.stats()
-    roof = _kernel_breakdown(sim, K, cells, ms / K, peak, peak_src, name)
-    out = {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"], "steps": K,
+    roof = _kernel_breakdown(sim, K, cells, ms / Kt, peak, peak_src, name)
+    K = Kt
+    out = {"workload": name, "cells": cells, "magnetic_cells": st["magnetic_cells"], "steps": K, "clocks": clocks,
            "gcell_s": cells * K / (ms * 1e-3) * 1e-9, "ms_per_step": ms / K,
            "launches_per_step": st["launches_per_step"], "staged_sweeps": st["staged_sweeps"],
            "merged_h": st["merged_h"], "staged_maxwell": st["staged_maxwell"],
@@ -508,7 +521,8 @@ def run_ours(args):
         other = {}
         for cfg in OTHER_CONFIGS:
             try:
-                other[f"config{cfg}"] = _measure_other(cfg, args.other_steps, max(W, 3), dev, args, peak, peak_src)
+                other[f"config{cfg}"] = _measure_other(cfg, args.other_steps, max(W, 3), dev, args, peak, peak_src,
+                                                       vis[local] if local < len(vis) else local)
             except Exception as e:  # a failure here must not lose the headline line
                 other[f"config{cfg}"] = {"error": repr(e)}
 
