@@ -169,7 +169,7 @@ def _free_port():
         return s.getsockname()[1]
 
 
-@pytest.mark.parametrize("cfg,shape", [(5, (40, 44, 36)), (2, (40, 36, 28))])
+@pytest.mark.parametrize("cfg,shape", [(5, (40, 44, 36)), (2, (40, 36, 28)), (4, (44, 36, 40))])
 def test_two_processes_map_each_other_with_cuda_ipc(cfg, shape, tmp_path):
     """One process per slab (as on a multi-GPU node), here both on GPU 0: workspaces exchanged as
     CUDA IPC handles, boundary planes stored straight into the other process's ghost planes."""
