@@ -287,8 +287,8 @@ def _kernel_breakdown(sim, K, cells, ms_step, peak, peak_src, name):
     dom_kernel = {"h_update": "k_h_update",
                   "hm_first": "k_hm_stage<FIRST>" if staged else "k_hm_sweep<FIRST>",
                   "hm_iter": "k_hm_stage<ITER>" if staged else "k_hm_sweep<ITER>",
-                  "e_update": "k_eh_stage<E>" if fused else "k_e_update",
-                  "eh_fused": "k_eh_stage<E+H>"}[dom]
+                  "e_update": "k_eh_stage" if fused else "k_e_update",
+                  "eh_fused": "k_eh_fused"}[dom]
     achieved = per_class[dom]["alg_GBps"]
     step_bytes = sum(per_class[c]["alg_bytes_per_launch"] * per_class[c]["launches"] for c in timed) / K
     traffic = _ncu_traffic(dom_kernel, name)
