@@ -101,8 +101,10 @@ typedef struct {
                          the first of step n+1 -- the same curl E^{n+1}, PAPER.md:94 -- as ONE update:
                          H is kept at half-integer time there and the integer-time value (the mean
                          the paper's scheme holds) is formed when fields are read.  A third less
-                         traffic; equal to the two half-steps up to rounding.  Not applied with a PML
-                         or with H sources.  0: two half-steps everywhere                        */
+                         traffic; equal to the two half-steps up to rounding.  The PML layer and the
+                         faces of an H source keep the plain half-steps: merging stops at a margin
+                         on each side of the grid (the layer; an H-source box within 8 cells of a
+                         side); an H source elsewhere switches it off.  0: two half-steps everywhere */
   int slab_ext[2];    /* z-low / z-high side of this grid is an INTERFACE to a neighbouring z-slab
                          (see Z-SLABS), neither wall nor periodic wrap; bc[2] must be FDTD_LLG_PEC
                          (it then describes the sides that are not interfaces)                    */
@@ -130,7 +132,7 @@ typedef struct {
                                        0: the direct-load kernel (general materials, kernel_path 1,
                                        or a sweep box too small to give every SM a work item)   */
   int merged_h;                     /* 1: the H half-steps outside the sweep box are merged
-                                       (options.merge_h and no PML, no H source)                */
+                                       (options.merge_h and no H source far from the sides)     */
   int staged_maxwell;               /* the E phase runs the staged sweeps (eh_stage.cuh): 0 no (small
                                        grid, PML, kernel_path 1: k_e_update), 1 yes, 2 yes and fused
                                        with the merged H update outside the sweep box            */

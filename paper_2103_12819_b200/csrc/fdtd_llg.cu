@@ -72,8 +72,12 @@ struct fdtd_llg {
   bool eh_ok = false;        // tensor map built, kernels configured (no PML, kernel_path != 1)
   CUtensorMap mapEH{}, mapEF{};   // boxes of k_eh_stage (18 rows) and of k_eh_fused (17 rows)
   unsigned *work_eh = nullptr;  // [2][8] item counters: one per staged launch of a step, by step parity
-  BoxP box_out[6]{};     // the complement of the sweep box, as slabs
+  BoxP box_out[6]{};     // the complement of the sweep box, as slabs (merged H: within the interior)
   int n_out = 0;
+  // merged H half-steps keep out of a margin at each side of the grid: the PML layer and thin boxes
+  // of H sources at a boundary (their faces need H at integer time); cells from the side
+  int um_lo[3]{}, um_hi[3]{};
+  std::vector<BoxP> box_um;   // the margins minus the sweep box: plain half-steps
   // open boundary: split parts of E and H, damping tables, the layer's slabs
   bool has_pml = false;
   double *Esp[6]{}, *Hsp[6]{};   // [2 * component + part]
@@ -376,33 +380,58 @@ int find_sweep_box(fdtd_llg *s) {
   return FDTD_LLG_OK;
 }
 
-// work decomposition: the sweep box, the whole grid, and the complement of the box as <= 6 slabs
+// outer \ inner as <= 6 disjoint boxes (inner inside outer, not empty): z slabs first (contiguous
+// planes), then y, then x
+template <class Emit>
+void peel(const int olo[3], const int ohi[3], const int ilo[3], const int ihi[3], Emit emit) {
+  int lo[3] = {olo[0], olo[1], olo[2]}, hi[3] = {ohi[0], ohi[1], ohi[2]};
+  for (int d = 2; d >= 0; --d) {
+    if (ilo[d] > lo[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      h[d] = ilo[d];
+      emit(l, h);
+    }
+    if (ihi[d] < hi[d]) {
+      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
+      l[d] = ihi[d];
+      emit(l, h);
+    }
+    lo[d] = ilo[d];
+    hi[d] = ihi[d];
+  }
+}
+bool clip(const int alo[3], const int ahi[3], const int blo[3], const int bhi[3], int lo[3], int hi[3]) {
+  bool any = true;
+  for (int d = 0; d < 3; ++d) {
+    lo[d] = std::max(alo[d], blo[d]);
+    hi[d] = std::min(ahi[d], bhi[d]);
+    any = any && lo[d] < hi[d];
+  }
+  return any;
+}
+
+// work decomposition: the sweep box, the whole grid, the complement of the box (within the interior
+// when the H half-steps are merged) as <= 6 slabs, and the unmerged margins minus the box
 void make_boxes(fdtd_llg *s) {
   const int zero[3] = {0, 0, 0};
   s->box_all = make_box(s, zero, s->g.n);
   s->n_out = 0;
-  if (!s->llg) {
-    s->box_out[s->n_out++] = s->box_all;
-    return;
-  }
-  s->box_llg = make_box(s, s->lo, s->hi);
-  int lo[3] = {0, 0, 0}, hi[3] = {s->g.n[0], s->g.n[1], s->g.n[2]};
-  for (int d = 2; d >= 0; --d) {  // peel z slabs first (contiguous planes), then y, then x
-    if (s->lo[d] > lo[d]) {
-      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
-      h[d] = s->lo[d];
-      s->box_out[s->n_out++] = make_box(s, l, h);
-    }
-    if (s->hi[d] < hi[d]) {
-      int l[3] = {lo[0], lo[1], lo[2]}, h[3] = {hi[0], hi[1], hi[2]};
-      l[d] = s->hi[d];
-      s->box_out[s->n_out++] = make_box(s, l, h);
-    }
-    lo[d] = s->lo[d];
-    hi[d] = s->hi[d];
-  }
+  s->box_um.clear();
+  if (s->llg) s->box_llg = make_box(s, s->lo, s->hi);
+  int ilo[3] = {0, 0, 0}, ihi[3] = {s->g.n[0], s->g.n[1], s->g.n[2]};   // the interior
+  if (s->merge)
+    for (int d = 0; d < 3; ++d) { ilo[d] = s->um_lo[d]; ihi[d] = s->g.n[d] - s->um_hi[d]; }
+  auto out = [&](const int *l, const int *h) { s->box_out[s->n_out++] = make_box(s, l, h); };
+  auto um = [&](const int *l, const int *h) { s->box_um.push_back(make_box(s, l, h)); };
+  int blo[3], bhi[3];
+  if (s->llg && clip(ilo, ihi, s->lo, s->hi, blo, bhi)) peel(ilo, ihi, blo, bhi, out);
+  else out(ilo, ihi);
+  if (s->merge)
+    peel(zero, s->g.n, ilo, ihi, [&](const int *l, const int *h) {   // the margins, each minus the box
+      if (s->llg && clip(l, h, s->lo, s->hi, blo, bhi)) peel(l, h, blo, bhi, um);
+      else um(l, h);
+    });
 }
-
 
 // ---- tensor maps for the staged sweeps -------------------------------------------------------
 
@@ -729,10 +758,27 @@ int set_tmp(const fdtd_llg *s, int par) {
   if (!s->merge) return 2;
   return s->opt.enable_llg ? (par ? 1 : 2) : 2;   // Maxwell-only: no sweep ever uses it
 }
-bool merge_allowed(const fdtd_llg *s) {
-  if (!s->opt.merge_h || s->has_pml) return false;
-  for (int q = 0; q < s->src.count; ++q)
-    if (s->src.s[q].kind == FDTD_LLG_SRC_SOFT_H || s->src.s[q].kind == FDTD_LLG_SRC_HARD_H) return false;
+// Can the H half-steps be merged (options.merge_h), and outside which margins?  The PML layer takes
+// two damped half-steps per step and an H source acts on H at integer time: their faces keep the
+// plain half-steps.  An H source box must lie within 8 cells of a side of the grid (the paper's
+// excitations sit on a wall plane), else nothing is merged.
+constexpr int UM_MAX = 8;
+bool decide_merge(fdtd_llg *s) {
+  for (int d = 0; d < 3; ++d) { s->um_lo[d] = s->opt.pml[2 * d]; s->um_hi[d] = s->opt.pml[2 * d + 1]; }
+  if (!s->opt.merge_h) return false;
+  for (int q = 0; q < s->src.count; ++q) {
+    const SourceP &S = s->src.s[q];
+    if (S.kind != FDTD_LLG_SRC_SOFT_H && S.kind != FDTD_LLG_SRC_HARD_H) continue;
+    int best = INT_MAX, bd = 0, bside = 0;
+    for (int d = 0; d < 3; ++d) {
+      if (S.hi[d] < best) { best = S.hi[d]; bd = d; bside = 0; }                         // from the low side
+      if (s->g.n[d] - S.lo[d] < best) { best = s->g.n[d] - S.lo[d]; bd = d; bside = 1; } // from the high side
+    }
+    if (best > std::max(UM_MAX, bside ? s->um_hi[bd] : s->um_lo[bd])) return false;
+    if (bside) s->um_hi[bd] = std::max(s->um_hi[bd], best); else s->um_lo[bd] = std::max(s->um_lo[bd], best);
+  }
+  for (int d = 0; d < 3; ++d)
+    if (s->um_lo[d] + s->um_hi[d] >= s->g.n[d]) return false;   // nothing left to merge
   return true;
 }
 
@@ -745,12 +791,18 @@ bool merge_allowed(const fdtd_llg *s) {
 struct ERegion {
   int lo[3], hi[3];
   bool staged, fuse;
+  int kind;   // 0: a slab of the complement of the sweep box (merged H: of the interior), 1: a piece of
+              // the unmerged margins, 2: the sweep box, 3: the whole grid (one direct-load launch)
 };
+constexpr int MAX_REG = 64;
+enum { OUT_ALL = 0, OUT_LEFTOVER = 1, OUT_MARGINS = 2 };
 int plan_e_regions(const fdtd_llg *s, ERegion *out);
 bool fold_bookkeeping(const fdtd_llg *s);
 int count_sources(const fdtd_llg *s, int kind);
+// which = OUT_ALL: every slab of box_out; OUT_LEFTOVER: those whose merged update the E phase did not
+// take along (not fused); OUT_MARGINS: the unmerged margins
 int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul, bool exports, int *launches,
-                    bool skip_fused = false) {
+                    int which = OUT_ALL) {
   const dim3 blk(TX, TY, 1);
   HArgs h{};
   h.g = s->g;
@@ -759,24 +811,22 @@ int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul,
   h.mu_r = s->mu_r.is_array ? s->mu_r.dev : nullptr;
   h.ch_uniform = s->dt / (2.0 * kMu0 * s->mu_r.uniform);
   h.cmul = cmul;
-  BoxP boxes[16];
-  int nb = 0;
-  if (!skip_fused) {
-    for (int b = 0; b < s->n_out; ++b) boxes[nb++] = s->box_out[b];
-  } else {  // the faces whose merged update the E phase did not take along
-    ERegion reg[16];
+  std::vector<BoxP> boxes;
+  if (which == OUT_MARGINS) {
+    boxes = s->box_um;
+  } else if (which == OUT_ALL) {
+    boxes.assign(s->box_out, s->box_out + s->n_out);
+  } else {
+    ERegion reg[MAX_REG];
     const int nr = plan_e_regions(s, reg);
-    const bool whole = nr == 1 && !reg[0].staged && reg[0].lo[0] == 0 && reg[0].hi[0] == s->g.n[0] &&
-                       reg[0].lo[1] == 0 && reg[0].hi[1] == s->g.n[1] && reg[0].lo[2] == 0 && reg[0].hi[2] == s->g.n[2];
-    if (whole) {
-      for (int b = 0; b < s->n_out; ++b) boxes[nb++] = s->box_out[b];
+    if (nr == 1 && reg[0].kind == 3) {
+      boxes.assign(s->box_out, s->box_out + s->n_out);
     } else {
-      const int nreg_out = nr - (s->llg ? 1 : 0);   // the last region is the sweep box
-      for (int r = 0; r < nreg_out; ++r)
-        if (!reg[r].fuse) boxes[nb++] = make_box(s, reg[r].lo, reg[r].hi);
+      for (int r = 0; r < nr; ++r)
+        if (reg[r].kind == 0 && !reg[r].fuse) boxes.push_back(make_box(s, reg[r].lo, reg[r].hi));
     }
   }
-  for (int b = 0; b < nb; ++b) {
+  for (size_t b = 0; b < boxes.size(); ++b) {
     h.box = boxes[b];
     if (h.box.items == 0) continue;
     const int grid = grid_for(s, h.box, 0);
@@ -796,8 +846,14 @@ int enqueue_outside(fdtd_llg *s, double *const *E, int in, int out, double cmul,
 // (PAPER.md:94), from the set the E update read into the set the next E update will read.
 int enqueue_half_pre(fdtd_llg *s, double *const *E, int in, int out, int merged_to, int *launches) {
   int rc = FDTD_LLG_OK;
-  if (!s->merge) rc = enqueue_outside(s, E, in, out, 1.0, true, launches);
-  else if (merged_to >= 0) rc = enqueue_outside(s, E, in, merged_to, 2.0, true, launches, true);
+  if (!s->merge) {
+    rc = enqueue_outside(s, E, in, out, 1.0, true, launches);
+  } else {
+    // the margins (PML layer, H-source planes) take the plain half-step; in a Maxwell-only handle
+    // `in` and `out` are the same set on odd steps: the update is pointwise, in place is fine
+    rc = enqueue_outside(s, E, in, out, 1.0, true, launches, OUT_MARGINS);
+    if (!rc && merged_to >= 0) rc = enqueue_outside(s, E, in, merged_to, 2.0, true, launches, OUT_LEFTOVER);
+  }
   if (rc) return rc;
   return enqueue_pml(s, false, E, s->Hset[out], launches);
 }
@@ -951,11 +1007,18 @@ int enqueue_e(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, co
 
 int plan_e_regions(const fdtd_llg *s, ERegion *out) {
   const int zero[3] = {0, 0, 0};
-  auto put = [&](int n, const int *lo, const int *hi, bool staged, bool fuse) {
+  auto put = [&](int n, const int *lo, const int *hi, bool staged, bool fuse, int kind) {
     for (int d = 0; d < 3; ++d) { out[n].lo[d] = lo[d]; out[n].hi[d] = hi[d]; }
     out[n].staged = staged;
     out[n].fuse = fuse;
+    out[n].kind = kind;
     return n + 1;
+  };
+  // a staged box begins on a 16-byte boundary, and its tiles (15 or 16 rows) must not be mostly empty:
+  // on a thin grid (the paper's ny = 4 guides) the direct-load kernels with their 1-, 2-, 4-row tiles do better
+  auto stageable = [&](const int *lo, const int *hi, int by) {
+    const int rows = hi[1] - lo[1], slots = (rows + by - 1) / by * by;
+    return (lo[0] & 1) == 0 && 5 * rows >= 3 * slots;
   };
   const bool can_fuse = s->merge && !s->mu_r.is_array && count_sources(s, FDTD_LLG_SRC_HARD_E) == 0;
   int n = 0;
@@ -964,27 +1027,30 @@ int plan_e_regions(const fdtd_llg *s, ERegion *out) {
     for (int b = 0; b < s->n_out; ++b) {
       const BoxP &B = s->box_out[b];
       if (B.items == 0) continue;
-      const bool st = (B.lo[0] & 1) == 0;   // staged boxes begin on 16-byte boundaries
+      const bool fu = can_fuse && stageable(B.lo, B.hi, FBY);
+      const bool st = fu || stageable(B.lo, B.hi, SBY);
       int hi[3] = {B.hi[0], B.hi[1], B.hi[2]};
-      if (st && can_fuse && s->g.ext[1] && hi[2] == s->g.n[2]) {
+      if (fu && s->g.ext[1] && hi[2] == s->g.n[2]) {
         // a slab's last plane needs E^{n+1} of the upper neighbour's first plane, which arrives with
         // that neighbour's E phase: its H update stays in the second half-step
         const int lo_top[3] = {B.lo[0], B.lo[1], std::max(B.lo[2], hi[2] - 1)};
-        n = put(n, lo_top, hi, false, false);
+        n = put(n, lo_top, hi, false, false, 0);
         hi[2] -= 1;
         if (hi[2] <= B.lo[2]) continue;
       }
-      n = put(n, B.lo, hi, st, st && can_fuse);
-      if (st) items += make_ehbox(s, B.lo, hi, st && can_fuse).items;
+      n = put(n, B.lo, hi, st, fu, 0);
+      if (st) items += make_ehbox(s, B.lo, hi, fu).items;
     }
+    for (size_t b = 0; b < s->box_um.size(); ++b)
+      if (s->box_um[b].items) n = put(n, s->box_um[b].lo, s->box_um[b].hi, false, false, 1);
     if (s->llg) {
-      const bool st = (s->lo[0] & 1) == 0;
-      n = put(n, s->lo, s->hi, st, false);
+      const bool st = stageable(s->lo, s->hi, SBY);
+      n = put(n, s->lo, s->hi, st, false, 2);
       if (st) items += make_ehbox(s, s->lo, s->hi, false).items;
     }
   }
   // a grid that cannot give every SM an item is latency bound: one direct-load launch serves it better
-  if (!s->eh_ok || (items < s->num_sms && s->opt.kernel_path != 5)) return put(0, zero, s->g.n, false, false);
+  if (!s->eh_ok || (items < s->num_sms && s->opt.kernel_path != 5)) return put(0, zero, s->g.n, false, false, 3);
   return n;
 }
 
@@ -992,13 +1058,13 @@ int plan_e_regions(const fdtd_llg *s, ERegion *out) {
 // also does the bookkeeping of the two H half-steps, and k_half_end is not launched (EHArgs::book)
 bool fold_bookkeeping(const fdtd_llg *s) {
   if (s->llg || s->has_pml) return false;
-  ERegion reg[16];
+  ERegion reg[MAX_REG];
   return plan_e_regions(s, reg) == 1 && reg[0].fuse;
 }
 
 int enqueue_e_regions(fdtd_llg *s, double *const *Ein, double *const *Eout, int hset, int hset_next, int par,
                       int *launches) {
-  ERegion reg[16];
+  ERegion reg[MAX_REG];
   const int nr = plan_e_regions(s, reg);
   const bool fold = fold_bookkeeping(s);
   int widx = 8 * par;   // the staged launches of a step draw from the eight counters of its parity
@@ -1145,6 +1211,10 @@ int reconstruct_h(fdtd_llg *s, int *read_set) {
   int launches = 0;
   int rc = enqueue_outside(s, e_set(s, par), dead, target, 1.0, false, &launches);
   if (rc) return rc;
+  // the margins hold H^N in set 0; a Maxwell-only handle reads from `target`: copy them over
+  // (the update with cmul = 0 is a copy)
+  if (target != 0) rc = enqueue_outside(s, e_set(s, par), 0, target, 0.0, false, &launches, OUT_MARGINS);
+  if (rc) return rc;
   s->recon_valid = true;
   return FDTD_LLG_OK;
 }
@@ -1163,6 +1233,7 @@ int unmerge(fdtd_llg *s) {
   s->primed = false;
   s->recon_valid = false;
   s->graph_valid[0] = s->graph_valid[1] = false;
+  make_boxes(s);
   return FDTD_LLG_OK;
 }
 
@@ -1335,7 +1406,8 @@ int fdtd_llg_create(fdtd_llg **out, int nx, int ny, int nz, double dx, double dy
   s->staged = s->llg && !s->alpha.is_array && !s->gamma.is_array && !s->mu_r.is_array &&
               (s->lo[0] & 1) == 0 && opt->kernel_path != 1;
   if (s->staged && (rc = setup_hm_stage(s))) return bail(rc);
-  s->merge = merge_allowed(s);
+  s->merge = decide_merge(s);
+  make_boxes(s);   // again: the merged region keeps out of the margins
   if (!s->has_pml && opt->kernel_path != 1 && (rc = setup_eh_stage(s))) return bail(rc);
   CUB(cudaStreamSynchronize(s->stream));
 #undef CUB
@@ -1473,6 +1545,11 @@ int fdtd_llg_add_source(fdtd_llg *s, int kind, int comp, const int *lo, const in
   }
   s->src.count++;
   s->graph_valid[0] = s->graph_valid[1] = false;  // the step's kernel arguments changed
+  if (kind == FDTD_LLG_SRC_SOFT_H || kind == FDTD_LLG_SRC_HARD_H) {
+    // (the state is at integer time now: unmerge above) merge again outside the margin this source needs
+    s->merge = decide_merge(s);
+    make_boxes(s);
+  }
   return FDTD_LLG_OK;
 }
 
@@ -1584,7 +1661,7 @@ int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out) {
   std::memset(out, 0, sizeof *out);
   out->merged_h = s->merge ? 1 : 0;
   {
-    ERegion reg[16];
+    ERegion reg[MAX_REG];
     const int nr = plan_e_regions(s, reg);
     for (int r = 0; r < nr; ++r)
       out->staged_maxwell = std::max(out->staged_maxwell, reg[r].fuse ? 2 : (reg[r].staged ? 1 : 0));

@@ -70,13 +70,6 @@ def _planes(plan: SlabPlan, nz_global: int) -> list:
     return ks
 
 
-def merge_ok(w) -> bool:
-    """merge_h is a property of the whole grid: a PML or an H source anywhere switches it off on the
-    handle that has it, and all slabs must agree (fdtd_llg_slab_connect checks)."""
-    pml = getattr(w, "pml", None)
-    return not (pml is not None and any(pml)) and not any(getattr(q, "kind", 0) in (2, 3) for q in w.sources)
-
-
 def cut_workload(w, plan: SlabPlan):
     """The slab-local workload: every array cut to the slab's planes plus the neighbours' adjacent
     planes, source boxes clipped to the slab (slab coordinates), the z boundary type kept only
@@ -95,7 +88,6 @@ def cut_workload(w, plan: SlabPlan):
         return t.index_select(0, torch.tensor(ks, device=t.device)).contiguous()
 
     s = copy.copy(w)
-    s.merge_ok = merge_ok(w)
     s.name = f"{w.name}[slab {plan.rank}/{plan.world}]"
     s.nz = plan.nz
     s.bc = (w.bc[0], w.bc[1], PEC)
@@ -155,7 +147,6 @@ def stack_copies(w, plan: SlabPlan):
         return torch.cat(parts, 0).contiguous()
 
     s = copy.copy(w)
-    s.merge_ok = merge_ok(w)
     s.name = f"{w.name}[copy {plan.rank} of {plan.world} stacked in z]"
     s.slab_ext = plan.ext
     s.materials = {k: ext(v, True) for k, v in w.materials.items()}
@@ -249,9 +240,17 @@ class LocalSlabs(SlabStepper):
         self.torch = torch
         self.plans = plan_slabs(w.nz, world, w.bc[2] == PERIODIC)
         self.stream = torch.cuda.Stream(device)
-        sims = [from_workload(cut_workload(w, p), device=device, stream=self.stream, use_graph=False,
-                              kernel_path=kernel_path, merge_h=merge_h and merge_ok(w), time_scheme=time_scheme,
-                              slab_ext=p.ext) for p in self.plans]
+        def make(merge):
+            return [from_workload(cut_workload(w, p), device=device, stream=self.stream, use_graph=False,
+                                  kernel_path=kernel_path, merge_h=merge, time_scheme=time_scheme,
+                                  slab_ext=p.ext) for p in self.plans]
+        sims = make(merge_h)
+        # merge_h is a property of the whole grid: a handle whose H source cannot be kept in a margin
+        # switches it off for itself; then nobody merges (fdtd_llg_slab_connect refuses a mismatch)
+        if len({s.stats()["merged_h"] for s in sims}) > 1:
+            for s in sims:
+                s.close()
+            sims = make(False)
         for p, s in zip(self.plans, sims):
             nb = [None if q is None else (sims[q].slab_info(), sims[q].workspace.data_ptr())
                   for q in (p.lo, p.hi)]
@@ -314,21 +313,31 @@ class DistSlab(SlabStepper):
         # workspace, mapping a neighbour's) is followed by a collective in which ALL ranks learn
         # whether it worked, so that a failure on one rank raises SlabSetupError on every rank
         # instead of leaving the others in a collective.
-        err, mine = None, None
-        try:
-            import os
-            if os.environ.get("FDTD_LLG_TEST_FAIL_RANK") == str(plan.rank):   # test hook: a rank that cannot set up
-                raise RuntimeError("FDTD_LLG_TEST_FAIL_RANK")
-            self.sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,
-                                     kernel_path=kernel_path, merge_h=merge_h and getattr(w, "merge_ok", True),
-                                     time_scheme=time_scheme, slab_ext=plan.ext)
-            if plan.world > 1:
-                mine = (self.sim.slab_info().as_tuple(),) + self.sim.ipc_export()
-        except Exception as e:          # noqa: BLE001  (reported to all ranks below)
-            err = e
-        if plan.world > 1:
-            everyone = [None] * plan.world
+        err, mine, everyone = None, None, [None] * plan.world
+        for merge in ((True, False) if merge_h else (False,)):
+            # merge_h is a property of the whole grid: if the slabs come out disagreeing (an H source
+            # that cannot be kept in a margin switches it off on the handle that has it), all are
+            # created again without it
+            try:
+                import os
+                if os.environ.get("FDTD_LLG_TEST_FAIL_RANK") == str(plan.rank):   # test hook: a rank that cannot set up
+                    raise RuntimeError("FDTD_LLG_TEST_FAIL_RANK")
+                if self.sim is not None:
+                    self.sim.close()
+                self.sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,
+                                         kernel_path=kernel_path, merge_h=merge, time_scheme=time_scheme,
+                                         slab_ext=plan.ext)
+                if plan.world > 1:
+                    mine = (self.sim.slab_info().as_tuple(),) + self.sim.ipc_export()
+            except Exception as e:          # noqa: BLE001  (reported to all ranks below)
+                err, mine = e, None
+            if plan.world == 1:
+                break
             dist.all_gather_object(everyone, mine, group=group)
+            states = {x[0][-1] for x in everyone if x is not None}     # SlabInfo.merged_h of every slab
+            if len(states) <= 1 or any(x is None for x in everyone):
+                break
+        if plan.world > 1:
             if err is None:
                 try:
                     nb = []

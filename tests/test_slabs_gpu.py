@@ -195,8 +195,8 @@ def test_two_processes_map_each_other_with_cuda_ipc(cfg, shape, tmp_path):
 def test_slabs_first_order_scheme_and_open_boundary_with_hard_h_source():
     """The other step variants across cuts: the first-order scheme (one explicit sweep per half-step),
     and the paper's tunable-filter set-up in small (PML at the z-low end, hard H source on the last
-    plane, LLG slab on a side wall, dielectric array: two H half-steps everywhere, k_pml on the end
-    slab only)."""
+    plane, LLG slab on a side wall, dielectric array: the H half-steps are merged outside the margins
+    -- the layer, the source plane -- and k_pml runs on the end slab only)."""
     from paper_2103_12819_b200.slabs import LocalSlabs
     w = wl.make_config(5, shape=(40, 44, 36))
     ref, st = _single(w, 10, time_scheme=1)
@@ -207,7 +207,7 @@ def test_slabs_first_order_scheme_and_open_boundary_with_hard_h_source():
         assert np.array_equal(got[n], ref[n]), n
     w = wl.paper_tunable_filter(nx=96, ny=4, nz=48, npml=8)
     ref, st = _single(w, 40)
-    assert st["merged_h"] == 0
+    assert st["merged_h"] == 1      # merged outside the margins: the PML layer and the source plane
     for world in (2, 3):
         grp = LocalSlabs(w, world)
         grp.step(40)
