@@ -525,6 +525,10 @@ int setup_hm_stage(fdtd_llg *s) {
   // the direct-load kernels with their 32 x 8 x 16 blocks fill the GPU better there (32^3: 9 us
   // against 79 us per sweep; the bits are the same).
   if (s->opt.kernel_path == 0 && s->st_box.items < s->num_sms) s->staged = false;
+  // ... and so is one whose 16-row tiles would be mostly empty (a box of a few rows: the paper's
+  // ny = 4 guides): the direct-load kernels have 1-, 2- and 4-row tiles
+  const int rows = s->hi[1] - s->lo[1], slots = (rows + SBY - 1) / SBY * SBY;
+  if (s->opt.kernel_path == 0 && 5 * rows < 3 * slots) s->staged = false;
   return FDTD_LLG_OK;
 }
 
