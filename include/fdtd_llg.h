@@ -238,8 +238,8 @@ int fdtd_llg_read_fields(fdtd_llg *s, double *const *E, double *const *H, double
 /* Statistics so far (synchronises the stream). */
 int fdtd_llg_get_stats(fdtd_llg *s, fdtd_llg_stats *out);
 
-/* Text of the last error on this handle; with s == NULL, of the last failed fdtd_llg_create on
- * this thread.  Never NULL. */
+/* Text of the last error on this handle; with s == NULL, of the last failed fdtd_llg_create (or
+ * other call that takes no handle) on this thread.  Never NULL. */
 const char *fdtd_llg_last_error(const fdtd_llg *s);
 
 /* Release the handle (host memory, graph).  The workspace stays the caller's.  NULL is a no-op. */
@@ -323,6 +323,56 @@ int fdtd_llg_residual_word(fdtd_llg *s, int r, void **dev_ptr);
 int fdtd_llg_ipc_export(fdtd_llg *s, unsigned char *handle64, unsigned long long *offset);
 int fdtd_llg_ipc_open(const unsigned char *handle64, unsigned long long offset, void **dev_ptr);
 int fdtd_llg_ipc_close(void *dev_ptr, unsigned long long offset);
+
+/* --------------------------------------------------------- A QUERY THAT ALLOCATES NOTHING AT ALL
+ * Where the magnet is, asked BEFORE a handle exists: the bounding box of the cells with Ms > 0 and
+ * their number -- what fdtd_llg_create finds out for itself (stats.magnetic_cells; stats.sweep_cells
+ * is this box plus the one-cell halo of the four-point averages) and what a caller
+ * wants earlier: to cut the grid into slabs that share the magnetic cells, to see whether a workload
+ * has an LLG part at all (+21 doubles per cell of workspace), to size the workspace it is about to
+ * reserve.
+ *
+ * WHO THIS IS FOR.  Everything else in this library works inside the workspace the caller hands to
+ * fdtd_llg_create, so it needs no allocation either -- but a caller with no handle yet has no
+ * workspace to lend, and some callers cannot get device memory on the spot: a host application that
+ * gave the whole GPU to its own memory pool at start-up (arena allocators of AMR frameworks such as the
+ * one the paper's code is built on; the caching allocators of ML runtimes), where a
+ * cudaMalloc from a library fails or fragments the pool; a time loop or a server thread that must not
+ * stall, for which cudaMalloc / cudaFree are off limits because they may wait for all work in flight on
+ * the device; code under a fixed memory budget that must not fail half-way.  For those callers this
+ * one entry point keeps its scratch (one partial result per thread block and a ticket word) in a
+ * fixed array that is part of the library's device image: FDTD_LLG_STATIC_SCRATCH_BYTES (1 MiB + 256 B)
+ * on every GPU that loads the library, from load to process exit, used by nothing else.  It calls no
+ * cudaMalloc, no cudaFree and no library routine that allocates device memory.
+ *
+ *   Ms    DEVICE, nx*ny*nz doubles, x fastest (the cell-centred map fdtd_llg_create takes), read only
+ *   nx, ny, nz >= 1 with nx*ny*nz <= FDTD_LLG_STATIC_MAX_CELLS (2^29: a 768^3 grid fits, 1024^3 does
+ *         not); beyond that EINVAL with a message that says so -- take the map in z ranges then and
+ *         merge the boxes
+ *   out7  DEVICE, 7 long long, written by the kernel: lo_x, lo_y, lo_z, hi_x, hi_y, hi_z (cell
+ *         indices, hi INCLUSIVE), count.  No magnetic cell: lo = (nx, ny, nz), hi = (-1, -1, -1), 0.
+ *         A NaN in the map is not magnetic (NaN > 0 is false), as in fdtd_llg_create's own scan
+ *   cuda_stream  a cudaStream_t of the CURRENT device (NULL = default stream); the call only enqueues
+ *         (one 256-byte memset of the ticket word and one kernel) and returns; out7 is valid once that
+ *         work has completed on the stream.
+ * Errors: EINVAL (NULL pointer, bad extent, too many cells), ECUDA; text through
+ * fdtd_llg_last_error(NULL) (the per-thread message of the handle-free calls).
+ *
+ * RULES THAT COME WITH A SHARED, FIXED ARRAY.
+ *  - The FIRST call on each device looks up the array's device address (once per device, under a
+ *    lock, with that device current); it may load the library's device code.  Make that first call
+ *    during set-up, before any stream capture is begun on the calling thread.
+ *  - Every call on a device uses the same array, and the array keeps what the previous call left.
+ *    The call clears the ticket word itself and overwrites every partial it later reads, so calls
+ *    one after the other -- on one stream, or ordered by events -- need no clean-up by the caller.
+ *    Two calls of one process that can be in flight on one GPU at the same time (streams without an
+ *    ordering between them, two host threads) RACE on the array and both results are garbage:
+ *    serialise them.  Separate processes do not share it: each has its own copy on the device.
+ *  - The stream's device must be the current device (as for any kernel launch). */
+#define FDTD_LLG_STATIC_MAX_CELLS (1LL << 29)
+#define FDTD_LLG_STATIC_SCRATCH_BYTES ((1 << 20) + 256)
+int fdtd_llg_magnetic_box_static(const double *Ms, int nx, int ny, int nz, long long *out7,
+                                 void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -66,7 +66,12 @@ EXPORTS = ("fdtd_llg_default_options", "fdtd_llg_workspace_bytes", "fdtd_llg_cre
            "fdtd_llg_read_fields",
            "fdtd_llg_get_stats", "fdtd_llg_last_error", "fdtd_llg_destroy",
            "fdtd_llg_get_slab_info", "fdtd_llg_slab_connect", "fdtd_llg_substep",
-           "fdtd_llg_residual_word", "fdtd_llg_ipc_export", "fdtd_llg_ipc_open", "fdtd_llg_ipc_close")
+           "fdtd_llg_residual_word", "fdtd_llg_ipc_export", "fdtd_llg_ipc_open", "fdtd_llg_ipc_close",
+           "fdtd_llg_magnetic_box_static")
+
+# limits of fdtd_llg_magnetic_box_static (fdtd_llg.h)
+STATIC_MAX_CELLS = 1 << 29
+STATIC_SCRATCH_BYTES = (1 << 20) + 256
 
 # sub-steps of one time step (fdtd_llg.h FDTD_LLG_SUB_*)
 SUB_BEGIN, SUB_HM1, SUB_HM1_END, SUB_E, SUB_HM2, SUB_HM2_END = range(6)
@@ -136,6 +141,8 @@ def lib() -> C.CDLL:
         L.fdtd_llg_ipc_open.restype = C.c_int
         L.fdtd_llg_ipc_close.argtypes = [_VP, C.c_ulonglong]
         L.fdtd_llg_ipc_close.restype = C.c_int
+        L.fdtd_llg_magnetic_box_static.argtypes = [_VP, C.c_int, C.c_int, C.c_int, _VP, _VP]
+        L.fdtd_llg_magnetic_box_static.restype = C.c_int
         _lib = L
     return _lib
 
@@ -402,6 +409,35 @@ def fdtd_llg_ipc_open(handle: bytes, offset: int) -> int:
 
 def fdtd_llg_ipc_close(ptr: int, offset: int) -> None:
     rc = lib().fdtd_llg_ipc_close(C.c_void_p(ptr), C.c_ulonglong(offset))
+    if rc != OK:
+        raise FdtdLlgError(rc, fdtd_llg_last_error(None))
+
+
+def fdtd_llg_magnetic_box_static(Ms, out7, stream=None) -> None:
+    """Bounding box and number of the cells with Ms > 0, for callers that must not allocate device
+    memory (a GPU handed over to the application's own memory pool, a loop that cannot afford the
+    device-wide wait an allocation may cost, a fixed memory budget): the kernel's scratch is a fixed
+    array inside the library, so neither the library nor this wrapper allocates anything.
+
+    ``Ms``: CUDA float64 tensor shaped (nz, ny, nx), contiguous, at most ``STATIC_MAX_CELLS`` cells;
+    ``out7``: CUDA int64 tensor of 7 entries on the same device, supplied by the caller, filled with
+    lo_x, lo_y, lo_z, hi_x, hi_y, hi_z (inclusive), count -- or (nx, ny, nz), (-1, -1, -1), 0 when no
+    cell is magnetic; ``stream``: a torch stream (default: the current one).  Only enqueues: read
+    ``out7`` in stream order.  Calls share the library's one scratch array per GPU: calls that could
+    run at the same time on one GPU race, keep them on one stream or order them.  The first call on
+    a device does a one-time address look-up; make it during set-up, before any stream capture."""
+    import torch
+    if not (isinstance(Ms, torch.Tensor) and Ms.is_cuda and Ms.dtype == torch.float64
+            and Ms.dim() == 3 and Ms.is_contiguous()):
+        raise ValueError("Ms must be a contiguous CUDA float64 tensor shaped (nz, ny, nx)")
+    if not (isinstance(out7, torch.Tensor) and out7.device == Ms.device and out7.dtype == torch.int64
+            and out7.numel() == 7 and out7.is_contiguous()):
+        raise ValueError("out7 must be a contiguous CUDA int64 tensor of 7 entries on Ms's device")
+    nz, ny, nx = Ms.shape
+    with torch.cuda.device(Ms.device):
+        st = stream if stream is not None else torch.cuda.current_stream(Ms.device)
+        rc = lib().fdtd_llg_magnetic_box_static(Ms.data_ptr(), nx, ny, nz, out7.data_ptr(),
+                                                st.cuda_stream)
     if rc != OK:
         raise FdtdLlgError(rc, fdtd_llg_last_error(None))
 

@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1851,3 +1852,171 @@ int fdtd_llg_ipc_close(void *dev_ptr, unsigned long long offset) {
 }
 
 }  // extern "C"
+
+// ================================================================================================
+// fdtd_llg_magnetic_box_static: the magnetic-cell scan for callers that cannot allocate
+// (include/fdtd_llg.h "A QUERY THAT ALLOCATES NOTHING AT ALL" says who they are and why).
+//
+// The scan inside fdtd_llg_create (k_mag_box above) works in the handle's workspace: the map is first
+// copied into the ghosted layout there and the box / count words it folds into with atomics live
+// there too.  A caller without a handle has no workspace, and the callers this variant is for may not
+// ask CUDA for one.  So the variant reads the caller's compact map directly and keeps its scratch --
+// one partial box + count per thread block, and the ticket that tells the last block to finish -- in
+// the fixed array below.  Array, kernel, address look-up and entry point sit in this one file because
+// the array has internal linkage (static): only this translation unit can name it.
+namespace {
+
+constexpr int SB_THREADS = 256;
+constexpr int SB_PER_THREAD = 64;
+constexpr long long SB_CHUNK = (long long)SB_THREADS * SB_PER_THREAD;          // cells per block
+constexpr long long SB_MAX_BLOCKS = FDTD_LLG_STATIC_MAX_CELLS / SB_CHUNK;      // 32768
+struct SbPartial { int lo[3]; int hi[3]; unsigned long long count; };          // 32 bytes
+constexpr size_t SB_HEAD = 256;   // the ticket word has the first 256 bytes to itself
+static_assert(sizeof(SbPartial) == 32, "partial record");
+static_assert(SB_HEAD + SB_MAX_BLOCKS * sizeof(SbPartial) == FDTD_LLG_STATIC_SCRATCH_BYTES,
+              "the header states the size of the static scratch");
+
+// The scratch.  Part of the library's device image: every GPU that loads the library holds these
+// bytes until the process exits.  In HOST code this name is only a stand-in for the symbol, NOT a
+// device address: handing it to a kernel makes the kernel fault or, where the GPU can reach host
+// memory, scribble over the wrong bytes without a word.  Host code gets the real address from
+// cudaGetSymbolAddress (static_scratch_address below) and passes that.
+static __device__ __align__(256) unsigned char g_static_scratch[FDTD_LLG_STATIC_SCRATCH_BYTES];
+
+// Block b scans cells [b * SB_CHUNK, (b + 1) * SB_CHUNK) of the compact map, leaves its partial in
+// scratch and takes a ticket; the block that draws the last ticket folds all partials into out7 and
+// puts the ticket word back to 0.  A partial is always written before it is read in the same launch,
+// so what an earlier call left in the array is never seen.
+__global__ void __launch_bounds__(SB_THREADS)
+k_mag_box_static(const double *__restrict__ Ms, int nx, int ny, int nz, long long n,
+                 unsigned char *scratch, long long *__restrict__ out7) {
+  unsigned *ticket = reinterpret_cast<unsigned *>(scratch);
+  SbPartial *part = reinterpret_cast<SbPartial *>(scratch + SB_HEAD);
+  int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {INT_MIN, INT_MIN, INT_MIN};
+  unsigned long long cnt = 0;
+
+  // (i, j, k) of this thread's first cell by division, of the following ones by adding the
+  // decomposition of the thread stride: 256 = si + nx * (sj + ny * sk)
+  long long t = (long long)blockIdx.x * SB_CHUNK + threadIdx.x;
+  int i = (int)(t % nx), j = (int)((t / nx) % ny), k = (int)(t / ((long long)nx * ny));
+  const int si = SB_THREADS % nx, sj = (SB_THREADS / nx) % ny, sk = SB_THREADS / nx / ny;
+  for (int m = 0; m < SB_PER_THREAD && t < n; ++m, t += SB_THREADS) {
+    if (Ms[t] > 0.0) {   // the test of k_mag_box: a NaN is not magnetic
+      lo[0] = min(lo[0], i); lo[1] = min(lo[1], j); lo[2] = min(lo[2], k);
+      hi[0] = max(hi[0], i); hi[1] = max(hi[1], j); hi[2] = max(hi[2], k);
+      ++cnt;
+    }
+    i += si;
+    if (i >= nx) { i -= nx; ++j; }
+    j += sj;
+    if (j >= ny) { j -= ny; ++k; }
+    k += sk;
+  }
+
+  __shared__ int s_lo[3][SB_THREADS / 32], s_hi[3][SB_THREADS / 32];
+  __shared__ unsigned long long s_cnt[SB_THREADS / 32];
+  __shared__ bool s_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  auto fold_block = [&]() {   // afterwards thread 0 holds the block's box and count
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        lo[d] = min(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+        hi[d] = max(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+      }
+      cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    }
+    if (lane == 0) {
+      for (int d = 0; d < 3; ++d) { s_lo[d][warp] = lo[d]; s_hi[d][warp] = hi[d]; }
+      s_cnt[warp] = cnt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0)
+      for (int w = 1; w < SB_THREADS / 32; ++w) {
+        for (int d = 0; d < 3; ++d) { lo[d] = min(lo[d], s_lo[d][w]); hi[d] = max(hi[d], s_hi[d][w]); }
+        cnt += s_cnt[w];
+      }
+  };
+
+  fold_block();
+  if (threadIdx.x == 0) {
+    SbPartial p;
+    for (int d = 0; d < 3; ++d) { p.lo[d] = lo[d]; p.hi[d] = hi[d]; }
+    p.count = cnt;
+    part[blockIdx.x] = p;
+    __threadfence();   // the partial is visible device-wide before the ticket is
+    s_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!s_last) return;
+
+  __threadfence();     // all other blocks' partials are visible to this block
+  for (int d = 0; d < 3; ++d) { lo[d] = INT_MAX; hi[d] = INT_MIN; }
+  cnt = 0;
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += SB_THREADS) {
+    const int4 a = __ldcg(reinterpret_cast<const int4 *>(part + b));       // lo x y z, hi x
+    const int4 c = __ldcg(reinterpret_cast<const int4 *>(part + b) + 1);   // hi y z, count
+    lo[0] = min(lo[0], a.x); lo[1] = min(lo[1], a.y); lo[2] = min(lo[2], a.z);
+    hi[0] = max(hi[0], a.w); hi[1] = max(hi[1], c.x); hi[2] = max(hi[2], c.y);
+    cnt += (unsigned long long)(unsigned)c.z | ((unsigned long long)(unsigned)c.w << 32);
+  }
+  __syncthreads();     // the shared arrays are reused
+  fold_block();
+  if (threadIdx.x == 0) {
+    const int nn[3] = {nx, ny, nz};
+    for (int d = 0; d < 3; ++d) {
+      out7[d] = cnt ? lo[d] : nn[d];
+      out7[3 + d] = cnt ? hi[d] : -1;
+    }
+    out7[6] = (long long)cnt;
+    *ticket = 0u;      // as the next call expects it (the entry point clears it as well)
+  }
+}
+
+// Device address of g_static_scratch on the CURRENT device: looked up on the first call per device
+// and kept.  (Each device has its own instance of a __device__ variable, hence one address per
+// device, asked for while that device is current.)
+constexpr int SB_MAX_DEVICES = 64;
+unsigned char *g_scratch_addr[SB_MAX_DEVICES] = {};
+std::mutex g_scratch_mutex;
+
+int static_scratch_address(unsigned char **out) {
+  int dev = -1;
+  CU(nullptr, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= SB_MAX_DEVICES)
+    return fail(nullptr, FDTD_LLG_EINVAL, "device ordinal %d is beyond the %d this call keeps addresses for", dev, SB_MAX_DEVICES);
+  std::lock_guard<std::mutex> lock(g_scratch_mutex);
+  if (!g_scratch_addr[dev]) {
+    void *p = nullptr;
+    CU(nullptr, cudaGetSymbolAddress(&p, g_static_scratch));
+    if (!p) return fail(nullptr, FDTD_LLG_ECUDA, "cudaGetSymbolAddress returned a NULL address");
+    g_scratch_addr[dev] = static_cast<unsigned char *>(p);
+  }
+  *out = g_scratch_addr[dev];
+  return FDTD_LLG_OK;
+}
+
+}  // namespace
+
+extern "C" int fdtd_llg_magnetic_box_static(const double *Ms, int nx, int ny, int nz,
+                                            long long *out7, void *cuda_stream) {
+  if (!Ms || !out7) return fail(nullptr, FDTD_LLG_EINVAL, "Ms and out7 must be DEVICE pointers, not NULL");
+  if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, FDTD_LLG_EINVAL, "nx, ny, nz must be >= 1");
+  const long long n = (long long)nx * ny * nz;
+  if (n > FDTD_LLG_STATIC_MAX_CELLS)
+    return fail(nullptr, FDTD_LLG_EINVAL,
+                "nx*ny*nz = %lld cells is more than the %lld the static scratch of this call is sized for "
+                "(FDTD_LLG_STATIC_MAX_CELLS): scan the map in z ranges and merge the boxes",
+                n, (long long)FDTD_LLG_STATIC_MAX_CELLS);
+  unsigned char *scratch = nullptr;
+  const int rc = static_scratch_address(&scratch);
+  if (rc) return rc;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  // the ticket must start at 0 whatever an earlier (perhaps aborted) call left behind
+  CU(nullptr, cudaMemsetAsync(scratch, 0, SB_HEAD, stream));
+  const unsigned blocks = (unsigned)((n + SB_CHUNK - 1) / SB_CHUNK);
+  k_mag_box_static<<<blocks, SB_THREADS, 0, stream>>>(Ms, nx, ny, nz, n, scratch, out7);
+  CU(nullptr, cudaGetLastError());
+  return FDTD_LLG_OK;
+}
