@@ -81,9 +81,15 @@ __device__ __forceinline__ void eh_issue_stage(const EHArgs &p, double *dst, uin
   if (SIG_ARR) tma_load_4d(dst + L::SG, &p.map, bar, x, y, z, p.aSig);
 }
 
-// soft sources on the D-edge of cell (i,j,k)
+// soft sources on the D-edge of cell (i,j,k).  The fused sweep recomputes
+// E^{n+1} on the high-side rim of a tile (row y0 + FBY, column x0 + SW, plane k1, the cells at T.hi of
+// a ragged tile); at the end of a PERIODIC axis that rim is index n, the image of index 0
+// (PAPER.md:185), and carries the current of the source at index 0
 template <int D>
 __device__ __forceinline__ double eh_source(const EHArgs &a, int i, int j, int k) {
+  if (a.g.per[0] && i == a.g.n[0]) i = 0;
+  if (a.g.per[1] && j == a.g.n[1]) j = 0;
+  if (a.g.per[2] && k == a.g.n[2]) k = 0;
   double J = 0.0;
   for (int s = 0; s < a.src.count; ++s) {
     const SourceP &S = a.src.s[s];
@@ -286,8 +292,8 @@ k_eh_fused(const __grid_constant__ EHArgs p) {
   double *const enew = ring + L::NS * S::STAGE;
   uint64_t *const full = reinterpret_cast<uint64_t *>(enew + L::ENEW);
   uint64_t *const empty = full + L::NS;
-  uint64_t *const efull = empty + L::NS;     // E^{n+1} plane b is complete (17 E warps arrive)
-  uint64_t *const eempty = efull + L::NEB;   // ... is no longer read (16 H warps arrive)
+  uint64_t *const efull = empty + L::NS;     // E^{n+1} plane b is complete (the NEW_ = FBY + 1 E warps arrive)
+  uint64_t *const eempty = efull + L::NEB;   // ... is no longer read (the NHW = FBY H warps arrive)
   int *const meta = reinterpret_cast<int *>(eempty + L::NEB);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from tests._util import FIELD_GROUPS, oracle_from_workload, record_parity, rel_linf
+from tests._util import FIELD_GROUPS, oracle_from_workload, record_parity, rel_linf, rel_linf_of_change
 from paper_2103_12819_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -44,6 +44,17 @@ def _assert_parity(got, ref, llg, tol=TOL, record=None):
     return errs
 
 
+def _assert_m_error_small_against_its_change(got, ref, w, tol=1e-6, **oracle_kw):
+    """|M| = Ms never moves, so an error of 1e-9 Ms says little about a run in which M turns by a
+    fraction of a radian: measure the error against how far M moved (a wrong damping or anisotropy
+    term shows here first)."""
+    ref0 = oracle_from_workload(w, **oracle_kw).read_fields()
+    assert max(float(np.max(np.abs(ref[n] - ref0[n]))) for n in FIELD_GROUPS["M"]) > 0   # M moved
+    e = rel_linf_of_change(got, ref, ref0, "M")
+    assert e <= tol, e
+    return e
+
+
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
 def test_parity_100_steps_all_configs(cfg):
     """On these shapes the default kernel_path picks the direct-load sweeps (the box is too small
@@ -68,6 +79,8 @@ def test_parity_100_steps_all_configs(cfg):
         assert gs["iters_total"] == int(os_["iters_total"])
         assert gs["nonconverged_halfsteps"] == 0
         assert gs["halfsteps"] == 200
+        _assert_m_error_small_against_its_change(got, ref, w)
+        _assert_m_error_small_against_its_change(_gpu_fields(sim), ref, w)
         # wall faces / non-magnetic faces carry exactly M = 0 on both sides
         for n in FIELD_GROUPS["M"]:
             assert np.array_equal(got[n] == 0.0, ref[n] == 0.0)
@@ -166,6 +179,45 @@ def test_fused_maxwell_sweep_equals_the_separate_kernels_bitwise(cfg, shape):
         assert np.array_equal(outs[0][n], outs[1][n]), (n, float(np.max(np.abs(outs[0][n] - outs[1][n]))))
 
 
+@pytest.mark.parametrize("cfg,shape", [(2, (40, 36, 28)), (2, (33, 31, 26)), (5, (40, 44, 36)), (5, (70, 19, 23))])
+def test_fused_sweep_carries_the_soft_current_onto_the_periodic_image(cfg, shape):
+    """A soft E source whose box touches index 0 of a periodic axis: the fused sweep recomputes
+    E^{n+1} at index n (the image of index 0) on the rim of its last tiles and must put
+    the same J there (eq. 11), or H at n-1 is built from an E without the current.
+    kernel_path 1 reads the stored ghost image instead: both must give the same bits, and the
+    oracle's values to 1e-9."""
+    from paper_2103_12819_b200.binding import from_workload
+    w = wl.make_config(cfg, shape=shape)
+    nx, ny, nz = shape
+    rng = np.random.default_rng(5)
+    f0, t0, tp = 3.0 / (40 * w.dt), 12 * w.dt, 5 * w.dt
+
+    def box_source(comp, lo, hi, amp):
+        nb = int(np.prod([h - l for l, h in zip(lo, hi)]))
+        return wl.Source(comp, lo, hi, amp, f0, t0, tp, profile=torch.from_numpy(0.5 + rng.random(nb)))
+
+    w.sources = list(w.sources) + [
+        box_source(0, (3, 0, 0), (nx - 2, 2, 3), 4e10),          # J_x from index 0 in y and z
+        box_source(1, (0, 2, 0), (3, ny - 1, 2), 3e10),          # J_y from index 0 in x and z
+        box_source(2, (0, 0, 1), (2, 3, nz - 1), 5e10),          # J_z from index 0 in x and y
+        wl.Source(2, (0, 0, 0), shape, 1e10, f0, t0, tp),        # everywhere, no profile
+    ]
+    outs = []
+    for path in (1, 5):
+        sim = from_workload(w, kernel_path=path)
+        st = sim.stats()
+        assert st["merged_h"] == 1
+        if path == 5:   # the fused sweep runs: everywhere (config 2) / outside the LLG box (config 5)
+            assert st["staged_maxwell"] == 2
+        sim.step(30)
+        outs.append(_gpu_fields(sim))
+    for n in outs[0]:
+        assert np.array_equal(outs[0][n], outs[1][n]), (n, float(np.max(np.abs(outs[0][n] - outs[1][n]))))
+    o = oracle_from_workload(w)
+    o.step(30)
+    _assert_parity(outs[1], o.read_fields(), w.enable_llg)
+
+
 def test_merged_h_equals_two_half_steps_to_rounding_and_reads_do_not_disturb():
     """merge_h: one update instead of two half-steps with the same curl E: equal up to rounding
     (1 ulp per step), and reading the fields mid-run (which forms the integer-time H) changes nothing."""
@@ -254,6 +306,7 @@ def test_first_order_scheme_parity_100_steps(cfg):
         assert st["iters_total"] == int(o.stats()["iters_total"]) == 200   # one sweep per half-step
         assert st["nonconverged_halfsteps"] == 0
     _assert_parity(outs[0], ref, True)
+    _assert_m_error_small_against_its_change(outs[0], ref, w, time_scheme=1)
     for other in outs[1:]:
         for n in outs[0]:
             assert np.array_equal(outs[0][n], other[n]), n
