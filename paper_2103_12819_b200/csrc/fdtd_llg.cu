@@ -776,8 +776,11 @@ bool decide_merge(fdtd_llg *s) {
     if (S.kind != FDTD_LLG_SRC_SOFT_H && S.kind != FDTD_LLG_SRC_HARD_H) continue;
     int best = INT_MAX, bd = 0, bside = 0;
     for (int d = 0; d < 3; ++d) {
-      if (S.hi[d] < best) { best = S.hi[d]; bd = d; bside = 0; }                         // from the low side
-      if (s->g.n[d] - S.lo[d] < best) { best = s->g.n[d] - S.lo[d]; bd = d; bside = 1; } // from the high side
+      // an interface to a neighbouring slab is not a side of the grid: the handle on the whole grid
+      // would not see one there, and the slabs must decide as it does (bit-for-bit contract)
+      const bool side_lo = !(d == 2 && s->g.ext[0]), side_hi = !(d == 2 && s->g.ext[1]);
+      if (side_lo && S.hi[d] < best) { best = S.hi[d]; bd = d; bside = 0; }                         // from the low side
+      if (side_hi && s->g.n[d] - S.lo[d] < best) { best = s->g.n[d] - S.lo[d]; bd = d; bside = 1; } // from the high side
     }
     if (best > std::max(UM_MAX, bside ? s->um_hi[bd] : s->um_lo[bd])) return false;
     if (bside) s->um_hi[bd] = std::max(s->um_hi[bd], best); else s->um_lo[bd] = std::max(s->um_lo[bd], best);
@@ -1062,7 +1065,9 @@ int plan_e_regions(const fdtd_llg *s, ERegion *out) {
 // A step without magnetic cells whose E phase is one fused launch over the whole grid: that launch
 // also does the bookkeeping of the two H half-steps, and k_half_end is not launched (EHArgs::book)
 bool fold_bookkeeping(const fdtd_llg *s) {
-  if (s->llg || s->has_pml) return false;
+  // not on a slab: its residual words receive the other slabs' maxima and k_half_end must clear them
+  // at the end of EVERY half-step, which one launch per step cannot do
+  if (s->llg || s->has_pml || s->is_slab) return false;
   ERegion reg[MAX_REG];
   return plan_e_regions(s, reg) == 1 && reg[0].fuse;
 }

@@ -564,12 +564,15 @@ __global__ void k_half_end(DevState *st, unsigned long long *resid, unsigned *wo
     if (R > st->iters_max) st->iters_max = R;
     st->resid_last = res;
     st->last_R_even = ((R & 1) == 0);
-    for (int r = 1; r <= max_iter; ++r) { resid[r] = 0ull; work[r] = 0u; }
-    work[0] = 0u;
   } else {
     st->iters_last = 0;
     st->last_R_even = 0;
   }
+  // Re-arm the residual words and item counters, magnetic faces or not: a slab WITHOUT magnetic faces
+  // still receives the maximum over all slabs in its words (the caller's max-allreduce writes it
+  // there, fdtd_llg.h "Z-SLABS") and would otherwise feed that value into every later maximum
+  for (int r = 1; r <= max_iter; ++r) { resid[r] = 0ull; work[r] = 0u; }
+  work[0] = 0u;
   r_hist[st->halfsteps % 4096] = st->iters_last;
   st->halfsteps++;
   if (last_of_step) st->steps++;

@@ -279,7 +279,10 @@ class LocalSlabs(SlabStepper):
                 x.copy_(m)
 
     def converged(self, r):
-        return float(self._word(r)[0].item()) < self.tol
+        # the word is written on self.stream (a non-blocking stream the default stream does not wait
+        # for): read it in that stream's order, or the host sees the re-armed 0 of a GPU that lags
+        with self.torch.cuda.stream(self.stream):
+            return float(self._word(r)[0].item()) < self.tol
 
     def read_fields(self, names=None) -> dict:
         """The global fields, slabs concatenated along z (host numpy arrays)."""

@@ -98,6 +98,31 @@ def test_slabs_hold_what_one_handle_holds_bit_for_bit(cfg, shape, world, path, m
     assert max(float(np.max(np.abs(ref[n]))) for n in FIELD_GROUPS["H"]) > 0
 
 
+def test_iteration_count_falls_again_with_slabs_that_hold_no_magnet():
+    """Config 4 on 24 x 20 x 40 at tol 1e-10: the pulse takes the iteration count from 2 to 3 and back
+    (the oracle's history of this workload), and three of the four slabs have no magnetic face.  Their
+    residual words receive the maximum over all slabs with every merge; unless the closing sub-step
+    clears them there too, the stopping test turns into a running maximum over the
+    past and the count never comes down again."""
+    from paper_2103_12819_b200.slabs import LocalSlabs
+    w = wl.make_config(4, shape=(24, 20, 40))
+    w.llg_tol = 1e-10
+    steps = 40
+    ref, st = _single(w, steps)
+    assert st["iters_max"] == 3 and 2 * 2 * steps < st["iters_total"] < 3 * 2 * steps   # 2, then 3, then 2
+    assert st["iters_last"] == 2
+    grp = LocalSlabs(w, 4)
+    its = [s.stats() for s in grp.sims]
+    assert [s["sweep_cells"] > 0 for s in its] == [True, False, False, False]
+    grp.step(steps)
+    got = grp.read_fields()
+    its = [s.stats() for s in grp.sims]
+    assert its[0]["iters_total"] == st["iters_total"] and its[0]["iters_last"] == 2
+    assert all(s["nonconverged_halfsteps"] == 0 for s in its)
+    for n in ALL:
+        assert np.array_equal(got[n], ref[n]), (n, float(np.max(np.abs(got[n] - ref[n]))))
+
+
 @pytest.mark.parametrize("bc", [(1, 0, 1), (0, 1, 0), (1, 1, 1)])
 def test_slabs_with_every_material_array_and_sources_across_the_cuts(bc):
     from paper_2103_12819_b200.slabs import LocalSlabs
