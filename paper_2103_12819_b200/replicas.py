@@ -1,10 +1,10 @@
 """Host-side plumbing of multi-process runs (one process per GPU, ``torch.distributed``).
 
-The hot path is single-GPU by scope: N processes advance N independent
-replicas and exchange nothing on the data path.  What is shared is the measurement protocol of
-``bench.py``: a barrier on both sides of the timed region, the MAX over ranks of the device time,
-and the whole-job rate = all ranks' cell updates / that time.  These helpers work on any backend
-(``nccl`` on GPUs, ``gloo`` in the CPU tests).
+The timing protocol ``bench.py`` uses at N > 1, whatever the ranks run -- the z-slabs of one grid
+(``slabs.py``, the default) or, when the slab set-up fails, N independent replicas (labelled as such,
+no headline value): a barrier on both sides of the timed region, the MAX over ranks of the device
+time, and the whole-job rate = all ranks' cell updates / that time.  These helpers work on any
+backend (``nccl`` on GPUs, ``gloo`` in the CPU tests) and hold none of the method's arithmetic.
 """
 from __future__ import annotations
 

@@ -322,9 +322,6 @@ class DistSlab(SlabStepper):
             # that cannot be kept in a margin switches it off on the handle that has it), all are
             # created again without it
             try:
-                import os
-                if os.environ.get("FDTD_LLG_TEST_FAIL_RANK") == str(plan.rank):   # test hook: a rank that cannot set up
-                    raise RuntimeError("FDTD_LLG_TEST_FAIL_RANK")
                 if self.sim is not None:
                     self.sim.close()
                 self.sim = from_workload(w, device=self.device, stream=self.stream, use_graph=False,

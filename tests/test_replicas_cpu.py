@@ -1,6 +1,6 @@
-"""The N > 1 path of bench.py on CPU: two gloo processes, each standing for one GPU's replica.
-The data path has no collective (replicas only); what the ranks share is
-the timing protocol -- barrier, MAX over ranks, whole-job rate."""
+"""The timing protocol of bench.py's N > 1 path on CPU: two gloo processes -- barrier, MAX over
+ranks, whole-job rate (paper_2103_12819_b200/replicas.py).  What the ranks run between the barriers
+(z-slabs of one grid, tests/test_slabs_cpu.py and test_slabs_gpu.py) is not this file's subject."""
 import os
 import socket
 
