@@ -15,6 +15,7 @@ on the default kernel path with CUDA-graph replay (the launch configuration benc
 Every measured error goes to the parity record (tests/_util.record_parity).
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -65,16 +66,38 @@ def test_100_steps_full_size_every_element(cfg):
     assert rec["err_E"] <= TOL and rec["err_H"] <= TOL, rec
 
 
-@pytest.mark.parametrize("cfg,shape", [(4, SHAPE_4), (5, SHAPE_5)])
+SHAPE_4_STAGED = (230, 200, 144)   # config 4's structure on a box wide enough that the DEFAULT path picks the
+                                   # staged LLG sweeps (8 x 13 ragged tiles x 2 z chunks = 208 work items >= 148
+                                   # SMs), as at the 384^3 bench.py times (that size itself: the slow test below)
+
+
+@pytest.mark.parametrize("cfg,shape", [(4, SHAPE_4), (5, SHAPE_5), (4, SHAPE_4_STAGED)])
 def test_100_steps_coupled_structure_at_size(cfg, shape):
     w, rec, st, got, ref = _run(cfg, shape)
     assert st["steps"] == 100 and st["nonconverged_halfsteps"] == 0
     assert rec["iters"] == rec["iters_oracle"] > 0
-    if cfg == 5:
+    if cfg == 5 or shape == SHAPE_4_STAGED:
         assert st["staged_sweeps"] == 1
     assert rec["err_E"] <= TOL and rec["err_H"] <= TOL and rec["err_M"] <= TOL, rec
     # M moved (the comparison is not one of two untouched arrays) and the error is small against
     # the movement too: a wrong damping or anisotropy term would show here first
+    assert rec["err_M_over_change"] <= 1e-6, rec
+    for n in FIELD_GROUPS["M"]:
+        assert np.array_equal(got[n] == 0.0, ref[n] == 0.0)
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("FDTD_LLG_FULL_PARITY") != "1",
+                    reason="config 4 at its full 384^3 for 100 steps: ~20 min of the oracle on 16 cores and ~20 GB of "
+                           "host memory; run once per round with FDTD_LLG_FULL_PARITY=1, result in profiles/parity_r03.md")
+def test_100_steps_config4_full_size_every_element():
+    """BASELINE.json configs[3] at its full size, in the launch configuration bench.py times (default
+    path: staged LLG sweeps, staged + fused Maxwell sweeps, CUDA-graph replay), all elements."""
+    w, rec, st, got, ref = _run(4, None)
+    assert (w.nx, w.ny, w.nz) == (384, 384, 384)
+    assert st["steps"] == 100 and st["nonconverged_halfsteps"] == 0 and st["staged_sweeps"] == 1
+    assert rec["iters"] == rec["iters_oracle"] > 0
+    assert rec["err_E"] <= TOL and rec["err_H"] <= TOL and rec["err_M"] <= TOL, rec
     assert rec["err_M_over_change"] <= 1e-6, rec
     for n in FIELD_GROUPS["M"]:
         assert np.array_equal(got[n] == 0.0, ref[n] == 0.0)
